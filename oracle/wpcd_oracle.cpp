@@ -1,0 +1,497 @@
+// wpcd_oracle.cpp -- CPU ORACLE for the WPCD hot path (arXiv:2106.00454).  TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, fp64, obviously-correct restatement of what the hot path computes, written from
+// /root/reference/PAPER.md (cited as PAPER.md:<line>) and the readings C1..C16 / G1..G3 of SURVEY.md section 8(c)
+// (restated in DESIGN.md).  It shares NO code with the CUDA library under paper_2106_00454_b200/csrc and must only
+// be imported / linked / executed by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+// legs.  No BLAS, no LAPACK, no blocking, no fusion: every function follows the paper's order and notation.
+//
+// Parity pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
+//   gl_rule          : weights sum to 2, exact on monomials to degree 2n-1, vs numpy.polynomial.legendre.leggauss
+//   legendre_Q       : vs mpmath.legenq (independent arbitrary-precision evaluation) and the Neumann integral
+//   V_yukawa         : vs adaptive quadrature of the radial (r-space) definition on tiny grids
+//   jacobi           : closed-form 2x2/3x3, rank-one secular equation by bisection (Yamaguchi), invariants, mpmath
+//   resolvent / T    : limits of Eq. B.3-B.6, sum rule, hand-evaluated tiny cases
+//   phases           : closed forms of Eqs. A.3-A.5 (unit-modulus S built from known angles)
+//   MI solver        : Yamaguchi analytic phase shifts; unitarity
+//   whole WPCD chain : converges to MI as N grows
+//   The paper prints no matrix, eigenvalue or phase shift for a reproducible input (its potential, NNLO_opt, is
+//   not available), so no value of the chain is pinned to a PAPER-PRINTED number: "parity unpinned by the paper
+//   itself"; the pins above are closed forms / independent evaluations instead.
+//
+// Units: momenta fm^-1, energies MeV, hbarc = 197.327 MeV fm, mu = 469.46 MeV; E = cE p^2, cE = hbarc^2/(2 mu).
+// Bins are 0-based: bin i spans [p_i, p_{i+1}], i = 0..N-1.  All matrices row-major.
+
+#include <cmath>
+#include <complex>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef std::complex<double> cplx;
+static const double PI = 3.14159265358979323846264338327950288;
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Gauss-Legendre rule on [-1,1]: nodes = roots of P_n by Newton, weights 2/((1-x^2) P_n'(x)^2).
+// Used for the bin integrals of Eq. 29 (the paper only says "quadrature", PAPER.md:229;
+// BASELINE.json fixes 8 points per bin) and for the MI grid.
+void orc_gl_rule(int n, double* x, double* w) {
+  for (int i = 0; i < n; ++i) {
+    double z = std::cos(PI * (i + 0.75) / (n + 0.5));  // Tricomi-type initial guess
+    double pp = 0.0;
+    for (int it = 0; it < 100; ++it) {
+      double p0 = 1.0, p1 = z;  // P_0, P_1
+      for (int k = 2; k <= n; ++k) {
+        double pk = ((2.0 * k - 1.0) * z * p1 - (k - 1.0) * p0) / k;
+        p0 = p1; p1 = pk;
+      }
+      if (n == 0) p1 = 1.0;
+      pp = n * (z * p1 - p0) / (z * z - 1.0);  // P_n'(z)
+      double dz = p1 / pp;
+      z -= dz;
+      if (std::fabs(dz) < 1e-16) break;
+    }
+    // recompute derivative at the converged node
+    double p0 = 1.0, p1 = z;
+    for (int k = 2; k <= n; ++k) {
+      double pk = ((2.0 * k - 1.0) * z * p1 - (k - 1.0) * p0) / k;
+      p0 = p1; p1 = pk;
+    }
+    pp = n * (z * p1 - p0) / (z * z - 1.0);
+    x[n - 1 - i] = z;  // ascending
+    w[n - 1 - i] = 2.0 / ((1.0 - z * z) * pp * pp);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Legendre function of the second kind Q_l(z), z > 1, l >= 0 (reading C7; not in the paper, which defers the
+// partial-wave projection to its ref. [26]).  int_0^inf r^2 dr j_l(k'r) (e^{-mu r}/r) j_l(kr)
+// = Q_l(z)/(2k'k), z = (k'^2+k^2+mu^2)/(2k'k).
+//   z <= zstar : Q_0 = 0.5*log1p(2/(z-1)),  Q_1 = z Q_0 - 1,  (l+1) Q_{l+1} = (2l+1) z Q_l - l Q_{l-1}   (upward)
+//   z >  zstar : Q_l = sqrt(pi) Gamma(l+1)/(Gamma(l+3/2) (2z)^{l+1}) * 2F1((l+1)/2,(l+2)/2; l+3/2; z^-2)  (series)
+// zstar = 1.1 (SURVEY proposed 1.5; 1.1 keeps the upward recurrence's error growth below ~1e-14 for l <= 5 while
+// the series still converges geometrically with ratio z^-2 <= 0.83; reading C7).
+double orc_legendre_Q(int l, double z) {
+  const double zstar = 1.1;
+  double q0 = 0.5 * std::log1p(2.0 / (z - 1.0));
+  if (l == 0) return q0;
+  if (z <= zstar) {
+    double qm = q0, q = z * q0 - 1.0;
+    for (int k = 1; k < l; ++k) {
+      double qn = ((2.0 * k + 1.0) * z * q - k * qm) / (k + 1.0);
+      qm = q; q = qn;
+    }
+    return q;
+  }
+  // prefactor sqrt(pi) Gamma(l+1)/Gamma(l+3/2) = 2^{l+1} l! / (2l+1)!!  ->  pref/(2z)^{l+1} = l!/((2l+1)!! z^{l+1})
+  double pref = 1.0;
+  for (int k = 1; k <= l; ++k) pref *= (double)k / (2.0 * k + 1.0);
+  double a = 0.5 * (l + 1.0), b = 0.5 * (l + 2.0), c = l + 1.5, x = 1.0 / (z * z);
+  double term = 1.0, sum = 1.0;
+  for (int k = 0; k < 2000; ++k) {
+    term *= (a + k) * (b + k) / ((c + k) * (k + 1.0)) * x;
+    sum += term;
+    if (term < 1e-18 * sum) break;
+  }
+  return pref * sum / std::pow(z, l + 1);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Step (i).  Config grid of BASELINE.json: p_i = alpha tan(pi i/(2N+1)), i = 0..N (row a0).
+void orc_grid_tan(int N, double alpha, double* p) {
+  for (int i = 0; i <= N; ++i) p[i] = alpha * std::tan(PI * i / (2.0 * N + 1.0));
+}
+
+// Free wave-packet (f(k)=1, N_i = Delta k_i, Eq. 17) kinetic energies and bin energy widths.
+// Reading C4: exact matrix element <x_i|h0|x_i> = cE (p_i^2 + p_i p_{i+1} + p_{i+1}^2)/3, not Eq. 18's midpoint.
+// Eedge_i = cE p_i^2 (E = p^2/m_N, m_N = 2 mu), dE_i = Eedge_{i+1} - Eedge_i.
+void orc_fwp(int N, const double* p, double hbarc, double mu, double* e0, double* dE, double* Eedge) {
+  double cE = hbarc * hbarc / (2.0 * mu);
+  for (int i = 0; i <= N; ++i) Eedge[i] = cE * p[i] * p[i];
+  for (int i = 0; i < N; ++i) {
+    e0[i] = cE * (p[i] * p[i] + p[i] * p[i + 1] + p[i + 1] * p[i + 1]) / 3.0;
+    dE[i] = Eedge[i + 1] - Eedge[i];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Eq. 29 with f=1, N_i = Delta k_i, convention B (reading C1):
+//   <k'|v_l|k>_B = (1/pi) sum_t V0_t Q_l(z_t)/(k'k),  z_t = (k'^2+k^2+mu_t^2)/(2k'k)
+//   V_ij = (1/(pi sqrt(Dk_i Dk_j))) sum_ab w_ia w_jb sum_t V0_t Q_l(z_t(k_ia,k_jb)),  n_gl points per bin.
+// Upper triangle computed, mirrored (bit-symmetric).
+void orc_V_yukawa(int N, const double* p, int l, int nterms, const double* V0, const double* mu, int ngl, double* V) {
+  std::vector<double> x(ngl), w(ngl);
+  orc_gl_rule(ngl, x.data(), w.data());
+  std::vector<double> k(N * ngl), om(N * ngl);
+  for (int i = 0; i < N; ++i)
+    for (int a = 0; a < ngl; ++a) {
+      double dk = p[i + 1] - p[i];
+      k[i * ngl + a] = 0.5 * (p[i] + p[i + 1]) + 0.5 * dk * x[a];
+      om[i * ngl + a] = 0.5 * dk * w[a];
+    }
+  for (int i = 0; i < N; ++i)
+    for (int j = i; j < N; ++j) {
+      double acc = 0.0;
+      for (int a = 0; a < ngl; ++a)
+        for (int b = 0; b < ngl; ++b) {
+          double kp = k[i * ngl + a], kk = k[j * ngl + b];
+          double s = 0.0;
+          for (int t = 0; t < nterms; ++t) {
+            double z = (kp * kp + kk * kk + mu[t] * mu[t]) / (2.0 * kp * kk);
+            s += V0[t] * orc_legendre_Q(l, z);
+          }
+          acc += om[i * ngl + a] * om[j * ngl + b] * s;
+        }
+      double v = acc / (PI * std::sqrt((p[i + 1] - p[i]) * (p[j + 1] - p[j])));
+      V[i * N + j] = v;
+      V[j * N + i] = v;
+    }
+}
+
+// Separable Yamaguchi potential (reading C15): <k'|v|k>_B = -lambdaB g(k') g(k), g(k) = 1/(k^2+beta^2)
+//   V_ij = -lambdaB G_i G_j,  G_i = Dk_i^{-1/2} int_{D_i} k g(k) dk.
+// closed_form != 0: G_i = 0.5 ln((p_{i+1}^2+beta^2)/(p_i^2+beta^2))/sqrt(Dk_i); else n_gl-point Gauss-Legendre.
+void orc_V_yamaguchi(int N, const double* p, double lambdaB, double beta, int ngl, int closed_form, double* V, double* G) {
+  std::vector<double> x(ngl), w(ngl);
+  orc_gl_rule(ngl, x.data(), w.data());
+  for (int i = 0; i < N; ++i) {
+    double dk = p[i + 1] - p[i];
+    if (closed_form) {
+      G[i] = 0.5 * std::log((p[i + 1] * p[i + 1] + beta * beta) / (p[i] * p[i] + beta * beta)) / std::sqrt(dk);
+    } else {
+      double acc = 0.0;
+      for (int a = 0; a < ngl; ++a) {
+        double k = 0.5 * (p[i] + p[i + 1]) + 0.5 * dk * x[a];
+        acc += 0.5 * dk * w[a] * k / (k * k + beta * beta);
+      }
+      G[i] = acc / std::sqrt(dk);
+    }
+  }
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) V[i * N + j] = -lambdaB * G[i] * G[j];
+}
+
+// H = H0 + V.  Uncoupled: n = N, H = diag(e0) + Vmm.  Coupled (degenerate FWP bases,
+// the same H0 in both blocks): n = 2N, H = [[H0 + Vmm, Vmp],[Vmp^T, H0 + Vpp]].  Also returns V (same layout).
+void orc_assemble_H(int N, int coupled, const double* e0, const double* Vmm, const double* Vpp, const double* Vmp,
+                    double* H, double* V) {
+  int n = coupled ? 2 * N : N;
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) {
+      int bi = i / N, bj = j / N, ii = i % N, jj = j % N;
+      double v;
+      if (bi == 0 && bj == 0) v = Vmm[ii * N + jj];
+      else if (bi == 1 && bj == 1) v = Vpp[ii * N + jj];
+      else if (bi == 0 && bj == 1) v = Vmp[ii * N + jj];
+      else v = Vmp[jj * N + ii];
+      V[i * n + j] = v;
+      H[i * n + j] = v + ((i == j) ? e0[ii] : 0.0);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Step (ii), Eq. 21: H = C D C^T by cyclic-by-row two-sided Jacobi (oracle step 4 of SURVEY 8(c)):
+//   theta = (a_qq - a_pp)/(2 a_pq), t = sgn(theta)/(|theta| + sqrt(theta^2+1)), c = 1/sqrt(t^2+1), s = t c;
+//   stop when a sweep starts with off(A) <= tol * ||A||_F  (tol = 1e-15 by default), eigenvalues = diagonal,
+//   sorted ascending together with the columns of C.  Returns the number of sweeps done (or -1 if max_sweeps hit).
+int orc_jacobi(int n, const double* Ain, double* W, double* C, double tol, int max_sweeps) {
+  std::vector<double> A(Ain, Ain + (size_t)n * n), V((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i) V[(size_t)i * n + i] = 1.0;
+  int sweeps = 0;
+  bool converged = false;
+  for (;;) {
+    double off = 0.0, fro = 0.0;
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) {
+        double a = A[(size_t)i * n + j];
+        fro += a * a;
+        if (i != j) off += a * a;
+      }
+    if (std::sqrt(off) <= tol * std::sqrt(fro)) { converged = true; break; }
+    if (sweeps >= max_sweeps) break;
+    for (int p = 0; p < n - 1; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        double apq = A[(size_t)p * n + q];
+        if (apq == 0.0) continue;
+        double app = A[(size_t)p * n + p], aqq = A[(size_t)q * n + q];
+        double theta = (aqq - app) / (2.0 * apq);
+        double t = (theta >= 0.0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+        double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
+        for (int k = 0; k < n; ++k) {  // columns p,q:  A <- A J
+          double akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
+          A[(size_t)k * n + p] = c * akp - s * akq;
+          A[(size_t)k * n + q] = s * akp + c * akq;
+        }
+        for (int k = 0; k < n; ++k) {  // rows p,q:  A <- J^T A
+          double apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
+          A[(size_t)p * n + k] = c * apk - s * aqk;
+          A[(size_t)q * n + k] = s * apk + c * aqk;
+        }
+        // the rotated pivot is zero by construction; diagonal by the stable update
+        A[(size_t)p * n + p] = app - t * apq;
+        A[(size_t)q * n + q] = aqq + t * apq;
+        A[(size_t)p * n + q] = 0.0;
+        A[(size_t)q * n + p] = 0.0;
+        for (int k = 0; k < n; ++k) {  // eigenvectors: V <- V J
+          double vkp = V[(size_t)k * n + p], vkq = V[(size_t)k * n + q];
+          V[(size_t)k * n + p] = c * vkp - s * vkq;
+          V[(size_t)k * n + q] = s * vkp + c * vkq;
+        }
+      }
+    ++sweeps;
+  }
+  std::vector<int> idx(n);
+  for (int i = 0; i < n; ++i) idx[i] = i;
+  std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return A[(size_t)a * n + a] < A[(size_t)b * n + b]; });
+  for (int k = 0; k < n; ++k) {
+    W[k] = A[(size_t)idx[k] * n + idx[k]];
+    for (int i = 0; i < n; ++i) C[(size_t)i * n + k] = V[(size_t)i * n + idx[k]];
+  }
+  return converged ? sweeps : -1;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Step (iii), Eq. 23, taken as printed (reading C5), for one branch of m positive eigenvalues
+// eps[0..m-1] (ascending): edge[0] = 0, edge[i] = (eps[i-1]+eps[i])/2, edge[m] = eps[m-1] + (edge[m-1]-edge[m-2])/2.
+// (m == 1: edge[1] = 2 eps[0], so that Eq. 22 holds.)
+void orc_swp_edges(int m, const double* eps, double* edge) {
+  if (m <= 0) return;
+  edge[0] = 0.0;
+  for (int i = 1; i < m; ++i) edge[i] = 0.5 * (eps[i - 1] + eps[i]);
+  if (m == 1) edge[1] = 2.0 * eps[0];
+  else edge[m] = eps[m - 1] + 0.5 * (edge[m - 1] - edge[m - 2]);
+}
+
+// Appendix B, Eqs. B.3-B.6 with the sign of the printed last line corrected (reading G2):
+//   Re g_k(E) = ln|(E - lo)/(E - hi)|/(hi - lo),  Im g_k(E) = -pi/(hi - lo) iff lo <= E < hi  (half-open, C11).
+cplx orc_resolvent(double E, double lo, double hi) {
+  double w = hi - lo;
+  double re = std::log(std::fabs((E - lo) / (E - hi))) / w;
+  double im = (E >= lo && E < hi) ? -PI / w : 0.0;
+  return cplx(re, im);
+}
+void orc_resolvent_c(double E, double lo, double hi, double* out) {
+  cplx g = orc_resolvent(E, lo, hi);
+  out[0] = g.real(); out[1] = g.imag();
+}
+
+// Steps (iv)-(v): Eq. 32 / Eq. 39 / Eq. 27, point-wise resolvent.
+//   uncoupled: T_ii(E) = V_ii + sum_b (VC)_ib^2/(E-eps_b) + sum_k (VC)_ik^2 g_k(E),  i = FWP bin with
+//              Eedge_i <= E < Eedge_{i+1};   out T[e] (re,im), bin[e] = i (or -1 if E is outside the grid: T = 0)
+//   coupled  : rows (alpha,i) -> alpha*N+i; T^{ab} = V_{(a i)(b i)} + sum_k (VC)_{(a i)k} g_k (VC)_{(b i)k};
+//              positive eigenvalues alternate between two branches by rank (reading C6), each branch with its own
+//              Eq. 23 edges; out T[e][a][b] (re,im).
+// W ascending, C columns = eigenvectors (as returned by orc_jacobi).  VC by the plain triple loop.
+void orc_onshell_T(int N, int coupled, const double* Eedge, const double* V, const double* W, const double* C,
+                   const double* Ecm, int nE, double* T, int* bin) {
+  int n = coupled ? 2 * N : N;
+  std::vector<double> VC((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      double s = 0.0;
+      for (int j = 0; j < n; ++j) s += V[(size_t)i * n + j] * C[(size_t)j * n + k];
+      VC[(size_t)i * n + k] = s;
+    }
+  int nb = 0;
+  while (nb < n && W[nb] < 0.0) ++nb;
+  int nbranch = coupled ? 2 : 1;
+  std::vector<std::vector<int>> members(nbranch);
+  for (int k = nb; k < n; ++k) members[(k - nb) % nbranch].push_back(k);
+  std::vector<double> lo(n, 0.0), hi(n, 0.0);
+  for (int br = 0; br < nbranch; ++br) {
+    int m = (int)members[br].size();
+    if (m == 0) continue;
+    std::vector<double> eps(m), edge(m + 1);
+    for (int i = 0; i < m; ++i) eps[i] = W[members[br][i]];
+    orc_swp_edges(m, eps.data(), edge.data());
+    for (int i = 0; i < m; ++i) { lo[members[br][i]] = edge[i]; hi[members[br][i]] = edge[i + 1]; }
+  }
+  int nc = coupled ? 2 : 1;
+  for (int e = 0; e < nE; ++e) {
+    double E = Ecm[e];
+    int ib = -1;
+    for (int i = 0; i < N; ++i)
+      if (E >= Eedge[i] && E < Eedge[i + 1]) { ib = i; break; }
+    bin[e] = ib;
+    for (int a = 0; a < nc; ++a)
+      for (int b = 0; b < nc; ++b) {
+        cplx t(0.0, 0.0);
+        if (ib >= 0) {
+          int ra = a * N + ib, rb = b * N + ib;
+          t = cplx(V[(size_t)ra * n + rb], 0.0);
+          for (int k = 0; k < nb; ++k) t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] / (E - W[k]);
+          for (int k = nb; k < n; ++k) t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] * orc_resolvent(E, lo[k], hi[k]);
+        }
+        size_t o = ((size_t)e * nc * nc + a * nc + b) * 2;
+        T[o] = t.real(); T[o + 1] = t.imag();
+      }
+  }
+}
+
+// Eqs. A.3-A.5 with the wave-packet normalisation of readings C2/A20:
+//   S = 1 - 2 pi i T_ii(E)/dE_i  (dE_i = FWP bin energy width)
+//   uncoupled: delta = 0.5 atan2(Im S, Re S) in degrees, in (-90, 90]; absS = |S|
+//   coupled (Stapp): delta_- = 0.5 arg S_11, delta_+ = 0.5 arg S_22,
+//                    sin 2eps = Re[-i S_12 e^{-i(delta_- + delta_+)}], cos 2eps = |S_11|, eps = 0.5 atan2(sin, cos)
+//   out delta[e] or delta[e][3] = (delta_-, delta_+, eps) in degrees; S[e] or S[e][2][2] (re,im) if S != NULL.
+void orc_phase_shifts(int coupled, int nE, const double* T, const int* bin, const double* dE, double* delta, double* S) {
+  const double deg = 180.0 / PI;
+  int nc = coupled ? 2 : 1;
+  for (int e = 0; e < nE; ++e) {
+    cplx s[2][2];
+    double w = (bin[e] >= 0) ? dE[bin[e]] : 1.0;
+    for (int a = 0; a < nc; ++a)
+      for (int b = 0; b < nc; ++b) {
+        size_t o = ((size_t)e * nc * nc + a * nc + b) * 2;
+        cplx t(T[o], T[o + 1]);
+        s[a][b] = (a == b ? 1.0 : 0.0) - cplx(0.0, 2.0 * PI) * t / w;
+        if (S) { S[o] = s[a][b].real(); S[o + 1] = s[a][b].imag(); }
+      }
+    if (!coupled) {
+      delta[e] = 0.5 * std::atan2(s[0][0].imag(), s[0][0].real()) * deg;
+    } else {
+      double dm = 0.5 * std::atan2(s[0][0].imag(), s[0][0].real());
+      double dp = 0.5 * std::atan2(s[1][1].imag(), s[1][1].real());
+      cplx r = cplx(0.0, -1.0) * s[0][1] * std::exp(cplx(0.0, -(dm + dp)));
+      double ep = 0.5 * std::atan2(r.real(), std::abs(s[0][0]));
+      delta[3 * e] = dm * deg; delta[3 * e + 1] = dp * deg; delta[3 * e + 2] = ep * deg;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Independent matrix-inversion (MI) Lippmann-Schwinger solver, Sec. 2.1, Eqs. 2-7 with D derived
+// from Eqs. 2-4 directly (reading C3/G1: the printed Eq. 5 is inconsistent):
+//   grid: GL nodes x_j on [-1,1] mapped k_j = c tan(pi(1+x_j)/4), w_j -> c (pi/4) w_j / cos^2(pi(1+x_j)/4), c = 1
+//   f = 2 mu/hbarc^2;   D_j = (2/pi) w_j k_j^2 f/(p^2-k_j^2);   D_{NQ+1} = -(2/pi) f p^2 sum_j w_j/(p^2-k_j^2) - i f p
+//   F = 1 - V diag(D)  (Eq. 7), solve F T = V (Eq. 6) by complex Gauss elimination with partial pivoting,
+//   on-shell T = element(s) at the on-shell index;  S = 1 - 2 i f p T  (conv. A, reading C2).
+// The potential is given by callback-free tables: vtab[(a*nc+b)][i][j] = v_A^{ab}(q_i,q_j) on the basis
+// q = {k_1..k_NQ, p}, prepared by orc_mi_potential_* below (convention A: v = sum_t V0_t Q_l(z_t)/(2k'k)).
+static void gauss_solve(int n, std::vector<cplx>& A, std::vector<cplx>& B, int nrhs) {
+  for (int c = 0; c < n; ++c) {
+    int piv = c; double best = std::abs(A[(size_t)c * n + c]);
+    for (int r = c + 1; r < n; ++r) { double v = std::abs(A[(size_t)r * n + c]); if (v > best) { best = v; piv = r; } }
+    if (piv != c) {
+      for (int k = 0; k < n; ++k) std::swap(A[(size_t)c * n + k], A[(size_t)piv * n + k]);
+      for (int k = 0; k < nrhs; ++k) std::swap(B[(size_t)c * nrhs + k], B[(size_t)piv * nrhs + k]);
+    }
+    for (int r = c + 1; r < n; ++r) {
+      cplx m = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+      if (m == cplx(0.0, 0.0)) continue;
+      for (int k = c; k < n; ++k) A[(size_t)r * n + k] -= m * A[(size_t)c * n + k];
+      for (int k = 0; k < nrhs; ++k) B[(size_t)r * nrhs + k] -= m * B[(size_t)c * nrhs + k];
+    }
+  }
+  for (int r = n - 1; r >= 0; --r)
+    for (int k = 0; k < nrhs; ++k) {
+      cplx s = B[(size_t)r * nrhs + k];
+      for (int c = r + 1; c < n; ++c) s -= A[(size_t)r * n + c] * B[(size_t)c * nrhs + k];
+      B[(size_t)r * nrhs + k] = s / A[(size_t)r * n + r];
+    }
+}
+
+void orc_mi_grid(int NQ, double cmap, double* k, double* w) {
+  std::vector<double> x(NQ), wx(NQ);
+  orc_gl_rule(NQ, x.data(), wx.data());
+  for (int j = 0; j < NQ; ++j) {
+    double ang = PI * (1.0 + x[j]) / 4.0;
+    k[j] = cmap * std::tan(ang);
+    w[j] = cmap * (PI / 4.0) * wx[j] / (std::cos(ang) * std::cos(ang));
+  }
+}
+
+// potential kinds for MI:  kind 0 = Yukawa sum (central terms V0/mu for block l; coupled: blocks l=J-1, J+1 with the
+// same central terms and the off-diagonal block V_T Q_J(z)/(2k'k), reading C8);  kind 1 = Yamaguchi -lambdaA g g.
+static double vA_yukawa(int l, int nterms, const double* V0, const double* mu, double kp, double k) {
+  double s = 0.0;
+  for (int t = 0; t < nterms; ++t) {
+    double z = (kp * kp + k * k + mu[t] * mu[t]) / (2.0 * kp * k);
+    s += V0[t] * orc_legendre_Q(l, z);
+  }
+  return s / (2.0 * kp * k);
+}
+
+// Solve at one lab energy.  out S (nc x nc complex, re/im interleaved), T likewise.
+void orc_mi_solve(int kind, int coupled, int l_or_J, int nterms, const double* V0, const double* mu, double VT, double muT,
+                  double lambdaA, double beta, double hbarc, double mured, int NQ, double Tlab, double* Sout, double* Tout) {
+  double p = std::sqrt(mured * Tlab) / hbarc;  // p = sqrt(mu T_lab)/hbarc (equal masses), E_cm = T_lab/2
+  double f = 2.0 * mured / (hbarc * hbarc);
+  std::vector<double> k(NQ), w(NQ);
+  orc_mi_grid(NQ, 1.0, k.data(), w.data());
+  int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M;
+  std::vector<double> q(M);
+  for (int j = 0; j < NQ; ++j) q[j] = k[j];
+  q[NQ] = p;
+  std::vector<cplx> D(M);
+  double ssum = 0.0;
+  for (int j = 0; j < NQ; ++j) {
+    D[j] = (2.0 / PI) * w[j] * k[j] * k[j] * f / (p * p - k[j] * k[j]);
+    ssum += w[j] / (p * p - k[j] * k[j]);
+  }
+  D[NQ] = cplx(-(2.0 / PI) * f * p * p * ssum, -f * p);
+  std::vector<cplx> Vm((size_t)n * n), F((size_t)n * n), B((size_t)n * nc);
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b)
+      for (int i = 0; i < M; ++i)
+        for (int j = 0; j < M; ++j) {
+          double v;
+          if (kind == 1) v = -lambdaA / ((q[i] * q[i] + beta * beta) * (q[j] * q[j] + beta * beta));
+          else if (!coupled) v = vA_yukawa(l_or_J, nterms, V0, mu, q[i], q[j]);
+          else if (a == b) v = vA_yukawa(a == 0 ? l_or_J - 1 : l_or_J + 1, nterms, V0, mu, q[i], q[j]);
+          else v = vA_yukawa(l_or_J, 1, &VT, &muT, q[i], q[j]);
+          Vm[(size_t)(a * M + i) * n + (b * M + j)] = v;
+        }
+  for (int r = 0; r < n; ++r)
+    for (int c = 0; c < n; ++c) F[(size_t)r * n + c] = (r == c ? 1.0 : 0.0) - Vm[(size_t)r * n + c] * D[c % M];
+  for (int r = 0; r < n; ++r)
+    for (int b = 0; b < nc; ++b) B[(size_t)r * nc + b] = Vm[(size_t)r * n + (b * M + NQ)];
+  gauss_solve(n, F, B, nc);
+  for (int a = 0; a < nc; ++a)
+    for (int b = 0; b < nc; ++b) {
+      cplx t = B[(size_t)(a * M + NQ) * nc + b];
+      cplx s = (a == b ? 1.0 : 0.0) - cplx(0.0, 2.0 * f * p) * t;
+      Tout[(a * nc + b) * 2] = t.real(); Tout[(a * nc + b) * 2 + 1] = t.imag();
+      Sout[(a * nc + b) * 2] = s.real(); Sout[(a * nc + b) * 2 + 1] = s.imag();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Whole chain for a batch of (sample, channel) solves, OpenMP over the batch (used only for timing the oracle as the
+// reported CPU baseline and by tests that need many solves).  Per solve b: H_b (n x n) and V_b are given
+// (assembled by orc_V_yukawa/orc_assemble_H), outputs W, C, T, delta.  Returns max sweeps (or -1).
+int orc_solve_batch(int N, int coupled, int batch, const double* Eedge, const double* dE, const double* H, const double* V,
+                    const double* Ecm, int nE, double tol, int max_sweeps, double* W, double* C, double* T, int* bin,
+                    double* delta, double* S, int* sweeps_out) {
+  int n = coupled ? 2 * N : N, nc = coupled ? 2 : 1, worst = 0;
+#pragma omp parallel for schedule(dynamic) reduction(max : worst)
+  for (int b = 0; b < batch; ++b) {
+    std::vector<int> binl(nE);
+    int sw = orc_jacobi(n, H + (size_t)b * n * n, W + (size_t)b * n, C + (size_t)b * n * n, tol, max_sweeps);
+    orc_onshell_T(N, coupled, Eedge, V + (size_t)b * n * n, W + (size_t)b * n, C + (size_t)b * n * n, Ecm, nE,
+                  T + (size_t)b * nE * nc * nc * 2, binl.data());
+    orc_phase_shifts(coupled, nE, T + (size_t)b * nE * nc * nc * 2, binl.data(), dE,
+                     delta + (size_t)b * nE * (coupled ? 3 : 1), S ? S + (size_t)b * nE * nc * nc * 2 : nullptr);
+    if (b == 0) std::memcpy(bin, binl.data(), sizeof(int) * nE);
+    if (sweeps_out) sweeps_out[b] = sw;
+    int swv = sw < 0 ? 1000000 : sw;
+    if (swv > worst) worst = swv;
+  }
+  return worst >= 1000000 ? -1 : worst;
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

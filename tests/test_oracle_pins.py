@@ -1,0 +1,412 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these re-types the oracle's own formula: each compares against an independent evaluation (mpmath arbitrary
+precision, scipy adaptive quadrature of the defining integral, closed forms, bisection of a secular equation,
+invariants, limits).
+"""
+import math
+
+import mpmath as mp
+import numpy as np
+import pytest
+from scipy import integrate
+
+from oracle import oracle as o
+from paper_2106_00454_b200 import inputs as inp
+
+MT = dict(V0=inp.MT_V0, mu=inp.MT_MU)
+
+
+# ---------------------------------------------------------------- P7: Gauss-Legendre rule
+@pytest.mark.parametrize("n", [1, 2, 5, 8, 24, 96])
+def test_gl_rule(n):
+    x, w = o.gl_rule(n)
+    assert abs(w.sum() - 2.0) < 1e-14
+    for d in range(0, 2 * n):  # exact for monomials up to degree 2n-1
+        exact = 0.0 if d % 2 else 2.0 / (d + 1)
+        assert abs(np.dot(w, x ** d) - exact) < 2e-14
+    xr, wr = np.polynomial.legendre.leggauss(n)
+    assert np.abs(x - xr).max() < 1e-14 and np.abs(w - wr).max() < 1e-14
+
+
+# ---------------------------------------------------------------- P8: Legendre Q_l (reading C7)
+def test_legendre_Q_vs_mpmath():
+    mp.mp.dps = 40
+    zs = np.concatenate([1.0 + np.logspace(-5, 7, 61), [1.0999999, 1.1, 1.1000001, 1.5]])
+    for l in range(0, 7):
+        for z in zs:
+            ref = float(mp.legenq(l, 0, mp.mpf(float(z)), type=3).real)
+            assert abs(o.legendre_Q(l, float(z)) / ref - 1.0) < 1e-12, (l, z)
+
+
+def test_legendre_Q_neumann_integral():
+    # Neumann's formula Q_l(z) = 1/2 int_{-1}^{1} P_l(t)/(z-t) dt, by scipy adaptive quadrature
+    from scipy.special import eval_legendre
+    for l in range(0, 6):
+        for z in [1.05, 1.3, 2.0, 7.0]:
+            val, _ = integrate.quad(lambda t: 0.5 * eval_legendre(l, t) / (z - t), -1, 1, epsabs=1e-14, epsrel=1e-13, limit=200)
+            assert abs(o.legendre_Q(l, z) - val) < 1e-11 * max(1.0, abs(val)), (l, z)
+
+
+def test_Q_is_the_yukawa_partial_wave():
+    # int_0^inf r^2 dr j_l(k'r) e^{-mu r}/r j_l(kr) = Q_l(z)/(2k'k)   (defining relation used by reading C7/C1)
+    mp.mp.dps = 30
+    for l, kp, k, mu in [(0, 0.7, 1.3, 1.55), (1, 0.5, 0.9, 3.11), (2, 1.1, 0.8, 2.0)]:
+        f = lambda r: r * mp.exp(-mu * r) * mp.besselj(l + 0.5, kp * r) * mp.besselj(l + 0.5, k * r) * mp.pi / (2 * mp.sqrt(kp * k) * r)
+        val = mp.quad(f, mp.linspace(0, 40, 81))
+        z = (kp * kp + k * k + mu * mu) / (2 * kp * k)
+        assert abs(o.legendre_Q(l, z) / (2 * kp * k) - float(val)) < 1e-10
+
+
+# ---------------------------------------------------------------- a0: grid and free wave packets
+def test_grid_and_fwp():
+    N = 50
+    p = o.grid_tan(N, 1.0)
+    assert np.abs(p - inp.grid_edges(N)).max() < 1e-13 * p[-1]
+    assert abs(p[50] - 64.29) < 0.01          # p_50 = 64.29 fm^-1
+    e0, dE, Ee = o.fwp(p)
+    cE = inp.HBARC ** 2 / (2 * inp.MU)
+    # <x_i|h0|x_i> = (1/Dk) int_{D_i} cE k^2 dk  (Eq. 17 with f=1) by adaptive quadrature
+    for i in [0, 7, 49]:
+        val, _ = integrate.quad(lambda k: cE * k * k, p[i], p[i + 1])
+        assert abs(e0[i] - val / (p[i + 1] - p[i])) < 1e-12 * e0[i]
+    assert np.allclose(np.cumsum(dE), Ee[1:], rtol=1e-13)
+
+
+# ---------------------------------------------------------------- a1: bin-averaged potential, Eq. 29
+def test_V_yukawa_vs_adaptive_double_integral():
+    # tiny grid, smooth region: 8x8 GL must agree with scipy's adaptive dblquad of Eq. 29 (conv. B, f=1, N_i=Dk_i)
+    p = np.array([0.4, 0.9, 1.5, 2.4])
+    for l in (0, 2):
+        V = o.V_yukawa(p, l, **MT)
+        assert np.array_equal(V, V.T)
+        for i, j in [(0, 0), (0, 2), (1, 2)]:
+            def integrand(k, kp):
+                s = 0.0
+                for V0, mu in zip(inp.MT_V0, inp.MT_MU):
+                    z = (kp * kp + k * k + mu * mu) / (2 * kp * k)
+                    s += V0 * float(mp.legenq(l, 0, z, type=3).real)
+                return s / math.pi
+            val, _ = integrate.dblquad(integrand, p[i], p[i + 1], p[j], p[j + 1], epsabs=1e-10, epsrel=1e-10)
+            ref = val / math.sqrt((p[i + 1] - p[i]) * (p[j + 1] - p[j]))
+            assert abs(V[i, j] - ref) < 2e-6 * abs(ref), (l, i, j, V[i, j], ref)
+
+
+def test_V_yamaguchi_closed_form_vs_gl():
+    p = inp.grid_edges(50)
+    lamA, lamB = inp.yamaguchi_lambda()
+    assert abs(lamA - 238.3487) < 1e-3 and abs(lamB - 151.7375) < 1e-3
+    V1, G1 = o.V_yamaguchi(p, lamB, inp.YAMAGUCHI_BETA, closed_form=True)
+    V2, G2 = o.V_yamaguchi(p, lamB, inp.YAMAGUCHI_BETA, closed_form=False)
+    assert np.abs(G1 - G2).max() < 1e-8
+    for i in (0, 10, 49):
+        val, _ = integrate.quad(lambda k: k / (k * k + inp.YAMAGUCHI_BETA ** 2), p[i], p[i + 1])
+        assert abs(G1[i] - val / math.sqrt(p[i + 1] - p[i])) < 1e-13
+    assert np.allclose(V1, -lamB * np.outer(G1, G1), rtol=1e-15)
+
+
+def test_assemble_coupled_layout():
+    N = 3
+    e0 = np.array([1.0, 2.0, 3.0])
+    Vmm = np.arange(9.0).reshape(3, 3); Vmm = Vmm + Vmm.T
+    Vpp = 10 + Vmm
+    Vmp = np.arange(9.0).reshape(3, 3) * 0.1
+    H, V = o.assemble_H(e0, Vmm, Vpp, Vmp)
+    ref = np.block([[Vmm, Vmp], [Vmp.T, Vpp]])
+    assert np.array_equal(V, ref)
+    assert np.array_equal(H, ref + np.diag(np.concatenate([e0, e0])))
+
+
+# ---------------------------------------------------------------- a2: Jacobi (P2, P3, P10)
+def test_jacobi_2x2_and_3x3_closed_form():
+    W, C, sw = o.jacobi(np.array([[2.0, 1.0], [1.0, 2.0]]))
+    assert np.allclose(W, [1.0, 3.0], atol=1e-15) and sw >= 1
+    assert np.allclose(np.abs(C), 1 / math.sqrt(2), atol=1e-15)
+    # tridiagonal Toeplitz (2,-1): eigenvalues 2 - 2 cos(k pi/(n+1))
+    n = 3
+    A = 2 * np.eye(n) - np.eye(n, k=1) - np.eye(n, k=-1)
+    W, C, _ = o.jacobi(A)
+    assert np.allclose(W, 2 - 2 * np.cos(np.arange(1, n + 1) * math.pi / (n + 1)), atol=1e-15)
+    n = 12
+    A = 2 * np.eye(n) - np.eye(n, k=1) - np.eye(n, k=-1)
+    W, C, _ = o.jacobi(A)
+    assert np.allclose(W, 2 - 2 * np.cos(np.arange(1, n + 1) * math.pi / (n + 1)), atol=4e-15)
+    # eigenvector k of the Toeplitz matrix is sin(i k pi/(n+1)) up to sign/norm: pins the column <-> eigenvalue order
+    for k in range(n):
+        v = np.sin(np.arange(1, n + 1) * (k + 1) * math.pi / (n + 1)); v /= np.linalg.norm(v)
+        assert min(np.abs(C[:, k] - v).max(), np.abs(C[:, k] + v).max()) < 1e-14
+
+
+def _mt_H(N, l=0):
+    p = inp.grid_edges(N)
+    e0, dE, Ee = o.fwp(p)
+    V = o.V_yukawa(p, l, **MT)
+    H, Vf = o.assemble_H(e0, V)
+    return p, e0, dE, Ee, H, Vf
+
+
+def test_jacobi_invariants_P3():
+    for N in (50, 100):
+        p, e0, dE, Ee, H, V = _mt_H(N)
+        W, C, sw = o.jacobi(H)
+        assert 1 <= sw <= 12
+        assert np.all(np.diff(W) >= 0)
+        assert np.abs(C.T @ C - np.eye(N)).max() < 1e-12
+        assert abs(np.trace(H) - W.sum()) < 1e-13 * np.abs(W).sum()
+        assert abs((H * H).sum() - (W * W).sum()) < 1e-13 * (W * W).sum()
+        assert np.abs(H @ C - C * W).max() < 1e-13 * np.abs(W).max()
+
+
+def test_jacobi_componentwise_vs_mpmath():
+    # reading C12: componentwise accuracy on a strongly graded H (N=24, MT potential), 50-digit reference
+    N = 24
+    p, e0, dE, Ee, H, V = _mt_H(N)
+    mp.mp.dps = 50
+    ref = sorted(float(x) for x in mp.eigsy(mp.matrix(H.tolist()), eigvals_only=True))
+    W, C, _ = o.jacobi(H)
+    assert np.abs(W / np.array(ref) - 1).max() < 1e-13
+
+
+def test_jacobi_rank_one_secular_P2():
+    # Yamaguchi H = diag(e) - lamB G G^T: eigenvalues are the roots of 1 = lamB sum_i G_i^2/(e_i - x); the bound
+    # state lies below e_0 and one root lies in each (e_{i-1}, e_i): bisection in 60-digit arithmetic.
+    N = 40
+    p = inp.grid_edges(N)
+    e0, dE, Ee = o.fwp(p)
+    lamA, lamB = inp.yamaguchi_lambda()
+    V, G = o.V_yamaguchi(p, lamB * 1.5, inp.YAMAGUCHI_BETA)  # x1.5: make it bind, so the x < e_0 root is exercised
+    H, _ = o.assemble_H(e0, V)
+    W, C, _ = o.jacobi(H)
+    mp.mp.dps = 60
+    e = [mp.mpf(float(x)) for x in e0]; g2 = [mp.mpf(float(x)) ** 2 for x in G]; lam = mp.mpf(float(lamB * 1.5))
+    f = lambda x: 1 - lam * sum(gi / (ei - x) for gi, ei in zip(g2, e))
+    roots = []
+    brackets = [(e[0] - 1e6, e[0])] + [(e[i - 1], e[i]) for i in range(1, N)]
+    for lo, hi in brackets:
+        w = hi - lo
+        a, b = lo + w * mp.mpf(10) ** -40, hi - w * mp.mpf(10) ** -40
+        fa, fb = f(a), f(b)
+        if fa * fb > 0:
+            continue
+        for _ in range(200):
+            m = (a + b) / 2
+            fm = f(m)
+            if fa * fm <= 0: b, fb = m, fm
+            else: a, fa = m, fm
+        roots.append(float((a + b) / 2))
+    assert len(roots) == N
+    assert roots[0] < 0 < roots[1]
+    assert np.abs(W / np.array(sorted(roots)) - 1).max() < 1e-13
+
+
+# ---------------------------------------------------------------- a3: Eq. 23
+def test_swp_edges_hand_values():
+    e = o.swp_edges(np.array([1.0, 3.0, 7.0]))
+    # E1=0, E2=(1+3)/2, E3=(3+7)/2, E4 = 7 + (E3-E2)/2 as printed (reading C5)
+    assert np.allclose(e, [0.0, 2.0, 5.0, 8.5], atol=0)
+    assert np.allclose(o.swp_edges(np.array([2.0])), [0.0, 4.0])
+    assert np.allclose(o.swp_edges(np.array([2.0, 4.0])), [0.0, 3.0, 5.5])
+
+
+# ---------------------------------------------------------------- a4: resolvent limits (P6) and T
+def test_resolvent_limits_P6():
+    lo, hi = 10.0, 10.5
+    g = o.resolvent(10.2, lo, hi)
+    assert abs(g.imag + math.pi / 0.5) < 1e-14          # Im g = -pi/width inside
+    assert o.resolvent(9.9, lo, hi).imag == 0.0 and o.resolvent(10.5, lo, hi).imag == 0.0  # half-open
+    assert o.resolvent(10.0, lo, hi + 1).imag != 0.0
+    # far away: narrow bin -> 1/(E - eps)   (from B.3 with the integrand constant over the bin)
+    for E in (200.0, -50.0, 0.3):
+        g = o.resolvent(E, lo, hi)
+        assert abs(g.real - 1 / (E - 10.25)) < 2e-3 * abs(1 / (E - 10.25)) ** 2 + 1e-6
+        assert abs(g.real * (E - 10.25) - 1) < 1e-3
+    # B.3 by adaptive principal-value-free quadrature for E outside the bin: (1/w) int_lo^hi dE'/(E - E')
+    for E in (3.0, 11.0, 40.0):
+        val, _ = integrate.quad(lambda x: 1 / (E - x), lo, hi)
+        assert abs(o.resolvent(E, lo, hi).real - val / 0.5) < 1e-12
+    # inside the bin: principal value
+    val, _ = integrate.quad(lambda x: 1.0, lo, hi, weight="cauchy", wvar=10.2)
+    assert abs(o.resolvent(10.2, lo, hi).real - (-val) / 0.5) < 1e-10
+
+
+def test_T_sum_rule_and_ImT():
+    N = 50
+    p, e0, dE, Ee, H, V = _mt_H(N)
+    W, C, _ = o.jacobi(H)
+    tl, Ecm = inp.energies(100)
+    T, b = o.onshell_T(N, False, Ee, V, W, C, Ecm)
+    assert b.min() == 3 and b.max() == 35      # on-shell bins 3..35 at N=50
+    nb = int((W < 0).sum()); assert nb == 1
+    edges = o.swp_edges(W[nb:])
+    VC = V @ C
+    for e in (0, 17, 99):
+        E = Ecm[e]
+        k = np.searchsorted(edges, E, side="right") - 1      # SWP bin containing E
+        # Im T = -pi (VC)_ik^2/width_k : only the bin containing E contributes an imaginary part
+        assert abs(T[e].imag - (-math.pi * VC[b[e], nb + k] ** 2 / (edges[k + 1] - edges[k]))) < 1e-12 * abs(T[e].imag)
+        # sum rule: sum_k width_k Im g_k(E) = -pi
+        s = sum((edges[j + 1] - edges[j]) * o.resolvent(E, edges[j], edges[j + 1]).imag for j in range(len(edges) - 1))
+        assert abs(s + math.pi) < 1e-12
+
+
+def test_T_tiny_case_by_hand():
+    # N=2, diagonal V => C = 1, eigenvalues = H diagonal; T_ii = V_ii + V_ii^2 g_i(E): checked with python complex math
+    Ee = np.array([0.0, 4.0, 10.0])
+    V = np.diag([0.5, -0.25]); H = np.diag([2.0, 7.0]) + V
+    W, C, _ = o.jacobi(H)
+    assert np.allclose(W, [2.5, 6.75]) and np.allclose(np.abs(C), np.eye(2))
+    T, b = o.onshell_T(2, False, Ee, V, W, C, np.array([1.0, 5.0, 12.0]))
+    assert list(b) == [0, 1, -1] and T[2] == 0
+    ed = [0.0, (2.5 + 6.75) / 2, 6.75 + ((2.5 + 6.75) / 2 - 0.0) / 2]
+    g0 = math.log(abs((1.0 - ed[0]) / (1.0 - ed[1]))) / (ed[1] - ed[0]) - 1j * math.pi / (ed[1] - ed[0])
+    assert abs(T[0] - (0.5 + 0.25 * g0)) < 1e-15
+    g1 = math.log(abs((5.0 - ed[1]) / (5.0 - ed[2]))) / (ed[2] - ed[1]) - 1j * math.pi / (ed[2] - ed[1])
+    assert abs(T[1] - (-0.25 + 0.0625 * g1)) < 1e-15
+
+
+def test_identity_I1_P4():
+    # (VC)_ik = C_ik (eps_k - e_i)  because H C = C D and H0 is diagonal
+    N = 50
+    p, e0, dE, Ee, H, V = _mt_H(N)
+    W, C, _ = o.jacobi(H)
+    VC = V @ C
+    I1 = C * (W[None, :] - e0[:, None])
+    assert np.abs(VC - I1).max() < 1e-13 * np.abs(VC).max()
+
+
+# ---------------------------------------------------------------- a5: S-matrix and phases
+def test_phase_shifts_from_known_angles():
+    rng = np.random.default_rng(3)
+    dE = np.array([0.7, 1.9])
+    bins = np.array([0, 1, 1, 0], dtype=np.int32)
+    d = np.array([-80.0, -10.0, 33.0, 89.0])
+    S = np.exp(2j * np.radians(d))
+    T = (1 - S) * dE[bins] / (2j * math.pi)            # invert S = 1 - 2 pi i T/dE
+    out, S2 = o.phase_shifts(False, T, bins, dE)
+    assert np.abs(out - d).max() < 1e-12 and np.abs(S2 - S).max() < 1e-14
+    # coupled, Stapp (Eq. A.4)
+    dm, dp, ep = np.radians([25.0, -7.0, 3.5])
+    S = np.array([[math.cos(2 * ep) * np.exp(2j * dm), 1j * math.sin(2 * ep) * np.exp(1j * (dm + dp))],
+                  [1j * math.sin(2 * ep) * np.exp(1j * (dm + dp)), math.cos(2 * ep) * np.exp(2j * dp)]])
+    T = (np.eye(2) - S) * dE[1] / (2j * math.pi)
+    out, S2 = o.phase_shifts(True, T[None], np.array([1], dtype=np.int32), dE)
+    assert np.abs(out[0] - [25.0, -7.0, 3.5]).max() < 1e-12
+
+
+# ---------------------------------------------------------------- MI solver: P1, P5
+def _yamaguchi_S_exact(tlab):
+    beta = inp.YAMAGUCHI_BETA
+    lamA, _ = inp.yamaguchi_lambda()
+    lp = lamA * inp.MU / inp.HBARC ** 2
+    p = math.sqrt(inp.MU * tlab) / inp.HBARC
+    g2 = 1.0 / (p * p + beta * beta) ** 2
+    # T = -lam g^2/(1 - lam' /(beta (beta - i p)^2)),  S = 1 - 2 i f p T,  f lam = 2 lam'
+    return 1 + 4j * lp * p * g2 / (1 - lp / (beta * (beta - 1j * p) ** 2))
+
+
+def test_mi_yamaguchi_analytic_P1():
+    lamA, _ = inp.yamaguchi_lambda()
+    for NQ in (48, 96):
+        for tlab in (1.0, 10.0, 50.0, 150.0, 350.0):
+            S, T = o.mi_solve(tlab, kind=1, lambdaA=lamA, beta=inp.YAMAGUCHI_BETA, NQ=NQ)
+            Sx = _yamaguchi_S_exact(tlab)
+            assert abs(abs(Sx) - 1) < 1e-14
+            d = 0.5 * math.degrees(math.atan2(S.imag, S.real)); dx = 0.5 * math.degrees(math.atan2(Sx.imag, Sx.real))
+            assert abs(d - dx) < 1e-9, (NQ, tlab, d, dx)
+    # SURVEY C15 probe values of the exact phase: 63.3159 / 45.8472 / 14.9765 deg at 1 / 50 / 350 MeV
+    for tlab, ref in ((1.0, 63.3159), (50.0, 45.8472), (350.0, 14.9765)):
+        Sx = _yamaguchi_S_exact(tlab)
+        assert abs(0.5 * math.degrees(math.atan2(Sx.imag, Sx.real)) - ref) < 1e-3
+    # effective-range expansion: p cot(delta) -> -1/a as p -> 0
+    tl = 1e-4
+    Sx = _yamaguchi_S_exact(tl); p = math.sqrt(inp.MU * tl) / inp.HBARC
+    dl = 0.5 * math.atan2(Sx.imag, Sx.real)
+    assert abs(p / math.tan(dl) + 1 / inp.YAMAGUCHI_A) < 1e-5
+
+
+def test_mi_unitarity_P5():
+    for l in (0, 1, 2):
+        for tlab in (1.0, 100.0, 350.0):
+            S, T = o.mi_solve(tlab, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=l)
+            assert abs(abs(S) - 1) < 1e-12
+    for J in (1, 2, 4):
+        for tlab in (5.0, 200.0):
+            S, T = o.mi_solve(tlab, coupled=True, l_or_J=J, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+            assert np.abs(S @ S.conj().T - np.eye(2)).max() < 1e-12
+            assert abs(S[0, 1] - S[1, 0]) < 1e-12
+
+
+# ---------------------------------------------------------------- whole chain: P9 and WPCD -> MI
+def _wpcd_phases(N, l=0, nE=11):
+    p, e0, dE, Ee, H, V = _mt_H(N, l)
+    W, C, _ = o.jacobi(H)
+    tl = np.linspace(1, 350, nE)
+    T, b = o.onshell_T(N, False, Ee, V, W, C, tl / 2)
+    d, S = o.phase_shifts(False, T, b, dE)
+    return tl, d, W
+
+
+def _dist180(a, b):
+    d = (a - b + 90.0) % 180.0 - 90.0
+    return np.abs(d)
+
+
+def test_bound_state_P9_and_convergence_to_MI():
+    tl = np.linspace(1, 350, 11)
+    mi = np.array([0.5 * math.degrees(np.angle(o.mi_solve(t, V0=inp.MT_V0, mu=inp.MT_MU)[0])) for t in tl])
+    errs, eb = [], []
+    for N in (50, 100, 200):
+        _, d, W = _wpcd_phases(N)
+        assert (W < 0).sum() == 1
+        eb.append(W[0])
+        errs.append(np.median(_dist180(d, mi)))
+    # SURVEY P9 probe: -2.19 / -2.22 / -2.228 MeV
+    assert abs(eb[0] + 2.19) < 0.01 and abs(eb[1] + 2.22) < 0.01 and abs(eb[2] + 2.228) < 0.002
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 1.0, errs
+
+
+def test_wpcd_yamaguchi_converges_to_exact():
+    lamA, lamB = inp.yamaguchi_lambda()
+    tl = np.linspace(1, 350, 25)
+    exact = np.array([0.5 * math.degrees(np.angle(_yamaguchi_S_exact(t))) for t in tl])
+    errs = []
+    for N in (50, 200):
+        p = inp.grid_edges(N)
+        e0, dE, Ee = o.fwp(p)
+        V, G = o.V_yamaguchi(p, lamB, inp.YAMAGUCHI_BETA)
+        H, Vf = o.assemble_H(e0, V)
+        W, C, _ = o.jacobi(H)
+        T, b = o.onshell_T(N, False, Ee, Vf, W, C, tl / 2)
+        d, S = o.phase_shifts(False, T, b, dE)
+        errs.append(np.median(_dist180(d, exact)))
+    assert errs[1] < errs[0] and errs[1] < 1.0, errs
+
+
+def test_coupled_wpcd_vs_mi():
+    # reading C6 (branch assignment) and C8 (coupling): coupled WPCD S-matrix approaches the coupled MI S-matrix
+    N, J = 100, 1
+    p = inp.grid_edges(N)
+    e0, dE, Ee = o.fwp(p)
+    Vmm = o.V_yukawa(p, J - 1, **MT); Vpp = o.V_yukawa(p, J + 1, **MT)
+    Vmp = o.V_yukawa(p, J, [inp.TENSOR_V], [inp.TENSOR_MU])
+    H, V = o.assemble_H(e0, Vmm, Vpp, Vmp)
+    W, C, _ = o.jacobi(H)
+    tl = np.linspace(20, 350, 7)
+    T, b = o.onshell_T(N, True, Ee, V, W, C, tl / 2)
+    d, S = o.phase_shifts(True, T, b, dE)
+    worst = 0.0
+    for e, t in enumerate(tl):
+        Smi, _ = o.mi_solve(t, coupled=True, l_or_J=J, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+        worst = max(worst, np.abs(S[e] - Smi).max())
+    assert worst < 0.15, worst      # |dS| ~ 2 sin(d delta): a few degrees at N=100
+
+
+def test_solve_batch_matches_single_calls():
+    N = 32
+    p, e0, dE, Ee, H, V = _mt_H(N)
+    tl, Ecm = inp.energies(20)
+    r = o.solve_batch(N, False, Ee, dE, np.stack([H, H]), np.stack([V, V]), Ecm)
+    W, C, _ = o.jacobi(H)
+    T, b = o.onshell_T(N, False, Ee, V, W, C, Ecm)
+    d, S = o.phase_shifts(False, T, b, dE)
+    assert np.array_equal(r["W"][1], W) and np.array_equal(r["delta"][0], d) and np.array_equal(r["bin"], b)
