@@ -1,0 +1,138 @@
+/* wpcd.h -- C ABI of the B200-native (sm_100a) WPCD hot path.
+ *
+ * Method: wave-packet continuum discretisation for NN scattering, Miller, Ekstrom, Forssen, arXiv:2106.00454
+ * (cited below as PAPER.md:<line>, the text under /root/reference).  The four compute calls are the steps (i)-(v)
+ * of the paper's recipe:
+ *
+ *   wpcd_build_channels : steps (i)+V  -- free wave-packet energies (Eqs. 17-19) and the bin-averaged potential
+ *                          <x_i|v|x_j> of Eq. 29, H = H0 + V per channel and potential sample
+ *   wpcd_diag_batched   : step (ii)    -- H = C D C^T, Eq. 21, batched block-Jacobi
+ *   wpcd_onshell_T      : steps (iii)-(v) -- pseudostate bin edges Eq. 23, analytic resolvent
+ *                          Eqs. B.3-B.6, on-shell T of Eq. 32/39/27
+ *   wpcd_phase_shifts   : S = 1 - 2 pi i T/dE (Eq. A.3 with the wave-packet normalisation of Eq. 25, PAPER.md:490,
+ *                          196, 257), phase shifts by Eqs. A.4-A.5
+ *
+ * Conventions
+ *   - fp64 everywhere.  Momenta fm^-1, energies MeV.  E = cE p^2, cE = hbarc^2/(2 mu)  (E = p^2/m_N).
+ *   - Bins are 0-based: bin i = [p_i, p_{i+1}], i = 0..N-1.  Momentum wave packets f(k)=1, N_i = Delta k_i.
+ *   - Matrices are row-major, batches are strided ("stored congruently"): element (b,i,j) at
+ *     base[(b*n + i)*n + j].  Uncoupled channels have n = N; coupled channels n = 2N with row index alpha*N + i,
+ *     alpha = 0 for l = J-1 and 1 for l = J+1, the SAME H0 in both blocks (degenerate bases).
+ *   - Pointers named d_* are DEVICE pointers, h_* (and all struct members) are HOST pointers.  Every buffer is
+ *     caller-allocated and caller-owned; the library allocates nothing after wpcd_create (workspace is passed in,
+ *     its size comes from the *_workspace_bytes queries).  Device buffers must be 16-byte aligned.
+ *   - Every compute call is asynchronous on `stream` (a cudaStream_t passed as void*, NULL = default stream) and
+ *     does not synchronise with the host.  Host-side tables in the structs are read before the call returns.
+ *   - Return value: WPCD_OK or a negative error code; argument errors are detected before any launch.
+ *     No exceptions, no errno, no global state.  There is no CPU fallback anywhere in this library.
+ */
+#ifndef WPCD_H
+#define WPCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WPCD_OK 0
+#define WPCD_EINVAL (-1) /* bad argument (NULL pointer, non-positive size, unsorted edges, ...) */
+#define WPCD_ESIZE (-2)  /* size not supported (n < 2, too many channels/terms for the tables) */
+#define WPCD_EWORK (-3)  /* workspace too small */
+#define WPCD_ECUDA (-4)  /* CUDA runtime / launch failure (see wpcd_last_cuda_error) */
+
+#define WPCD_MAX_CHANNELS 16
+#define WPCD_MAX_TERMS 4
+
+/* Local potential = sum of Yukawas V(r) = sum_t V0_t exp(-mu_t r)/r, projected on partial wave l with the Legendre
+ * function of the second kind: <k'|v_l|k> = (1/pi) sum_t V0_t Q_l(z_t)/(k'k), z_t = (k'^2+k^2+mu_t^2)/(2k'k)
+ * (convention B of DESIGN.md reading C1).  Coupled channels add the symmetric off-diagonal block
+ * (1/pi) VT Q_J(z_T)/(k'k) (reading C8).  kind 1: separable Yamaguchi <k'|v|k> = -lambda g(k')g(k),
+ * g = 1/(k^2+beta^2) (uncoupled only; lambda in convention B, MeV fm^-1). */
+typedef struct {
+  int kind;             /* 0 = Yukawa sum, 1 = Yamaguchi */
+  int n_terms;          /* kind 0: number of Yukawa terms, 1..WPCD_MAX_TERMS */
+  const double* V0;     /* [n_terms] strengths, MeV fm (sign included: repulsive > 0) */
+  const double* mu;     /* [n_terms] ranges, fm^-1 */
+  const int* scale_idx; /* [n_terms] column of d_scales multiplying V0_t for each sample, or -1 (NULL = all -1) */
+  double VT, muT;       /* coupled-channel off-diagonal Yukawa: strength MeV fm, range fm^-1 */
+  int VT_scale_idx;     /* column of d_scales multiplying VT, or -1 */
+  double lambda, beta;  /* kind 1 */
+} wpcd_potential;
+
+typedef struct {
+  int coupled; /* 0: uncoupled channel of orbital angular momentum lJ; 1: coupled l = J-1, J+1 with J = lJ >= 1 */
+  int lJ;
+} wpcd_channel;
+
+typedef struct {
+  int N;                 /* number of wave packets */
+  const double* h_edges; /* [N+1] bin edges p_0 < p_1 < ... < p_N, fm^-1, p_0 >= 0 */
+  double hbarc, mu;      /* MeV fm, MeV (reduced mass) */
+  int n_gl;              /* Gauss-Legendre points per bin for Eq. 29, 1..16 (BASELINE configs: 8) */
+} wpcd_grid;
+
+/* Handle: owns only immutable device tables.  One handle per host thread/stream.  device = CUDA ordinal. */
+int wpcd_create(void** handle, int device);
+void wpcd_destroy(void* handle);
+const char* wpcd_strerror(int code);
+const char* wpcd_last_cuda_error(void* handle); /* text of the last CUDA error seen by this handle ("" if none) */
+int wpcd_num_sms(void* handle);
+
+/* Workspace sizes in bytes (0 is a valid answer). */
+size_t wpcd_build_workspace_bytes(void* handle, int N, int n_chan);
+size_t wpcd_diag_workspace_bytes(void* handle, int n, int batch);
+size_t wpcd_onshell_workspace_bytes(void* handle, int N, int coupled, int batch, int nE);
+
+/* Steps (i) + Eq. 29.  For every sample s = 0..S-1 and channel c of the list builds H = H0 + V.
+ *   d_scales : [S][P] per-sample multiplicative scales (reading C14), or NULL with P = 0 (then S must be 1 or all
+ *              samples are identical).  Strength t of sample s is V0_t * d_scales[s][scale_idx[t]].
+ *   d_H_unc  : [S][n_unc][N][N]   (n_unc = number of uncoupled channels, list order), may be NULL if n_unc = 0
+ *   d_H_cpl  : [S][n_cpl][2N][2N] (n_cpl = number of coupled channels, list order),   may be NULL if n_cpl = 0
+ *   d_e0     : [N]   FWP kinetic energies e_i = cE (p_i^2 + p_i p_{i+1} + p_{i+1}^2)/3 (reading C4)
+ *   d_dE     : [N]   FWP bin energy widths,  d_Eedge : [N+1] bin edges in energy (cE p_i^2)
+ * The basis matrices (one per distinct (l, mu_t)) are built in the workspace by an 8x8-point (n_gl x n_gl)
+ * Gauss-Legendre rule per bin pair and combined per sample with coalesced, vectorised stores.  H is exactly
+ * symmetric.  V is not stored: V = H - diag(e0) (wpcd_onshell_T recomputes it on the fly). */
+int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
+                        int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl,
+                        double* d_e0, double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, void* stream);
+
+/* Step (ii), Eq. 21.  Batched real-symmetric eigendecomposition by two-sided block-Jacobi (8-wide blocks paired in
+ * a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered Jacobi sweep inside one warp; the
+ * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products).  n <= 112: one CTA per
+ * matrix, matrix and eigenvectors resident in shared memory; larger n: same algorithm through a global workspace.
+ *   d_A    : [batch][n][n] input (only read; must be symmetric)
+ *   d_W    : [batch][n] eigenvalues ascending
+ *   d_C    : [batch][n][n] eigenvectors, column k belongs to d_W[k]  (C_ij = <x_i|z_j>)
+ *   d_info : [batch] sweeps used (>= 1), or -1 if not converged in max_sweeps
+ *   tol    : a pivot is rotated iff |a_pq| > tol sqrt(|a_pp a_qq|); convergence = a full sweep without rotation.
+ *            tol <= 0 selects the default 2^-52. */
+int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                      double tol, int max_sweeps, void* d_work, size_t work_bytes, void* stream);
+
+/* Steps (iii)-(v).  For every matrix b and energy e: FWP bin i(e) with Eedge_i <= E_e < Eedge_{i+1}, then
+ *   uncoupled: T_ii(E) = V_ii + sum_b (VC)_ib^2/(E - eps_b) + sum_k (VC)_ik^2 g_k(E)
+ *   coupled  : T^{ab}(E) = V_{(a i)(b i)} + sum_k (VC)_{(a i)k} g_k(E) (VC)_{(b i)k},  a,b in {0,1}
+ * with g_k(E) = [ln|(E-lo_k)/(E-hi_k)| - i pi 1{lo_k <= E < hi_k}]/(hi_k - lo_k) (readings G2, C11), edges from
+ * Eq. 23 as printed (C5), negative eigenvalues = bound states, positive eigenvalues of coupled channels alternate
+ * between two branches by rank (C6).  VC = (H - diag(e0)) C is formed for the on-shell rows only.
+ *   d_H, d_W, d_C : as given to / returned by wpcd_diag_batched (n = N or 2N)
+ *   d_Ecm  : [nE] c.m. energies, MeV;  mode: 0 = point-wise resolvent (only mode implemented)
+ *   d_T    : [batch][nE][2] (re,im) or [batch][nE][2][2][2] for coupled;  zero where E is outside the grid
+ *   d_bin  : [nE] FWP bin of each energy (-1 if outside the grid) */
+int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
+                   const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE, int mode,
+                   double* d_T, int* d_bin, void* d_work, size_t work_bytes, void* stream);
+
+/* Eqs. A.3-A.5.  S = 1 - 2 pi i T/dE_bin.  Uncoupled: delta = atan2(Im S, Re S)/2 in degrees, (-90, 90].
+ * Coupled (Stapp): delta_- = arg(S_11)/2, delta_+ = arg(S_22)/2, eps = atan2(Re[-i S_12 e^{-i(d- + d+)}], |S_11|)/2.
+ *   d_delta : [batch][nE] or [batch][nE][3] = (delta_-, delta_+, eps), degrees
+ *   d_S     : optional (may be NULL) S-matrix, same layout as d_T */
+int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
+                      const double* d_dE, double* d_delta, double* d_S, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WPCD_H */

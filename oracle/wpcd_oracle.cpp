@@ -77,9 +77,11 @@ void orc_gl_rule(int n, double* x, double* w) {
 //   z >  zstar : Q_l = sqrt(pi) Gamma(l+1)/(Gamma(l+3/2) (2z)^{l+1}) * 2F1((l+1)/2,(l+2)/2; l+3/2; z^-2)  (series)
 // zstar = 1.1 (SURVEY proposed 1.5; 1.1 keeps the upward recurrence's error growth below ~1e-14 for l <= 5 while
 // the series still converges geometrically with ratio z^-2 <= 0.83; reading C7).
-double orc_legendre_Q(int l, double z) {
+// zm1 = z - 1 is passed separately so that callers can form it without cancellation:
+//   z - 1 = ((k'-k)^2 + mu^2)/(2k'k)   (z itself is within 1e-5 of 1 on the high-momentum diagonal).
+double orc_legendre_Qz(int l, double z, double zm1) {
   const double zstar = 1.1;
-  double q0 = 0.5 * std::log1p(2.0 / (z - 1.0));
+  double q0 = 0.5 * std::log1p(2.0 / zm1);
   if (l == 0) return q0;
   if (z <= zstar) {
     double qm = q0, q = z * q0 - 1.0;
@@ -100,6 +102,13 @@ double orc_legendre_Q(int l, double z) {
     if (term < 1e-18 * sum) break;
   }
   return pref * sum / std::pow(z, l + 1);
+}
+double orc_legendre_Q(int l, double z) { return orc_legendre_Qz(l, z, z - 1.0); }
+
+// z and z-1 of a Yukawa of range mu between momenta kp, k.
+static inline void yukawa_z(double kp, double k, double mu, double* z, double* zm1) {
+  *zm1 = ((kp - k) * (kp - k) + mu * mu) / (2.0 * kp * k);
+  *z = 1.0 + *zm1;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -143,8 +152,9 @@ void orc_V_yukawa(int N, const double* p, int l, int nterms, const double* V0, c
           double kp = k[i * ngl + a], kk = k[j * ngl + b];
           double s = 0.0;
           for (int t = 0; t < nterms; ++t) {
-            double z = (kp * kp + kk * kk + mu[t] * mu[t]) / (2.0 * kp * kk);
-            s += V0[t] * orc_legendre_Q(l, z);
+            double z, zm1;
+            yukawa_z(kp, kk, mu[t], &z, &zm1);
+            s += V0[t] * orc_legendre_Qz(l, z, zm1);
           }
           acc += om[i * ngl + a] * om[j * ngl + b] * s;
         }
@@ -412,8 +422,9 @@ void orc_mi_grid(int NQ, double cmap, double* k, double* w) {
 static double vA_yukawa(int l, int nterms, const double* V0, const double* mu, double kp, double k) {
   double s = 0.0;
   for (int t = 0; t < nterms; ++t) {
-    double z = (kp * kp + k * k + mu[t] * mu[t]) / (2.0 * kp * k);
-    s += V0[t] * orc_legendre_Q(l, z);
+    double z, zm1;
+    yukawa_z(kp, k, mu[t], &z, &zm1);
+    s += V0[t] * orc_legendre_Qz(l, z, zm1);
   }
   return s / (2.0 * kp * k);
 }

@@ -1,0 +1,137 @@
+// C-ABI entry points of libwpcd.so (see include/wpcd.h): argument checks, then kernel launches.  No CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "wpcd_internal.cuh"
+
+int wpcd_check_cuda(WpcdHandle* h, cudaError_t e, const char* where) {
+  if (e == cudaSuccess) return WPCD_OK;
+  if (h) snprintf(h->cuda_err, sizeof(h->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+  return WPCD_ECUDA;
+}
+
+extern "C" {
+
+int wpcd_create(void** handle, int device) {
+  if (!handle) return WPCD_EINVAL;
+  *handle = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return WPCD_ECUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return WPCD_ECUDA;
+  if (prop.major < 10) return WPCD_ECUDA;  // sm_100a only
+  WpcdHandle* h = new (std::nothrow) WpcdHandle();
+  if (!h) return WPCD_EINVAL;
+  h->device = device;
+  h->num_sms = prop.multiProcessorCount;
+  h->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+  h->cuda_err[0] = 0;
+  *handle = h;
+  return WPCD_OK;
+}
+
+void wpcd_destroy(void* handle) { delete static_cast<WpcdHandle*>(handle); }
+
+const char* wpcd_strerror(int code) {
+  switch (code) {
+    case WPCD_OK: return "ok";
+    case WPCD_EINVAL: return "invalid argument";
+    case WPCD_ESIZE: return "unsupported size";
+    case WPCD_EWORK: return "workspace too small";
+    case WPCD_ECUDA: return "CUDA runtime or launch failure";
+    default: return "unknown error";
+  }
+}
+
+const char* wpcd_last_cuda_error(void* handle) { return handle ? static_cast<WpcdHandle*>(handle)->cuda_err : ""; }
+int wpcd_num_sms(void* handle) { return handle ? static_cast<WpcdHandle*>(handle)->num_sms : 0; }
+
+size_t wpcd_build_workspace_bytes(void* handle, int N, int n_chan) {
+  if (!handle || N < 1 || n_chan < 1) return 0;
+  return wpcd_build_workspace(N, n_chan);
+}
+size_t wpcd_diag_workspace_bytes(void* handle, int n, int batch) {
+  if (!handle || n < 2 || batch < 1) return 0;
+  return wpcd_jacobi_workspace(static_cast<WpcdHandle*>(handle), n, batch);
+}
+size_t wpcd_onshell_workspace_bytes(void* handle, int N, int coupled, int batch, int nE) {
+  if (!handle || N < 1 || batch < 1 || nE < 1) return 0;
+  return wpcd_onshell_workspace(N, coupled, batch, nE);
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<size_t>(p) & 15) == 0; }
+
+int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
+                        int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl,
+                        double* d_e0, double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !grid || !pot || !chan || !d_e0 || !d_dE || !d_Eedge) return WPCD_EINVAL;
+  if (grid->N < 1 || !grid->h_edges || grid->n_gl < 1 || grid->n_gl > 16 || !(grid->hbarc > 0) || !(grid->mu > 0)) return WPCD_EINVAL;
+  if (n_chan < 1 || S < 1 || P < 0 || (P > 0 && !d_scales)) return WPCD_EINVAL;
+  if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
+  if (!(grid->h_edges[0] >= 0)) return WPCD_EINVAL;
+  for (int i = 0; i < grid->N; ++i)
+    if (!(grid->h_edges[i + 1] > grid->h_edges[i])) return WPCD_EINVAL;
+  if (pot->kind != 0 && pot->kind != 1) return WPCD_EINVAL;
+  if (pot->kind == 0) {
+    if (pot->n_terms < 1 || !pot->V0 || !pot->mu) return WPCD_EINVAL;
+    if (pot->n_terms > WPCD_MAX_TERMS) return WPCD_ESIZE;
+    for (int t = 0; t < pot->n_terms; ++t) {
+      if (!(pot->mu[t] > 0)) return WPCD_EINVAL;
+      if (pot->scale_idx && pot->scale_idx[t] >= P) return WPCD_EINVAL;
+    }
+    if (pot->VT_scale_idx >= P) return WPCD_EINVAL;
+  } else {
+    if (!(pot->beta > 0)) return WPCD_EINVAL;
+  }
+  int n_unc = 0, n_cpl = 0;
+  for (int c = 0; c < n_chan; ++c) {
+    if (chan[c].coupled) {
+      if (chan[c].lJ < 1 || pot->kind == 1 || !(pot->muT > 0)) return WPCD_EINVAL;
+      ++n_cpl;
+    } else {
+      if (chan[c].lJ < 0) return WPCD_EINVAL;
+      ++n_unc;
+    }
+    if (chan[c].lJ > 20) return WPCD_ESIZE;
+  }
+  if ((n_unc && !d_H_unc) || (n_cpl && !d_H_cpl)) return WPCD_EINVAL;
+  if (!aligned16(d_H_unc) || !aligned16(d_H_cpl) || !aligned16(d_work)) return WPCD_EINVAL;
+  if (work_bytes < wpcd_build_workspace(grid->N, n_chan) || (!d_work && wpcd_build_workspace(grid->N, n_chan))) return WPCD_EWORK;
+  return wpcd_build_launch(h, grid, pot, chan, n_chan, d_scales, S, P, d_H_unc, d_H_cpl, d_e0, d_dE, d_Eedge, d_work,
+                           work_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                      double tol, int max_sweeps, void* d_work, size_t work_bytes, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !d_A || !d_W || !d_C || !d_info || batch < 1 || max_sweeps < 1) return WPCD_EINVAL;
+  if (n < 2 || n > 4096) return WPCD_ESIZE;
+  if (!aligned16(d_A) || !aligned16(d_C) || !aligned16(d_work)) return WPCD_EINVAL;
+  size_t need = wpcd_jacobi_workspace(h, n, batch);
+  if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
+  return wpcd_jacobi_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, d_work, work_bytes,
+                            static_cast<cudaStream_t>(stream));
+}
+
+int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
+                   const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE, int mode,
+                   double* d_T, int* d_bin, void* d_work, size_t work_bytes, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !d_e0 || !d_Eedge || !d_H || !d_W || !d_C || !d_Ecm || !d_T || !d_bin) return WPCD_EINVAL;
+  if (N < 1 || batch < 1 || nE < 1 || mode != 0) return WPCD_EINVAL;
+  size_t need = wpcd_onshell_workspace(N, coupled, batch, nE);
+  if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
+  return wpcd_onshell_launch(h, N, coupled ? 1 : 0, batch, d_e0, d_Eedge, d_H, d_W, d_C, d_Ecm, nE, d_T, d_bin, d_work,
+                             work_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
+                      const double* d_dE, double* d_delta, double* d_S, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !d_T || !d_bin || !d_dE || !d_delta || batch < 1 || nE < 1) return WPCD_EINVAL;
+  return wpcd_phase_launch(h, coupled ? 1 : 0, batch, nE, d_T, d_bin, d_dE, d_delta, d_S,
+                           static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

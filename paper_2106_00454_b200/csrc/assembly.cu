@@ -1,0 +1,255 @@
+// assembly.cu -- steps (i) and Eq. 29 of the WPCD recipe: H = H0 + V for every channel
+// and potential sample.  Three kernels:
+//   k_grid    : bin quantities (e0, dE, Eedge) and the n_gl-point Gauss-Legendre nodes/weights of every bin
+//   k_basis   : one "basis matrix" per distinct (l, mu):  B[i][j] = (1/(pi sqrt(Dk_i Dk_j))) sum_ab w_ia w_jb Q_l(z)
+//               (n_gl x n_gl rule per bin pair; FP64/SFU bound, done once per grid)
+//   k_combine : H[s][c] = diag(e0) + sum_t V0_t scale[s][t] B_t   -- HBM-write bound: 8 B written per element,
+//               double2 stores, the basis matrices stay L2-resident.
+// Strengths enter linearly, so the per-sample work is the combine only.
+#include <math.h>
+#include "wpcd_internal.cuh"
+
+#define MAX_BASIS (WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1))
+
+struct BasisDesc { int l; int kind; double mu; double beta; };  // kind 0: Yukawa Q_l, 1: Yamaguchi G_i G_j
+struct BasisTable { int nbasis; BasisDesc d[MAX_BASIS]; };
+
+struct BlockTerms { int nterms; int basis[WPCD_MAX_TERMS]; int sidx[WPCD_MAX_TERMS]; double V0[WPCD_MAX_TERMS]; };
+struct ChanDesc { int coupled; int slot; BlockTerms mm, pp, mp; };
+struct ChanTable { int nchan; int n_unc; int n_cpl; ChanDesc c[WPCD_MAX_CHANNELS]; };
+
+// ------------------------------------------------------------------------------------------------ k_grid
+// thread (i, a): Newton iteration for the a-th root of P_ngl, then maps it into bin i.
+__global__ void k_grid(int N, int ngl, double hbarc, double mu, const double* __restrict__ p, double* __restrict__ e0,
+                       double* __restrict__ dE, double* __restrict__ Eedge, double* __restrict__ knode,
+                       double* __restrict__ wnode) {
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  double cE = hbarc * hbarc / (2.0 * mu);
+  if (idx <= N) Eedge[idx] = cE * p[idx] * p[idx];
+  if (idx < N) {
+    double a = p[idx], b = p[idx + 1];
+    e0[idx] = cE * (a * a + a * b + b * b) / 3.0;
+    dE[idx] = cE * b * b - cE * a * a;
+  }
+  if (idx < N * ngl) {
+    int i = idx / ngl, a = idx % ngl;
+    // root a (ascending) of the Legendre polynomial P_ngl
+    double x = -cos(WPCD_PI * (a + 0.75) / (ngl + 0.5));
+    double dp = 1.0;
+    for (int it = 0; it < 50; ++it) {
+      double pm = 1.0, pc = x;
+      for (int k = 2; k <= ngl; ++k) {
+        double pn = ((2 * k - 1) * x * pc - (k - 1) * pm) / k;
+        pm = pc; pc = pn;
+      }
+      if (ngl == 1) { pm = 1.0; pc = x; }
+      dp = ngl * (x * pc - pm) / (x * x - 1.0);
+      double dx = pc / dp;
+      x -= dx;
+      if (fabs(dx) < 1e-16) break;
+    }
+    {  // derivative at the converged root
+      double pm = 1.0, pc = x;
+      for (int k = 2; k <= ngl; ++k) {
+        double pn = ((2 * k - 1) * x * pc - (k - 1) * pm) / k;
+        pm = pc; pc = pn;
+      }
+      dp = ngl * (x * pc - pm) / (x * x - 1.0);
+    }
+    double w = 2.0 / ((1.0 - x * x) * dp * dp);
+    double lo = p[i], hi = p[i + 1], half = 0.5 * (hi - lo);
+    knode[idx] = 0.5 * (lo + hi) + half * x;
+    wnode[idx] = half * w;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ Q_l
+// Legendre function of the second kind for z > 1 given z-1 (reading C7): log1p form for Q_0, upward
+// recurrence below z = 1.1, Gauss hypergeometric series in 1/z^2 above.
+__device__ double legendre_q(int l, double zm1) {
+  double z = 1.0 + zm1;
+  double q0 = 0.5 * log1p(2.0 / zm1);
+  if (l == 0) return q0;
+  if (z < 1.1) {
+    double qa = q0, qb = fma(z, q0, -1.0);
+    for (int k = 1; k < l; ++k) {
+      double qn = ((2 * k + 1) * z * qb - k * qa) / (k + 1);
+      qa = qb; qb = qn;
+    }
+    return qb;
+  }
+  double pref = 1.0, zi = 1.0 / z, zp = zi;
+  for (int k = 1; k <= l; ++k) { pref *= (double)k / (double)(2 * k + 1); zp *= zi; }
+  double x = zi * zi, a = 0.5 * (l + 1), b = 0.5 * (l + 2), c = l + 1.5;
+  double term = 1.0, sum = 1.0;
+  for (int k = 0; k < 1000; ++k) {
+    term *= (a + k) * (b + k) / ((c + k) * (k + 1.0)) * x;
+    sum += term;
+    if (term < 1e-18 * sum) break;
+  }
+  return pref * zp * sum;
+}
+
+// ------------------------------------------------------------------------------------------------ k_basis
+// grid (ceil(ntri/128), nbasis); thread = upper-triangle element (i <= j); mirrored store keeps B symmetric.
+__global__ void __launch_bounds__(128) k_basis(int N, int ngl, BasisTable tab, const double* __restrict__ p,
+                                               const double* __restrict__ knode, const double* __restrict__ wnode,
+                                               double* __restrict__ basis) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  int ntri = N * (N + 1) / 2;
+  if (e >= ntri) return;
+  // row i of the upper triangle: first element index i*N - i(i-1)/2
+  int i = (int)((2.0 * N + 1.0 - sqrt((2.0 * N + 1.0) * (2.0 * N + 1.0) - 8.0 * e)) * 0.5);
+  while (i * N - i * (i - 1) / 2 > e) --i;
+  while ((i + 1) * N - (i + 1) * i / 2 <= e) ++i;
+  int j = i + (e - (i * N - i * (i - 1) / 2));
+  BasisDesc d = tab.d[blockIdx.y];
+  double* B = basis + (size_t)blockIdx.y * N * N;
+  double dki = p[i + 1] - p[i], dkj = p[j + 1] - p[j];
+  double v;
+  if (d.kind == 1) {
+    // Yamaguchi form factor, closed form of int k/(k^2+beta^2) dk over the bin (reading C15)
+    double b2 = d.beta * d.beta;
+    double gi = 0.5 * log((p[i + 1] * p[i + 1] + b2) / (p[i] * p[i] + b2)) / sqrt(dki);
+    double gj = 0.5 * log((p[j + 1] * p[j + 1] + b2) / (p[j] * p[j] + b2)) / sqrt(dkj);
+    v = gi * gj;
+  } else {
+    double mu2 = d.mu * d.mu, acc = 0.0;
+    for (int a = 0; a < ngl; ++a) {
+      double kp = knode[i * ngl + a], wa = wnode[i * ngl + a];
+      double row = 0.0;
+      for (int b = 0; b < ngl; ++b) {
+        double k = knode[j * ngl + b];
+        double diff = kp - k;
+        double zm1 = fma(diff, diff, mu2) / (2.0 * kp * k);
+        row = fma(wnode[j * ngl + b], legendre_q(d.l, zm1), row);
+      }
+      acc = fma(wa, row, acc);
+    }
+    v = acc / (WPCD_PI * sqrt(dki * dkj));
+  }
+  B[(size_t)i * N + j] = v;
+  B[(size_t)j * N + i] = v;
+}
+
+// ------------------------------------------------------------------------------------------------ k_combine
+__device__ __forceinline__ double combine_elem(const ChanDesc& c, int N, int i, int j, const double* __restrict__ basis,
+                                               const double* __restrict__ e0, const double* __restrict__ scale, int P) {
+  int bi = 0, bj = 0, ii = i, jj = j;
+  if (c.coupled) { bi = i >= N; bj = j >= N; ii = i - bi * N; jj = j - bj * N; }
+  const BlockTerms& bt = (bi == bj) ? (bi ? c.pp : c.mm) : c.mp;
+  double v = (i == j) ? e0[ii] : 0.0;
+  double acc = 0.0;
+  for (int t = 0; t < bt.nterms; ++t) {
+    double coef = bt.V0[t];
+    if (bt.sidx[t] >= 0) coef *= scale[bt.sidx[t]];
+    acc = fma(coef, basis[(size_t)bt.basis[t] * N * N + (size_t)ii * N + jj], acc);
+  }
+  return v + acc;
+}
+
+// grid: (ceil(n*n/2/256), nchan_of_kind, S).  Each thread writes two adjacent elements (double2) when n is even.
+__global__ void __launch_bounds__(256) k_combine(int N, int coupled, ChanTable tab, const double* __restrict__ basis,
+                                                 const double* __restrict__ e0, const double* __restrict__ scales, int P,
+                                                 double* __restrict__ Hout) {
+  int n = coupled ? 2 * N : N;
+  int nkind = coupled ? tab.n_cpl : tab.n_unc;
+  // find the channel with this slot
+  int ci = 0;
+  for (int c = 0; c < tab.nchan; ++c)
+    if (tab.c[c].coupled == coupled && tab.c[c].slot == (int)blockIdx.y) ci = c;
+  const ChanDesc& cd = tab.c[ci];
+  const double* scale = scales ? scales + (size_t)blockIdx.z * P : nullptr;
+  double* H = Hout + ((size_t)blockIdx.z * nkind + blockIdx.y) * (size_t)n * n;
+  size_t total = (size_t)n * n;
+  size_t e = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2;
+  if (e >= total) return;
+  if ((total & 1) == 0) {
+    int i = (int)(e / n), j = (int)(e % n);
+    double2 out;
+    out.x = combine_elem(cd, N, i, j, basis, e0, scale, P);
+    size_t e1 = e + 1;
+    int i1 = (int)(e1 / n), j1 = (int)(e1 % n);
+    out.y = combine_elem(cd, N, i1, j1, basis, e0, scale, P);
+    *reinterpret_cast<double2*>(H + e) = out;
+  } else {
+    for (size_t k = e; k < e + 2 && k < total; ++k) H[k] = combine_elem(cd, N, (int)(k / n), (int)(k % n), basis, e0, scale, P);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+size_t wpcd_build_workspace(int N, int n_chan) {
+  size_t nb = (size_t)n_chan * (2 * WPCD_MAX_TERMS + 1);
+  if (nb > MAX_BASIS) nb = MAX_BASIS;
+  return align256((size_t)(N + 1) * 8) + 2 * align256((size_t)N * 16 * 8) + nb * align256((size_t)N * N * 8);
+}
+
+static int find_or_add(BasisTable& t, int l, int kind, double mu, double beta) {
+  for (int b = 0; b < t.nbasis; ++b)
+    if (t.d[b].l == l && t.d[b].kind == kind && t.d[b].mu == mu && t.d[b].beta == beta) return b;
+  if (t.nbasis >= MAX_BASIS) return -1;
+  t.d[t.nbasis].l = l; t.d[t.nbasis].kind = kind; t.d[t.nbasis].mu = mu; t.d[t.nbasis].beta = beta;
+  return t.nbasis++;
+}
+
+int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
+                      int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl, double* d_e0,
+                      double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, cudaStream_t st) {
+  const int N = grid->N, ngl = grid->n_gl;
+  BasisTable bt; bt.nbasis = 0;
+  ChanTable ct; ct.nchan = n_chan; ct.n_unc = 0; ct.n_cpl = 0;
+  for (int c = 0; c < n_chan; ++c) {
+    ChanDesc& cd = ct.c[c];
+    cd.coupled = chan[c].coupled ? 1 : 0;
+    cd.slot = cd.coupled ? ct.n_cpl++ : ct.n_unc++;
+    cd.mm.nterms = cd.pp.nterms = cd.mp.nterms = 0;
+    auto fill_central = [&](BlockTerms& b, int l) -> int {
+      b.nterms = pot->n_terms;
+      for (int t = 0; t < pot->n_terms; ++t) {
+        int id = find_or_add(bt, l, 0, pot->mu[t], 0.0);
+        if (id < 0) return WPCD_ESIZE;
+        b.basis[t] = id; b.V0[t] = pot->V0[t]; b.sidx[t] = pot->scale_idx ? pot->scale_idx[t] : -1;
+      }
+      return WPCD_OK;
+    };
+    int rc = WPCD_OK;
+    if (pot->kind == 1) {
+      int id = find_or_add(bt, 0, 1, 0.0, pot->beta);
+      if (id < 0) return WPCD_ESIZE;
+      cd.mm.nterms = 1; cd.mm.basis[0] = id; cd.mm.V0[0] = -pot->lambda; cd.mm.sidx[0] = -1;
+    } else if (!cd.coupled) {
+      rc = fill_central(cd.mm, chan[c].lJ);
+    } else {
+      rc = fill_central(cd.mm, chan[c].lJ - 1);
+      if (rc == WPCD_OK) rc = fill_central(cd.pp, chan[c].lJ + 1);
+      int id = find_or_add(bt, chan[c].lJ, 0, pot->muT, 0.0);
+      if (id < 0) return WPCD_ESIZE;
+      cd.mp.nterms = 1; cd.mp.basis[0] = id; cd.mp.V0[0] = pot->VT; cd.mp.sidx[0] = pot->VT_scale_idx;
+    }
+    if (rc != WPCD_OK) return rc;
+  }
+  char* w = static_cast<char*>(d_work);
+  double* d_p = reinterpret_cast<double*>(w); w += align256((size_t)(N + 1) * 8);
+  double* d_k = reinterpret_cast<double*>(w); w += align256((size_t)N * 16 * 8);
+  double* d_w = reinterpret_cast<double*>(w); w += align256((size_t)N * 16 * 8);
+  double* d_basis = reinterpret_cast<double*>(w);
+  if ((size_t)(w - static_cast<char*>(d_work)) + (size_t)bt.nbasis * N * N * 8 > work_bytes) return WPCD_EWORK;
+
+  int rc = wpcd_check_cuda(h, cudaMemcpyAsync(d_p, grid->h_edges, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, st), "edges H2D");
+  if (rc) return rc;
+  int tot = N * ngl > N + 1 ? N * ngl : N + 1;
+  k_grid<<<(tot + 127) / 128, 128, 0, st>>>(N, ngl, grid->hbarc, grid->mu, d_p, d_e0, d_dE, d_Eedge, d_k, d_w);
+  int ntri = N * (N + 1) / 2;
+  k_basis<<<dim3((ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, bt, d_p, d_k, d_w, d_basis);
+  if (ct.n_unc) {
+    size_t half = ((size_t)N * N + 1) / 2;
+    k_combine<<<dim3((unsigned)((half + 255) / 256), ct.n_unc, S), 256, 0, st>>>(N, 0, ct, d_basis, d_e0, d_scales, P, d_H_unc);
+  }
+  if (ct.n_cpl) {
+    size_t half = ((size_t)4 * N * N + 1) / 2;
+    k_combine<<<dim3((unsigned)((half + 255) / 256), ct.n_cpl, S), 256, 0, st>>>(N, 1, ct, d_basis, d_e0, d_scales, P, d_H_cpl);
+  }
+  return wpcd_check_cuda(h, cudaGetLastError(), "build_channels launch");
+}

@@ -1,0 +1,239 @@
+// onshell.cu -- steps (iii)-(v) of the WPCD recipe and the S-matrix / phase-shift conversion.
+//   k_bins   : FWP bin of every on-shell energy (Eedge_i <= E < Eedge_{i+1}) and the range of bins in use
+//   k_onshell: one CTA per matrix.  Pseudostate bin edges from the sorted eigenvalues (Eq. 23 as printed,
+//              PAPER.md:166-173; bound states eps < 0 separate; coupled channels: two branches by rank parity),
+//              then for chunks of on-shell bins: rows of VC = (H - diag e0) C, and for every energy in the chunk
+//              (one warp per energy, lanes over eigenstates) T = V_ii + sum_k (VC)_ik (VC)_i'k g_k(E) with the
+//              analytic resolvent g_k of Eqs. B.3-B.6 (sign of the printed last line corrected).
+//   k_phase  : S = 1 - 2 pi i T/dE_i, Eqs. A.3-A.5.
+// HBM traffic per matrix: C and the on-shell rows of H are read (C once per chunk, from L2 after the first pass).
+#include <math.h>
+#include "wpcd_internal.cuh"
+
+namespace {
+
+constexpr int kOnThreads = 256;
+
+__global__ void k_bins(int N, int nE, const double* __restrict__ Eedge, const double* __restrict__ Ecm,
+                       int* __restrict__ bin, int* __restrict__ range) {
+  __shared__ int smin, smax;
+  if (threadIdx.x == 0) { smin = 1 << 30; smax = -1; }
+  __syncthreads();
+  for (int e = threadIdx.x; e < nE; e += blockDim.x) {
+    double E = Ecm[e];
+    int b = -1;
+    if (E >= Eedge[0] && E < Eedge[N]) {
+      int lo = 0, hi = N;  // invariant Eedge[lo] <= E < Eedge[hi]
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (E >= Eedge[mid]) lo = mid; else hi = mid;
+      }
+      b = lo;
+      atomicMin(&smin, b);
+      atomicMax(&smax, b);
+    }
+    bin[e] = b;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) { range[0] = smin; range[1] = smax; }
+}
+
+struct OnshellParams {
+  const double *e0, *H, *W, *C, *Ecm;
+  const int* bin;
+  const int* range;
+  double* T;
+  int N, n, nc, nE, R;  // R = bins per chunk
+};
+
+__global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int N = P.N, n = P.n, nc = P.nc, nE = P.nE, R = P.R;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kOnThreads / 32;
+  double* sW = reinterpret_cast<double*>(smem_raw);  // [n]
+  double* sLo = sW + n;                                // [n]
+  double* sHi = sLo + n;                               // [n]
+  double* sV = sHi + n;                                // [R*nc][n]
+  double* sVC = sV + (size_t)R * nc * n;               // [R*nc][n]
+  __shared__ int s_nb;
+  const size_t mat = blockIdx.x;
+  const double* H = P.H + mat * (size_t)n * n;
+  const double* C = P.C + mat * (size_t)n * n;
+  const double* W = P.W + mat * (size_t)n;
+  double* T = P.T + mat * (size_t)nE * nc * nc * 2;
+
+  if (tid == 0) s_nb = 0;
+  for (int k = tid; k < n; k += kOnThreads) sW[k] = W[k];
+  __syncthreads();
+  {  // number of bound states = number of negative eigenvalues (ascending order)
+    int cnt = 0;
+    for (int k = tid; k < n; k += kOnThreads) cnt += sW[k] < 0.0;
+    if (cnt) atomicAdd(&s_nb, cnt);
+  }
+  __syncthreads();
+  const int nbd = s_nb;
+  for (int k = tid; k < n; k += kOnThreads) {
+    double lo = 0.0, hi = 0.0;
+    if (k >= nbd) {
+      int br = (k - nbd) % nc, i = (k - nbd) / nc;
+      int mbr = (n - nbd - br + nc - 1) / nc;  // states in this branch
+      double w = sW[k];
+      lo = i == 0 ? 0.0 : 0.5 * (sW[k - nc] + w);
+      if (i < mbr - 1) hi = 0.5 * (w + sW[k + nc]);
+      else if (mbr == 1) hi = 2.0 * w;
+      else {
+        double lop = i == 1 ? 0.0 : 0.5 * (sW[k - 2 * nc] + sW[k - nc]);
+        hi = w + 0.5 * (lo - lop);
+      }
+    }
+    sLo[k] = lo; sHi[k] = hi;
+  }
+  // energies outside the grid: T = 0
+  for (int e = tid; e < nE; e += kOnThreads)
+    if (P.bin[e] < 0)
+      for (int x = 0; x < nc * nc * 2; ++x) T[(size_t)e * nc * nc * 2 + x] = 0.0;
+  const int bmin = P.range[0], bmax = P.range[1];
+  for (int b0 = bmin; b0 <= bmax; b0 += R) {
+    const int nbins = min(R, bmax - b0 + 1), nrows = nbins * nc;
+    __syncthreads();
+    // V rows of this chunk: chunk row rr = (b - b0)*nc + alpha  <->  matrix row alpha*N + b
+    for (int e = tid; e < nrows * n; e += kOnThreads) {
+      int rr = e / n, j = e - rr * n;
+      int row = (rr % nc) * N + b0 + rr / nc;
+      double v = H[(size_t)row * n + j];
+      if (j == row) v -= P.e0[b0 + rr / nc];
+      sV[(size_t)rr * n + j] = v;
+    }
+    __syncthreads();
+    // VC rows: thread per column k, 16 accumulators
+    for (int k = tid; k < n; k += kOnThreads) {
+      double acc[16];
+#pragma unroll
+      for (int r = 0; r < 16; ++r) acc[r] = 0.0;
+      for (int j = 0; j < n; ++j) {
+        double c = C[(size_t)j * n + k];
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+          if (r < nrows) acc[r] = fma(sV[(size_t)r * n + j], c, acc[r]);
+      }
+#pragma unroll
+      for (int r = 0; r < 16; ++r)
+        if (r < nrows) sVC[(size_t)r * n + k] = acc[r];
+    }
+    __syncthreads();
+    // energies of this chunk: one warp per energy
+    for (int e = warp; e < nE; e += nwarps) {
+      int b = P.bin[e];
+      if (b < b0 || b >= b0 + nbins) continue;
+      const double E = P.Ecm[e];
+      const double* vc0 = sVC + (size_t)((b - b0) * nc) * n;
+      const double* vc1 = vc0 + (nc - 1) * n;  // == vc0 for uncoupled
+      double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
+      for (int k = lane; k < n; k += 32) {
+        double gr, gi = 0.0;
+        if (k < nbd) gr = 1.0 / (E - sW[k]);
+        else {
+          double lo = sLo[k], hi = sHi[k], wdt = hi - lo;
+          gr = log(fabs((E - lo) / (E - hi))) / wdt;
+          if (E >= lo && E < hi) gi = -WPCD_PI / wdt;
+        }
+        double a = vc0[k];
+        re00 = fma(a * a, gr, re00); im00 = fma(a * a, gi, im00);
+        if (nc == 2) {
+          double bb = vc1[k];
+          re01 = fma(a * bb, gr, re01); im01 = fma(a * bb, gi, im01);
+          re11 = fma(bb * bb, gr, re11); im11 = fma(bb * bb, gi, im11);
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        re00 += __shfl_xor_sync(0xffffffffu, re00, o); im00 += __shfl_xor_sync(0xffffffffu, im00, o);
+        if (nc == 2) {
+          re01 += __shfl_xor_sync(0xffffffffu, re01, o); im01 += __shfl_xor_sync(0xffffffffu, im01, o);
+          re11 += __shfl_xor_sync(0xffffffffu, re11, o); im11 += __shfl_xor_sync(0xffffffffu, im11, o);
+        }
+      }
+      if (lane == 0) {
+        const double* v0 = sV + (size_t)((b - b0) * nc) * n;  // row (0, b)
+        if (nc == 1) {
+          T[(size_t)e * 2] = v0[b] + re00;
+          T[(size_t)e * 2 + 1] = im00;
+        } else {
+          const double* v1 = v0 + n;  // row (1, b)
+          double* t = T + (size_t)e * 8;
+          t[0] = v0[b] + re00;     t[1] = im00;
+          t[2] = v0[N + b] + re01; t[3] = im01;
+          t[4] = v1[b] + re01;     t[5] = im01;
+          t[6] = v1[N + b] + re11; t[7] = im11;
+        }
+      }
+    }
+  }
+}
+
+__global__ void k_phase(int coupled, size_t total, int nE, const double* __restrict__ T, const int* __restrict__ bin,
+                        const double* __restrict__ dE, double* __restrict__ delta, double* __restrict__ S) {
+  size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total) return;
+  const int e = (int)(idx % nE);
+  const int b = bin[e];
+  const double w = b >= 0 ? dE[b] : 1.0;
+  const double f = 2.0 * WPCD_PI / w, deg = 180.0 / WPCD_PI;
+  if (!coupled) {
+    double tr = T[idx * 2], ti = T[idx * 2 + 1];
+    // S = 1 - i f T = 1 + f ti - i f tr
+    double sr = 1.0 + f * ti, si = -f * tr;
+    delta[idx] = 0.5 * atan2(si, sr) * deg;
+    if (S) { S[idx * 2] = sr; S[idx * 2 + 1] = si; }
+  } else {
+    const double* t = T + idx * 8;
+    double sr[4], si[4];
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      sr[x] = ((x == 0 || x == 3) ? 1.0 : 0.0) + f * t[2 * x + 1];
+      si[x] = -f * t[2 * x];
+      if (S) { S[idx * 8 + 2 * x] = sr[x]; S[idx * 8 + 2 * x + 1] = si[x]; }
+    }
+    double dm = 0.5 * atan2(si[0], sr[0]), dp = 0.5 * atan2(si[3], sr[3]);
+    // -i S12 e^{-i(dm+dp)}:  real part = Im(S12 e^{-i phi}) = si cos(phi) - sr sin(phi)
+    double sp, cp;
+    sincos(dm + dp, &sp, &cp);
+    double re = si[1] * cp - sr[1] * sp;
+    double ep = 0.5 * atan2(re, hypot(sr[0], si[0]));
+    delta[idx * 3] = dm * deg; delta[idx * 3 + 1] = dp * deg; delta[idx * 3 + 2] = ep * deg;
+  }
+}
+
+int chunk_bins(int n, int nc, int max_smem) {
+  int R = 16 / nc;  // at most 16 accumulator rows
+  while (R > 1 && (size_t)(3 * n + 2 * R * nc * n) * 8 > (size_t)max_smem - 1024) R >>= 1;
+  return R;
+}
+
+}  // namespace
+
+size_t wpcd_onshell_workspace(int, int, int, int) { return 256; }
+
+int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
+                        const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE,
+                        double* d_T, int* d_bin, void* d_work, size_t, cudaStream_t st) {
+  OnshellParams P;
+  P.e0 = d_e0; P.H = d_H; P.W = d_W; P.C = d_C; P.Ecm = d_Ecm; P.bin = d_bin; P.range = static_cast<int*>(d_work);
+  P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE;
+  int budget = h->max_smem_optin < 100 * 1024 ? h->max_smem_optin : 100 * 1024;
+  P.R = chunk_bins(P.n, P.nc, budget);
+  size_t smem = (size_t)(3 * P.n + 2 * P.R * P.nc * P.n) * 8;
+  if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
+  k_bins<<<1, 256, 0, st>>>(N, nE, d_Eedge, d_Ecm, d_bin, static_cast<int*>(d_work));
+  int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
+  if (rc) return rc;
+  k_onshell<<<batch, kOnThreads, smem, st>>>(P);
+  return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
+}
+
+int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
+                      const double* d_dE, double* d_delta, double* d_S, cudaStream_t st) {
+  size_t total = (size_t)batch * nE;
+  k_phase<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(coupled, total, nE, d_T, d_bin, d_dE, d_delta, d_S);
+  return wpcd_check_cuda(h, cudaGetLastError(), "phase_shifts launch");
+}

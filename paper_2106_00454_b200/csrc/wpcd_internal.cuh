@@ -1,0 +1,35 @@
+// Internal declarations shared by the translation units of libwpcd.so (CUDA side only; nothing here is used by
+// the CPU oracle under /oracle).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include "../../include/wpcd.h"
+
+#define WPCD_PI 3.14159265358979323846264338327950288
+
+struct WpcdHandle {
+  int device;
+  int num_sms;
+  int max_smem_optin;
+  char cuda_err[256];
+};
+
+// Records a CUDA error text in the handle and returns WPCD_ECUDA (or WPCD_OK).
+int wpcd_check_cuda(WpcdHandle* h, cudaError_t e, const char* where);
+
+// jacobi.cu
+size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch);
+int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                       double tol, int max_sweeps, void* d_work, size_t work_bytes, cudaStream_t st);
+// assembly.cu
+size_t wpcd_build_workspace(int N, int n_chan);
+int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
+                      int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl, double* d_e0,
+                      double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, cudaStream_t st);
+// onshell.cu
+size_t wpcd_onshell_workspace(int N, int coupled, int batch, int nE);
+int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
+                        const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE,
+                        double* d_T, int* d_bin, void* d_work, size_t work_bytes, cudaStream_t st);
+int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
+                      const double* d_dE, double* d_delta, double* d_S, cudaStream_t st);
