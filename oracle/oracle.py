@@ -30,6 +30,7 @@ _Vyuk = _sig("orc_V_yukawa", None, [_i, _pd, _i, _i, _pd, _pd, _i, _pd])
 _Vyam = _sig("orc_V_yamaguchi", None, [_i, _pd, _d, _d, _i, _i, _pd, _pd])
 _asm = _sig("orc_assemble_H", None, [_i, _i, _pd, _pd, _vp, _vp, _pd, _pd])
 _jac = _sig("orc_jacobi", _i, [_i, _pd, _pd, _pd, _d, _i])
+_jac_ld = _sig("orc_jacobi_ld", _i, [_i, _pd, _pd, _pd, _d, _i])
 _edges = _sig("orc_swp_edges", None, [_i, _pd, _pd])
 _res = _sig("orc_resolvent_c", None, [_d, _d, _d, _pd])
 _onT = _sig("orc_onshell_T", None, [_i, _i, _pd, _pd, _pd, _pd, _pd, _i, _pd, _pi])
@@ -107,6 +108,14 @@ def jacobi(A, tol=1e-15, max_sweeps=60):
     A = _f(A); n = A.shape[0]
     W = np.empty(n); Cm = np.empty((n, n))
     sw = _jac(n, A, W, Cm, tol, max_sweeps)
+    return W, Cm, sw
+
+
+def jacobi_ld(A, tol=1e-18, max_sweeps=60):
+    """Same algorithm in 80-bit extended precision (pin for the fp64 oracle; results rounded to fp64)."""
+    A = _f(A); n = A.shape[0]
+    W = np.empty(n); Cm = np.empty((n, n))
+    sw = _jac_ld(n, A, W, Cm, tol, max_sweeps)
     return W, Cm, sw
 
 

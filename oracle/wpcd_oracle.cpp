@@ -210,46 +210,48 @@ void orc_assemble_H(int N, int coupled, const double* e0, const double* Vmm, con
 //   theta = (a_qq - a_pp)/(2 a_pq), t = sgn(theta)/(|theta| + sqrt(theta^2+1)), c = 1/sqrt(t^2+1), s = t c;
 //   stop when a sweep starts with off(A) <= tol * ||A||_F  (tol = 1e-15 by default), eigenvalues = diagonal,
 //   sorted ascending together with the columns of C.  Returns the number of sweeps done (or -1 if max_sweeps hit).
-int orc_jacobi(int n, const double* Ain, double* W, double* C, double tol, int max_sweeps) {
-  std::vector<double> A(Ain, Ain + (size_t)n * n), V((size_t)n * n, 0.0);
-  for (int i = 0; i < n; ++i) V[(size_t)i * n + i] = 1.0;
+}  // extern "C" (template below has C++ linkage)
+template <typename R>
+static int jacobi_impl(int n, const double* Ain, double* W, double* C, double tol, int max_sweeps) {
+  std::vector<R> A(Ain, Ain + (size_t)n * n), V((size_t)n * n, R(0));
+  for (int i = 0; i < n; ++i) V[(size_t)i * n + i] = R(1);
   int sweeps = 0;
   bool converged = false;
   for (;;) {
-    double off = 0.0, fro = 0.0;
+    R off = 0, fro = 0;
     for (int i = 0; i < n; ++i)
       for (int j = 0; j < n; ++j) {
-        double a = A[(size_t)i * n + j];
+        R a = A[(size_t)i * n + j];
         fro += a * a;
         if (i != j) off += a * a;
       }
-    if (std::sqrt(off) <= tol * std::sqrt(fro)) { converged = true; break; }
+    if (std::sqrt(off) <= R(tol) * std::sqrt(fro)) { converged = true; break; }
     if (sweeps >= max_sweeps) break;
     for (int p = 0; p < n - 1; ++p)
       for (int q = p + 1; q < n; ++q) {
-        double apq = A[(size_t)p * n + q];
-        if (apq == 0.0) continue;
-        double app = A[(size_t)p * n + p], aqq = A[(size_t)q * n + q];
-        double theta = (aqq - app) / (2.0 * apq);
-        double t = (theta >= 0.0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
-        double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
+        R apq = A[(size_t)p * n + q];
+        if (apq == 0) continue;
+        R app = A[(size_t)p * n + p], aqq = A[(size_t)q * n + q];
+        R theta = (aqq - app) / (R(2) * apq);
+        R t = (theta >= 0 ? R(1) : R(-1)) / (std::fabs(theta) + std::sqrt(theta * theta + R(1)));
+        R c = R(1) / std::sqrt(t * t + R(1)), s = t * c;
         for (int k = 0; k < n; ++k) {  // columns p,q:  A <- A J
-          double akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
+          R akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
           A[(size_t)k * n + p] = c * akp - s * akq;
           A[(size_t)k * n + q] = s * akp + c * akq;
         }
         for (int k = 0; k < n; ++k) {  // rows p,q:  A <- J^T A
-          double apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
+          R apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
           A[(size_t)p * n + k] = c * apk - s * aqk;
           A[(size_t)q * n + k] = s * apk + c * aqk;
         }
         // the rotated pivot is zero by construction; diagonal by the stable update
         A[(size_t)p * n + p] = app - t * apq;
         A[(size_t)q * n + q] = aqq + t * apq;
-        A[(size_t)p * n + q] = 0.0;
-        A[(size_t)q * n + p] = 0.0;
+        A[(size_t)p * n + q] = 0;
+        A[(size_t)q * n + p] = 0;
         for (int k = 0; k < n; ++k) {  // eigenvectors: V <- V J
-          double vkp = V[(size_t)k * n + p], vkq = V[(size_t)k * n + q];
+          R vkp = V[(size_t)k * n + p], vkq = V[(size_t)k * n + q];
           V[(size_t)k * n + p] = c * vkp - s * vkq;
           V[(size_t)k * n + q] = s * vkp + c * vkq;
         }
@@ -260,10 +262,19 @@ int orc_jacobi(int n, const double* Ain, double* W, double* C, double tol, int m
   for (int i = 0; i < n; ++i) idx[i] = i;
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return A[(size_t)a * n + a] < A[(size_t)b * n + b]; });
   for (int k = 0; k < n; ++k) {
-    W[k] = A[(size_t)idx[k] * n + idx[k]];
-    for (int i = 0; i < n; ++i) C[(size_t)i * n + k] = V[(size_t)i * n + idx[k]];
+    W[k] = (double)A[(size_t)idx[k] * n + idx[k]];
+    for (int i = 0; i < n; ++i) C[(size_t)i * n + k] = (double)V[(size_t)i * n + idx[k]];
   }
   return converged ? sweeps : -1;
+}
+
+extern "C" {
+int orc_jacobi(int n, const double* Ain, double* W, double* C, double tol, int max_sweeps) {
+  return jacobi_impl<double>(n, Ain, W, C, tol, max_sweeps);
+}
+// The same algorithm in x87 extended precision (64-bit mantissa): a pin for the fp64 run, never timed.
+int orc_jacobi_ld(int n, const double* Ain, double* W, double* C, double tol, int max_sweeps) {
+  return jacobi_impl<long double>(n, Ain, W, C, tol, max_sweeps);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -1,0 +1,110 @@
+"""Batched WPCD pipeline on one GPU: the four C-ABI calls in sequence with preallocated device buffers.
+
+This is host orchestration only (buffer ownership, streams, events); every arithmetic step runs in the CUDA kernels
+behind include/wpcd.h.  `solve_device` keeps inputs and outputs in HBM; `solve_host` is the end-to-end user call with
+pinned host buffers (scales in, phase shifts out) and the copies inside.
+"""
+import numpy as np
+import torch
+
+from . import wpcd
+
+
+class Pipeline:
+    """Channels x samples -> phase shifts.  channels: list of (coupled, lJ); potential: dict for build_channels."""
+
+    KERNELS_PER_STEP_FIXED = 2  # k_grid, k_basis
+
+    def __init__(self, edges, channels, Ecm, S, potential, n_scale_cols=3, device=0, max_sweeps=30, tol=0.0):
+        self.h = wpcd.Handle(device)
+        self.dev = self.h.device
+        self.edges = np.asarray(edges, dtype=np.float64)
+        self.N = len(self.edges) - 1
+        self.channels = list(channels)
+        self.S = int(S)
+        self.potential = dict(potential)
+        self.max_sweeps, self.tol = max_sweeps, tol
+        self.n_unc = sum(1 for c, _ in self.channels if not c)
+        self.n_cpl = len(self.channels) - self.n_unc
+        N, f64 = self.N, torch.float64
+        self.nE = len(Ecm)
+        self.Ecm = torch.as_tensor(np.ascontiguousarray(Ecm, dtype=np.float64), device=self.dev)
+        self.scales = torch.ones((self.S, n_scale_cols), dtype=f64, device=self.dev)
+        self.geo = dict(e0=torch.empty(N, dtype=f64, device=self.dev), dE=torch.empty(N, dtype=f64, device=self.dev),
+                        Eedge=torch.empty(N + 1, dtype=f64, device=self.dev), H_unc=None, H_cpl=None)
+        self.kind = {}
+        for kind, nch in ((0, self.n_unc), (1, self.n_cpl)):
+            if not nch:
+                continue
+            n = (2 * N) if kind else N
+            batch = self.S * nch
+            H = torch.empty((self.S, nch, n, n), dtype=f64, device=self.dev)
+            self.geo["H_cpl" if kind else "H_unc"] = H
+            wb = self.h.diag_workspace_bytes(n, batch)
+            self.kind[kind] = dict(
+                n=n, batch=batch, nch=nch, H=H.view(batch, n, n),
+                W=torch.empty((batch, n), dtype=f64, device=self.dev), C=torch.empty((batch, n, n), dtype=f64, device=self.dev),
+                info=torch.empty(batch, dtype=torch.int32, device=self.dev),
+                work=torch.empty(max(wb, 16), dtype=torch.uint8, device=self.dev),
+                T=torch.empty((batch, self.nE, 2, 2, 2) if kind else (batch, self.nE, 2), dtype=f64, device=self.dev),
+                bins=torch.empty(self.nE, dtype=torch.int32, device=self.dev),
+                owork=torch.empty(256, dtype=torch.uint8, device=self.dev),
+                delta=torch.empty((batch, self.nE, 3) if kind else (batch, self.nE), dtype=f64, device=self.dev))
+        # pinned host buffers of the end-to-end call
+        self.h_scales = torch.empty((self.S, n_scale_cols), dtype=f64).pin_memory()
+        self.h_delta = {k: torch.empty(v["delta"].shape, dtype=f64).pin_memory() for k, v in self.kind.items()}
+        self.h_info = {k: torch.empty(v["info"].shape, dtype=torch.int32).pin_memory() for k, v in self.kind.items()}
+
+    @property
+    def channel_solves(self):
+        return self.S * len(self.channels)
+
+    @property
+    def launches_per_step(self):
+        # k_grid, k_basis, k_combine per kind; k_jacobi, k_bins, k_onshell, k_phase per kind
+        return 2 + len(self.kind) * 5
+
+    def solve_device(self, events=None):
+        """One pass of the whole hot path with inputs resident in HBM.  events: optional dict name -> (start, end)
+        torch.cuda.Event pairs recorded on the current stream around each stage."""
+        def rec(name, which):
+            if events is not None:
+                events[name][which].record()
+        p = self.potential
+        rec("build", 0)
+        self.h.build_channels(self.edges, self.channels, scales=self.scales, S=self.S, out=self.geo, **p)
+        rec("build", 1)
+        for kind, b in self.kind.items():
+            tag = "cpl" if kind else "unc"
+            rec("diag_" + tag, 0)
+            self.h.diag_batched(b["H"], tol=self.tol, max_sweeps=self.max_sweeps, W=b["W"], Cm=b["C"], info=b["info"], work=b["work"])
+            rec("diag_" + tag, 1)
+            rec("onshell_" + tag, 0)
+            self.h.onshell_T(self.N, kind, self.geo["e0"], self.geo["Eedge"], b["H"], b["W"], b["C"], self.Ecm,
+                             T=b["T"], bins=b["bins"], work=b["owork"])
+            self.h.phase_shifts(kind, b["T"], b["bins"], self.geo["dE"], want_S=False, delta=b["delta"])
+            rec("onshell_" + tag, 1)
+
+    def stage_names(self):
+        names = ["build"]
+        for kind in self.kind:
+            tag = "cpl" if kind else "unc"
+            names += ["diag_" + tag, "onshell_" + tag]
+        return names
+
+    def solve_host(self, scales_host):
+        """End-to-end user call: host scales [S][P] -> host phase shifts (pinned buffers), copies included."""
+        self.h_scales.copy_(torch.as_tensor(scales_host))
+        self.scales.copy_(self.h_scales, non_blocking=True)
+        self.solve_device()
+        for k, b in self.kind.items():
+            self.h_delta[k].copy_(b["delta"], non_blocking=True)
+            self.h_info[k].copy_(b["info"], non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return self.h_delta, self.h_info
+
+    def h2d_bytes(self):
+        return self.h_scales.numel() * 8
+
+    def d2h_bytes(self):
+        return sum(t.numel() * 8 for t in self.h_delta.values()) + sum(t.numel() * 4 for t in self.h_info.values())

@@ -1,0 +1,51 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol include/wpcd.h declares
+(no compute calls without a GPU), and the host-side input recipe is what DESIGN.md states."""
+import ctypes
+import os
+import re
+
+import numpy as np
+
+from paper_2106_00454_b200 import inputs as inp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "wpcd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(wpcd_[A-Za-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2106_00454_b200 import build
+    lib = ctypes.CDLL(build.build())
+    names = _declared()
+    assert {"wpcd_build_channels", "wpcd_diag_batched", "wpcd_onshell_T", "wpcd_phase_shifts"} <= set(names)
+    for nm in names:
+        assert hasattr(lib, nm), nm
+    lib.wpcd_strerror.restype = ctypes.c_char_p
+    assert lib.wpcd_strerror(0) == b"ok" and lib.wpcd_strerror(-2) == b"unsupported size"
+    # without a device the handle cannot be created and says so (no CPU fallback)
+    import torch
+    if not torch.cuda.is_available():
+        h = ctypes.c_void_p()
+        assert lib.wpcd_create(ctypes.byref(h), 0) == -4 and not h.value
+
+
+def test_input_recipe():
+    p = inp.grid_edges(100)
+    assert len(p) == 101 and p[0] == 0 and abs(p[100] - 127.96) < 0.01 and np.all(np.diff(p) > 0)
+    s = inp.sample_scales(1024)
+    assert s.shape == (1024, 3) and np.allclose(s[0], [1.012573, 0.986790, 1.064042], atol=1e-6)
+    assert 0.6 < s.min() < 0.62 and 1.30 < s.max() < 1.32        # range 0.61...1.31
+    assert len(inp.CHANNELS_J4) == 14 and sum(c for _, c, _ in inp.CHANNELS_J4) == 4
+    tl, ecm = inp.energies(350)
+    assert tl[0] == 1.0 and tl[-1] == 350.0 and np.allclose(ecm, tl / 2)
+
+
+def test_binding_does_not_import_oracle():
+    for fn in ("wpcd.py", "inputs.py", "build.py", "__init__.py"):
+        src = open(os.path.join(ROOT, "paper_2106_00454_b200", fn)).read()
+        assert not re.search(r"^\s*(from|import)\s+\.*oracle", src, flags=re.M), fn
+        assert "liboracle" not in src, fn

@@ -1,0 +1,228 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI (ctypes binding), against the CPU
+oracle on the same seeded inputs.  Tolerances are north_star's: eigenvalues 1e-11 relative (componentwise),
+phase shifts 1e-8 degrees absolute (mod 180; coupled channels also through |dS| <= 3.5e-10), H 1e-12 max|H|."""
+import numpy as np
+import pytest
+
+from paper_2106_00454_b200 import inputs as inp
+from tests import helpers as hp
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import torch
+    from paper_2106_00454_b200 import wpcd
+    h = wpcd.Handle(0)
+    yield dict(torch=torch, wpcd=wpcd, h=h, dev=torch.device("cuda", 0))
+    h.close()
+
+
+def _to_dev(ctx, a, dtype=None):
+    t = ctx["torch"].as_tensor(np.ascontiguousarray(a), device=ctx["dev"])
+    return t if dtype is None else t.to(dtype)
+
+
+def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0.0):
+    """Full hot path on the GPU for a channel list; returns per-kind dicts of numpy arrays."""
+    h, torch = ctx["h"], ctx["torch"]
+    p = inp.grid_edges(N)
+    d_scales = None if scales is None else _to_dev(ctx, scales)
+    kw = dict(yamaguchi=yamaguchi) if yamaguchi is not None else dict(
+        V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1] if scales is not None else None, VT=inp.TENSOR_V,
+        muT=inp.TENSOR_MU, VT_scale_idx=2 if scales is not None else -1)
+    out = h.build_channels(p, channels, scales=d_scales, S=S, **kw)
+    d_E = _to_dev(ctx, Ecm)
+    res = {}
+    for kind, key in ((0, "H_unc"), (1, "H_cpl")):
+        H = out[key]
+        if H is None:
+            continue
+        n = H.shape[-1]
+        Hb = H.reshape(-1, n, n)
+        W, C, info = h.diag_batched(Hb, tol=tol)
+        T, bins = h.onshell_T(N, kind, out["e0"], out["Eedge"], Hb, W, C, d_E)
+        delta, Sm = h.phase_shifts(kind, T, bins, out["dE"])
+        torch.cuda.synchronize()
+        nch = H.shape[1]
+        cplx = lambda x: x[..., 0].cpu().numpy() + 1j * x[..., 1].cpu().numpy()
+        res[kind] = dict(H=H.cpu().numpy(), W=W.cpu().numpy().reshape(S, nch, n), C=C.cpu().numpy().reshape(S, nch, n, n),
+                         info=info.cpu().numpy().reshape(S, nch), T=cplx(T).reshape((S, nch) + tuple(T.shape[1:-1])),
+                         S=cplx(Sm).reshape((S, nch) + tuple(T.shape[1:-1])),
+                         delta=delta.cpu().numpy().reshape((S, nch) + tuple(delta.shape[1:])), bin=bins.cpu().numpy())
+    res["e0"] = out["e0"].cpu().numpy(); res["dE"] = out["dE"].cpu().numpy(); res["Eedge"] = out["Eedge"].cpu().numpy()
+    return res
+
+
+def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguchi=None, label=""):
+    ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi)
+    ref = hp.oracle_solve(N, kind, ch, Ecm)
+    g = res[kind]
+    n = ch["H"].shape[0]
+    normH = np.abs(ch["H"]).max()
+    errH = np.abs(g["H"][s, c] - ch["H"]).max() / normH
+    assert errH <= hp.TOL_H_REL, (label, "H", errH)
+    assert np.array_equal(g["H"][s, c], g["H"][s, c].T), (label, "H symmetric")
+    assert g["info"][s, c] >= 1, (label, "info", g["info"][s, c])
+    errW = hp.check_eig(g["W"][s, c], ref["W"], normH)
+    assert errW <= hp.TOL_EIG_REL, (label, "eig", errW)
+    C = g["C"][s, c]
+    assert np.abs(C.T @ C - np.eye(n)).max() < 1e-12, (label, "orth")
+    assert np.abs(ch["H"] @ C - C * g["W"][s, c]).max() < 1e-13 * n * normH, (label, "residual")
+    assert np.array_equal(g["bin"], ref["bin"]), (label, "bins")
+    dphi, dS, nok = hp.check_phases(kind, g["delta"][s, c], g["S"][s, c], ref, Ecm)
+    assert nok > 0.9 * len(Ecm)
+    assert dphi <= hp.TOL_PHASE_DEG, (label, "phase", dphi)
+    assert dS <= hp.TOL_S_ABS, (label, "S", dS)
+    return errH, errW, dphi, dS
+
+
+# ----------------------------------------------------------------------------------------------- config 1
+def test_config1_1S0_N50(ctx):
+    tl, Ecm = inp.energies(100)
+    res = _gpu_pipeline(ctx, 50, [(0, 0)], Ecm)
+    errs = _compare_channel(res, 0, 0, 0, 50, 0, Ecm, label="cfg1")
+    assert abs(res[0]["W"][0, 0, 0] + 2.19) < 0.01     # the bound state
+    print("cfg1 errs (H, eig, phase, S):", errs)
+
+
+# ----------------------------------------------------------------------------------------------- config 2
+def test_config2_all_channels_N100(ctx):
+    tl, Ecm = inp.energies(350)
+    chans = [(c, l) for _, c, l in inp.CHANNELS_J4]
+    res = _gpu_pipeline(ctx, 100, chans, Ecm)
+    iu = ic = 0
+    worst = np.zeros(4)
+    for name, c, l in inp.CHANNELS_J4:
+        idx = ic if c else iu
+        worst = np.maximum(worst, _compare_channel(res, c, 0, idx, 100, l, Ecm, label=name))
+        if c: ic += 1
+        else: iu += 1
+    print("cfg2 worst errs (H, eig, phase, S):", worst)
+
+
+# ----------------------------------------------------------------------------------------------- config 3
+def test_config3_sampled_batch(ctx):
+    """1024 seeded samples on the GPU (full size); the oracle checks a seeded subsample of (sample, channel)."""
+    S = 1024
+    tl, Ecm = inp.energies(350)
+    scales = inp.sample_scales(S, seed=0)
+    assert np.allclose(scales[0], [1.012573, 0.986790, 1.064042], atol=1e-6)   # reading C14
+    chans = [(c, l) for _, c, l in inp.CHANNELS_J4]
+    res = _gpu_pipeline(ctx, 100, chans, Ecm, scales=scales, S=S)
+    assert (res[0]["info"] >= 1).all() and (res[1]["info"] >= 1).all()
+    nbound = (res[0]["W"][:, 0, :] < 0).sum(axis=1)          # 1S0: SURVEY 8(d): 957 samples bind, 67 do not
+    assert set(np.unique(nbound)) == {0, 1} and (nbound == 1).sum() == 957
+    rng = np.random.default_rng(1)
+    picks = [(0, 0, 0, 0), (0, 1, 0, 1)] + [(int(rng.integers(S)), int(k), None, None) for k in rng.integers(0, 14, 6)]
+    unc = [(i, l) for i, (_, c, l) in enumerate(inp.CHANNELS_J4) if not c]
+    for s, k, _, _ in picks:
+        name, c, l = inp.CHANNELS_J4[k % 14]
+        idx = sum(1 for (_, cc, _) in inp.CHANNELS_J4[:k % 14] if cc == c)
+        _compare_channel(res, c, s, idx, 100, l, Ecm, scale=tuple(scales[s]), label=f"cfg3 s={s} {name}")
+    # a sample without an S-wave bound state must be among the checked ones (both n_b paths)
+    s0 = int(np.where(nbound == 0)[0][0])
+    _compare_channel(res, 0, s0, 0, 100, 0, Ecm, scale=tuple(scales[s0]), label=f"cfg3 unbound s={s0}")
+
+
+# ----------------------------------------------------------------------------------------------- config 4
+def test_config4_large_n_and_yamaguchi(ctx):
+    """N=200 (n=200 and 400: beyond shared memory -> global-workspace path) + the Yamaguchi analytic check."""
+    S = 4
+    tl, Ecm = inp.energies(350)
+    scales = inp.sample_scales(256, seed=0)[:S]
+    chans = [(0, 0), (0, 2), (1, 1), (1, 4)]
+    res = _gpu_pipeline(ctx, 200, chans, Ecm, scales=scales, S=S)
+    _compare_channel(res, 0, 0, 0, 200, 0, Ecm, scale=tuple(scales[0]), label="cfg4 1S0")
+    _compare_channel(res, 0, 3, 1, 200, 2, Ecm, scale=tuple(scales[3]), label="cfg4 1D2 s3")
+    _compare_channel(res, 1, 1, 0, 200, 1, Ecm, scale=tuple(scales[1]), label="cfg4 3S1-3D1 s1")
+    _compare_channel(res, 1, 0, 1, 200, 4, Ecm, scale=tuple(scales[0]), label="cfg4 3F4-3H4")
+    # Yamaguchi at N=200: GPU vs oracle, and GPU vs the closed-form phase shift (median error < 1 degree)
+    lamA, lamB = inp.yamaguchi_lambda()
+    yres = _gpu_pipeline(ctx, 200, [(0, 0)], Ecm, yamaguchi=(lamB, inp.YAMAGUCHI_BETA))
+    _compare_channel(yres, 0, 0, 0, 200, 0, Ecm, yamaguchi=(lamB, inp.YAMAGUCHI_BETA), label="cfg4 yamaguchi")
+    lp = lamA * inp.MU / inp.HBARC ** 2
+    beta = inp.YAMAGUCHI_BETA
+    pm = np.sqrt(inp.MU * tl) / inp.HBARC
+    Sx = 1 + 4j * lp * pm / (pm * pm + beta * beta) ** 2 / (1 - lp / (beta * (beta - 1j * pm) ** 2))
+    exact = 0.5 * np.degrees(np.angle(Sx))
+    assert np.median(hp.dist180(yres[0]["delta"][0, 0], exact)) < 1.0
+
+
+# ----------------------------------------------------------------------------------------------- config 5
+@pytest.mark.parametrize("N", [32, 48, 64, 100, 150, 200, 300, 400])
+def test_config5_size_sweep(ctx, N):
+    """single (l=0, n=N) and coupled (J=1, n=2N) matrices at every N of the sweep, S seeded samples on the GPU, the
+    oracle on one of them (cyclic Jacobi at n = 800 costs ~1e11 flops)."""
+    S = 3
+    tl, Ecm = inp.energies(350)
+    scales = inp.sample_scales(4096, seed=0)[:S]
+    res = _gpu_pipeline(ctx, N, [(0, 0), (1, 1)], Ecm, scales=scales, S=S)
+    assert (res[0]["info"] >= 1).all() and (res[1]["info"] >= 1).all()
+    _compare_channel(res, 0, 2, 0, N, 0, Ecm, scale=tuple(scales[2]), label=f"cfg5 N={N} single")
+    _compare_channel(res, 1, 1, 0, N, 1, Ecm, scale=tuple(scales[1]), label=f"cfg5 N={N} coupled")
+
+
+# ----------------------------------------------------------------------------------------------- edge cases
+def _diag_check(ctx, A, tol_rel=1e-11):
+    from oracle import oracle as o
+    W, C, info = ctx["h"].diag_batched(_to_dev(ctx, A))
+    ctx["torch"].cuda.synchronize()
+    W = W.cpu().numpy(); C = C.cpu().numpy(); info = info.cpu().numpy()
+    for b in range(A.shape[0]):
+        Wr, Cr, _ = o.jacobi(A[b])
+        n = A.shape[1]
+        nrm = max(np.abs(A[b]).max(), 1e-300)
+        assert info[b] >= 1
+        assert np.abs(W[b] - Wr).max() <= tol_rel * nrm, (b, np.abs(W[b] - Wr).max() / nrm)
+        assert np.abs(C[b].T @ C[b] - np.eye(n)).max() < 1e-12
+        assert np.abs(A[b] @ C[b] - C[b] * W[b]).max() < 1e-13 * n * nrm
+    return W, C, info
+
+
+@pytest.mark.parametrize("n", [2, 3, 7, 8, 9, 16, 17, 31, 33, 63, 104, 105, 112, 113, 120, 129])
+def test_diag_ragged_sizes_random(ctx, n):
+    rng = np.random.default_rng(n)
+    A = rng.standard_normal((5, n, n)); A = A + A.transpose(0, 2, 1)
+    _diag_check(ctx, A)
+
+
+def test_diag_degenerate_cases(ctx):
+    n = 24
+    A = np.zeros((4, n, n))
+    A[0] = np.diag(np.arange(n, 0, -1.0))                       # already diagonal, descending: pure sort
+    A[1] = np.eye(n) * 3.0                                       # all eigenvalues equal
+    A[2] = np.ones((n, n))                                       # rank one: eigenvalues {0 x23, 24}
+    A[3][:] = 0.0                                                # zero matrix
+    W, C, info = _diag_check(ctx, A)
+    assert np.array_equal(W[0], np.arange(1.0, n + 1)) and info[0] == 1
+    assert np.allclose(W[1], 3.0) and np.allclose(W[3], 0.0)
+    assert abs(W[2][-1] - n) < 1e-12 and np.abs(W[2][:-1]).max() < 1e-12
+
+
+def test_onshell_energy_outside_grid_and_empty_like_inputs(ctx):
+    N = 16
+    Ecm = np.array([-1.0, 0.5, 40.0, 1e9])      # below 0, inside, inside, above the last edge
+    res = _gpu_pipeline(ctx, N, [(0, 0)], Ecm)
+    ch = hp.oracle_channel(N, 0, 0)
+    ref = hp.oracle_solve(N, 0, ch, Ecm)
+    assert list(res[0]["bin"]) == list(ref["bin"]) and res[0]["bin"][0] == -1 and res[0]["bin"][3] == -1
+    assert res[0]["T"][0, 0, 0] == 0 and res[0]["T"][0, 0, 3] == 0
+    assert np.abs(res[0]["T"][0, 0, 1:3] - ref["T"][1:3]).max() < 1e-9 * np.abs(ref["T"][1:3]).max()
+
+
+def test_abi_argument_errors(ctx):
+    import ctypes as C
+    wp = ctx["wpcd"]
+    lib = wp._lib
+    h = ctx["h"]._h
+    assert lib.wpcd_diag_batched(h, 1, 1, None, None, None, None, 0.0, 10, None, 0, None) == -1      # NULL pointers
+    t = ctx["torch"].zeros(16, dtype=ctx["torch"].float64, device=ctx["dev"])
+    ti = ctx["torch"].zeros(4, dtype=ctx["torch"].int32, device=ctx["dev"])
+    assert lib.wpcd_diag_batched(h, 1, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None) == -2
+    assert lib.wpcd_diag_batched(h, 200, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None) == -3
+    edges = (C.c_double * 3)(0.0, 2.0, 1.0)     # not increasing
+    g = wp.Grid(2, edges, 197.327, 469.46, 8)
+    assert lib.wpcd_build_channels(h, C.byref(g), None, None, 1, None, 1, 0, None, None, None, None, None, None, 0, None) == -1
+    assert wp._lib.wpcd_strerror(-3) == b"workspace too small"
