@@ -57,12 +57,41 @@ struct Smem {
   int* rot;      // [nslots]
   int* src;      // [np]
   int* ctr;      // [4]: 0 = work queue, 1 = rotations this sweep
+  uchar2* pq;    // [15*8] pair table of the pivot sweep
 };
 
 // ---------------------------------------------------------------------------------------------- phase 1
-// One warp: load S = A[IJ,IJ], run one parallel-ordered sweep, write S back, leave Q in the slot.
+// Pair table of one full sweep of a 16x16 pivot: 15 rounds of 8 disjoint pairs (p < q).  Rounds 0..7 take the 64
+// "cross" pairs (i in block I, j in block J), rounds 8..14 the pairs inside I and inside J (two 8-player round-robin
+// tournaments side by side), so every pair is met exactly once.
+__device__ __forceinline__ void pivot_pair(int r, int j, int& p, int& q) {
+  if (r < 8) { p = j; q = 8 + ((j + r) & 7); return; }
+  int a, b;
+  rr_pair(8, r - 8, j >> 1, a, b);
+  const int off = (j & 1) << 3;
+  p = off + (a < b ? a : b);
+  q = off + (a < b ? b : a);
+}
+
+// Jacobi rotation annihilating a_pq (classical choice |angle| <= pi/4, "Jacobi method"), written with two
+// reciprocal square roots and no division:  with d = a_qq - a_pp, b = 2 a_pq, h = sqrt(d^2 + b^2):
+//   cos 2phi = |d|/h,  c = sqrt((1 + cos 2phi)/2),  s = sgn(d) (b/h)/(2c),  t = s/c.
+__device__ __forceinline__ void rotation(double app, double aqq, double apq, double& c, double& s, double& t) {
+  const double d = aqq - app, b = apq + apq;
+  const double rh = rsqrt(fma(d, d, b * b));
+  const double c2 = fma(0.5 * fabs(d), rh, 0.5);
+  const double rc = rsqrt(c2);
+  c = c2 * rc;
+  s = copysign(0.5, d) * b * rh * rc;
+  t = s * rc;
+}
+
+// One warp: load S = A[IJ,IJ], run one full sweep (15 rounds of 8 simultaneous rotations), write S back, leave the
+// accumulated 16x16 rotation product in the slot's Q.  Lane (k0 = lane>>3, j = lane&7) owns the 2x2 blocks
+// (row pair k0, column pair j) and (row pair k0+4, column pair j) of S and rows k0, k0+4, k0+8, k0+12 of Q; one
+// round = S <- R^T S R, Q <- Q R with R the product of the round's 8 disjoint rotations, one __syncwarp per round.
 __device__ void inner_solve(const Smem& sm, int ld, int slot, int I, int J, double tol, int lane, int warp) {
-  double* S = sm.S + warp * 16 * LDSS;
+  double* S = sm.S + warp * 16 * LDSS;  // warp < min(nslots, kWarps)
   double* Q = sm.Q + slot * 16 * LDQ;
   for (int e = lane; e < 256; e += 32) {
     int a = e >> 4, b = e & 15;
@@ -70,49 +99,47 @@ __device__ void inner_solve(const Smem& sm, int ld, int slot, int I, int J, doub
     S[a * LDSS + b] = sm.A[(size_t)r * ld + swz(r, c)];
   }
   __syncwarp();
-  const int j = lane >> 2, sub = lane & 3;
+  const int j = lane & 7, k0 = lane >> 3;
+  const double tol2 = tol * tol;
   bool any = false;
+#pragma unroll 1
   for (int r = 0; r < 15; ++r) {
-    int a, b;
-    if (j == 0) { a = 15; b = r; }
-    else { a = (r + j) % 15; b = (r - j + 15) % 15; }
-    const int p = a < b ? a : b, q = a < b ? b : a;
+    const uchar2 pj = sm.pq[r * 8 + j], pa = sm.pq[r * 8 + k0], pb = sm.pq[r * 8 + k0 + 4];
+    const int p = pj.x, q = pj.y;
     const double app = S[p * LDSS + p], aqq = S[q * LDSS + q], apq = S[p * LDSS + q];
-    const bool doit = (apq != 0.0) && (fabs(apq) > tol * sqrt(fabs(app * aqq)));
-    double c = 1.0, s = 0.0, t = 0.0;
-    if (doit) {
-      double theta = (aqq - app) / (2.0 * apq);
-      t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(fma(theta, theta, 1.0)));
-      c = rsqrt(fma(t, t, 1.0));
-      s = t * c;
-      any = true;
+    double ba[4], bb[4], qx[4], qy[4];
+    ba[0] = S[pa.x * LDSS + p]; ba[1] = S[pa.x * LDSS + q]; ba[2] = S[pa.y * LDSS + p]; ba[3] = S[pa.y * LDSS + q];
+    bb[0] = S[pb.x * LDSS + p]; bb[1] = S[pb.x * LDSS + q]; bb[2] = S[pb.y * LDSS + p]; bb[3] = S[pb.y * LDSS + q];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {  // columns p,q of S and of Q
-        int i = sub + 4 * u;
-        double x = S[i * LDSS + p], y = S[i * LDSS + q];
-        S[i * LDSS + p] = c * x - s * y;
-        S[i * LDSS + q] = s * x + c * y;
-        double qx = Q[i * LDQ + p], qy = Q[i * LDQ + q];
-        Q[i * LDQ + p] = c * qx - s * qy;
-        Q[i * LDQ + q] = s * qx + c * qy;
-      }
+    for (int u = 0; u < 4; ++u) { qx[u] = Q[(k0 + 4 * u) * LDQ + p]; qy[u] = Q[(k0 + 4 * u) * LDQ + q]; }
+    // pivot test |a_pq| > tol sqrt(|a_pp a_qq|), squared
+    const bool doit = apq * apq > tol2 * fabs(app * aqq);
+    double c, s, t;
+    rotation(app, aqq, apq, c, s, t);
+    if (!doit) { c = 1.0; s = 0.0; t = 0.0; }
+    any |= doit;
+    const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
+    const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
+    {  // block (k0, j)
+      double x00 = c * ba[0] - s * ba[1], x01 = s * ba[0] + c * ba[1];
+      double x10 = c * ba[2] - s * ba[3], x11 = s * ba[2] + c * ba[3];
+      double y00 = ca * x00 - sa * x10, y10 = sa * x00 + ca * x10;
+      double y01 = ca * x01 - sa * x11, y11 = sa * x01 + ca * x11;
+      if (k0 == j && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
+      S[pa.x * LDSS + p] = y00; S[pa.x * LDSS + q] = y01; S[pa.y * LDSS + p] = y10; S[pa.y * LDSS + q] = y11;
     }
-    __syncwarp();
-    if (doit) {
+    {  // block (k0 + 4, j)
+      double x00 = c * bb[0] - s * bb[1], x01 = s * bb[0] + c * bb[1];
+      double x10 = c * bb[2] - s * bb[3], x11 = s * bb[2] + c * bb[3];
+      double y00 = cb * x00 - sb * x10, y10 = sb * x00 + cb * x10;
+      double y01 = cb * x01 - sb * x11, y11 = sb * x01 + cb * x11;
+      if (k0 + 4 == j && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
+      S[pb.x * LDSS + p] = y00; S[pb.x * LDSS + q] = y01; S[pb.y * LDSS + p] = y10; S[pb.y * LDSS + q] = y11;
+    }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {  // rows p,q of S
-        int i = sub + 4 * u;
-        double x = S[p * LDSS + i], y = S[q * LDSS + i];
-        S[p * LDSS + i] = c * x - s * y;
-        S[q * LDSS + i] = s * x + c * y;
-      }
-    }
-    __syncwarp();
-    if (doit && sub == 0) {
-      S[p * LDSS + p] = app - t * apq;
-      S[q * LDSS + q] = aqq + t * apq;
-      S[p * LDSS + q] = 0.0;
-      S[q * LDSS + p] = 0.0;
+    for (int u = 0; u < 4; ++u) {
+      Q[(k0 + 4 * u) * LDQ + p] = c * qx[u] - s * qy[u];
+      Q[(k0 + 4 * u) * LDQ + q] = s * qx[u] + c * qy[u];
     }
     __syncwarp();
   }
@@ -270,14 +297,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
       sm.V = d; d += (size_t)np * ld;
     }
     sm.Q = d; d += (size_t)nslots * 16 * LDQ;
-    sm.S = d; d += kWarps * 16 * LDSS;
+    sm.S = d; d += (nslots < kWarps ? nslots : kWarps) * 16 * LDSS;
     sm.wsort = d; d += np;
     int* ip = reinterpret_cast<int*>(d);
     sm.slotI = ip; ip += nslots;
     sm.slotJ = ip; ip += nslots;
     sm.rot = ip; ip += nslots;
     sm.src = ip; ip += np;
-    sm.ctr = ip;
+    sm.ctr = ip; ip += 4;
+    sm.pq = reinterpret_cast<uchar2*>(ip);
+  }
+  if (tid < 120) {
+    int p, q;
+    pivot_pair(tid >> 3, tid & 7, p, q);
+    sm.pq[tid] = make_uchar2((unsigned char)p, (unsigned char)q);
   }
   const int ntiles = nslots * (nslots - 1) / 2;
   const int nvgrp = (P.nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
@@ -381,10 +414,17 @@ Geometry geometry(int n) {
   g.ld = (g.np + 15) / 16 * 16;
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
   g.nslots = g.m / 2;
-  g.smem_fixed = (size_t)g.nslots * 16 * LDQ * 8 + (size_t)kWarps * 16 * LDSS * 8 + (size_t)g.np * 8 +
-                 (size_t)(3 * g.nslots + g.np + 4) * 4 + 64;
+  g.smem_fixed = (size_t)g.nslots * 16 * LDQ * 8 + (size_t)(g.nslots < kWarps ? g.nslots : kWarps) * 16 * LDSS * 8 + (size_t)g.np * 8 +
+                 (size_t)(3 * g.nslots + g.np + 4) * 4 + 240 + 64;
   g.smem_mat = (size_t)2 * g.np * g.ld * 8;
   return g;
+}
+
+// CTAs of the global-workspace path: two per SM while all their workspaces together stay well inside the 126 MB L2.
+int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
+  int per_sm = ((size_t)2 * h->num_sms * g.smem_mat <= ((size_t)80 << 20)) ? 2 : 1;
+  int grid = per_sm * h->num_sms;
+  return batch < grid ? batch : grid;
 }
 
 }  // namespace
@@ -392,7 +432,7 @@ Geometry geometry(int n) {
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
   Geometry g = geometry(n);
   if (g.smem_fixed + g.smem_mat <= (size_t)h->max_smem_optin) return 0;
-  int grid = batch < 2 * h->num_sms ? batch : 2 * h->num_sms;
+  int grid = global_grid(h, g, batch);
   return (size_t)grid * g.smem_mat;
 }
 
@@ -413,7 +453,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
     k_jacobi<false><<<batch, kThreads, smem, st>>>(P);
   } else {
     if (g.smem_fixed > (size_t)h->max_smem_optin) return WPCD_ESIZE;
-    int grid = batch < 2 * h->num_sms ? batch : 2 * h->num_sms;
+    int grid = global_grid(h, g, batch);
     if (work_bytes < (size_t)grid * g.smem_mat) return WPCD_EWORK;
     rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem_fixed), "jacobi attr");
     if (rc) return rc;
