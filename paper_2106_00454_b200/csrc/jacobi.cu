@@ -1,33 +1,47 @@
 // jacobi.cu -- step (ii) of the WPCD recipe: H = C D C^T (Eq. 21), batched, fp64.
 //
-// Two-sided BLOCK Jacobi, one CTA per matrix.
-//   * The n x n matrix is cut into 8-wide blocks.  A round-robin tournament pairs the blocks; each pair (I,J) is a
-//     "slot" with a 16x16 symmetric pivot sub-problem S = A[IJ,IJ].
-//   * Phase 1 (one warp per slot): one parallel-ordered Jacobi sweep of S (15 rounds of 8 disjoint rotations) with
-//     the textbook rotation (theta, t, c, s; Rutishauser diagonal update), accumulating the 16x16 orthogonal Q.
-//   * Phase 2 (all warps, dynamic work queue): A <- Q^T A Q tile by tile (only the upper slot-triangle is computed,
-//     the mirror image is stored) and V <- V Q, as fp64 tensor-core products (mma.sync m8n8k4 = DMMA, which runs
-//     at the full FP64 rate of the SM, 64 FMA/clk, with operands distributed over the warp).  The accumulator
-//     fragment of the first product is re-used directly as the B fragment of the second one (the k index of an
-//     MMA may be permuted freely), so a two-sided tile update needs no shuffle and no shared-memory round trip.
-//   * A sweep = m-1 steps (m = number of blocks rounded up to even).  Converged when a whole sweep rotates nothing
-//     (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
-// n <= 112: A and V live in shared memory (XOR-swizzled so that every fragment load/store pattern used below is
-// bank-conflict free).  Larger n: same code on a per-CTA global workspace (L2 resident for moderate n).
+// Two-sided BLOCK Jacobi, one CTA per matrix, software-pipelined over the steps of the block tournament.
+//   * The n x n matrix is cut into 8-wide blocks.  A round-robin tournament (jacobi_schedule.cuh) pairs the blocks;
+//     each pair (I,J) is a "slot" with a 16x16 symmetric pivot sub-problem S = A[IJ,IJ].
+//   * Pivot solve (one warp per slot): one full Brent-Luk sweep of S (15 rounds of 8 disjoint rotations, classical
+//     rotation angle, division-free), accumulating the 16x16 orthogonal Q.  It is latency bound.
+//   * Apply (all warps, dynamic work queue): A <- Q^T A Q tile by tile (one tile per slot pair; the mirror image is
+//     stored too) and V <- V Q, as fp64 tensor-core products (mma.sync m8n8k4 = DMMA, which runs at the full FP64
+//     rate of the SM with operands distributed over the warp).  The accumulator fragment of the first product is
+//     re-used directly as the B fragment of the second one (the k index of an MMA may be permuted freely), so a
+//     two-sided tile update needs no shuffle and no shared-memory round trip.
+//   * Pipeline: the pivot of a slot of step g+1 only needs ONE tile of step g (its "critical" tile) besides the
+//     diagonal blocks.  In phase g the first warps update their critical tile and go straight on to the pivot solve
+//     of step g+1 (into the other Q buffer) while the remaining warps work through the other tiles and the V
+//     updates of step g; one __syncthreads per step.
+//   * A sweep = m-1 steps.  Converged when a whole sweep rotates nothing (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
+// n <= 104: A and V live in shared memory; larger n: same code on a per-CTA global workspace kept L2 resident.
 //
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
-// Jacobi"); blocking, tensor-core application and the schedule are this library's design.
+// Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
 #include <math.h>
+#include "jacobi_schedule.cuh"
 #include "wpcd_internal.cuh"
 
 namespace {
 
+// Optional cycle counters (only in profiling builds, -DWPCD_PROFILE), accumulated by CTA 0:
+//   [0] whole steps (thread 0), [1] critical tile + pivot solve of warp 1, [2] number of steps,
+//   [3] queue part of warp 15, [4] queue part of warp 1
+#ifdef WPCD_PROFILE
+__device__ long long wpcd_prof[8];
+#define WPCD_PROF_ADD(k, v) atomicAdd((unsigned long long*)&wpcd_prof[k], (unsigned long long)(v))
+#endif
+
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
-constexpr int LDQ = 20;   // row stride of a slot's Q (doubles); == 4 mod 16 -> conflict-free fragment loads
-constexpr int LDSS = 17;  // row stride of the warp-private 16x16 pivot block
+constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), columns XOR-swizzled by the storage row
+constexpr int LDSS = 18;  // row stride of the warp-private 16x16 pivot block (even: 16-byte aligned row pairs)
+constexpr int kQSlot = 16 * LDQ;
+constexpr int kPivotSmsp = 2;                          // SM sub-partitions reserved for the pivot solves
+constexpr int kPivotWarps = kWarps / 4 * kPivotSmsp;   // warps that solve pivots
 
-// XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
+// A: XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
 __device__ __forceinline__ int swz(int r, int c) { return c ^ (((r & 6) << 1) ^ ((r & 1) << 3)); }
 
 __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
@@ -36,41 +50,31 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
                : "d"(a), "d"(b));
 }
 
-// storage row of logical row k inside a slot's Q: within each group of 8 rows the order is 0,2,4,6,1,3,5,7 so that
-// the k-chunks {8c+2t+r : t=0..3} used by the MMAs are 4 consecutive storage rows.
+// Q layout: logical row k sits in storage row qrow(k) -- within each group of 8 rows the order is 0,2,4,6,1,3,5,7 so
+// that the k-chunks {8c+2t+r : t=0..3} used by the MMAs are 4 consecutive storage rows -- and column c of storage
+// row sr sits at c ^ ((sr & 3) << 2), which makes the B-fragment loads bank-conflict free with LDQ = 16.
 __device__ __forceinline__ int qrow(int k) { return (k & 8) | ((k & 1) << 2) | ((k >> 1) & 3); }
 
-// Round-robin tournament (circle method) for m players, step t in [0,m-1), slot s in [0,m/2).
-__device__ __forceinline__ void rr_pair(int m, int t, int s, int& a, int& b) {
-  if (s == 0) { a = m - 1; b = t; }
-  else { a = (t + s) % (m - 1); b = (t - s + (m - 1)) % (m - 1); }
-}
-
 struct Smem {
-  double* A;     // [np][ld] swizzled (shared or global)
-  double* V;     // [np][ld] swizzled
-  double* Q;     // [nslots][16][LDQ]
-  double* S;     // [kWarps][16][LDSS]
+  double* A;     // [np][ld] swizzled, full symmetric (shared or global)
+  double* V;     // [np][ldv] plain (shared or global)
+  double* Q;     // [2][nslots][16][LDQ] (shared or global), double buffered over the steps
+  double* S;     // [min(nslots,kWarps)][16][LDSS]
   double* wsort; // [np]
-  int* slotI;    // [nslots]
-  int* slotJ;    // [nslots]
-  int* rot;      // [nslots]
+  int* rot;      // [2][nslots] slot rotated something
   int* src;      // [np]
-  int* ctr;      // [4]: 0 = work queue, 1 = rotations this sweep
-  uchar2* pq;    // [15*8] pair table of the pivot sweep
+  int* ctr;      // [0..1] work queues (step parity), [2..3] rotations per sweep (sweep parity)
 };
 
-// ---------------------------------------------------------------------------------------------- phase 1
-// Pair table of one full sweep of a 16x16 pivot: 15 rounds of 8 disjoint pairs (p < q).  Rounds 0..7 take the 64
-// "cross" pairs (i in block I, j in block J), rounds 8..14 the pairs inside I and inside J (two 8-player round-robin
-// tournaments side by side), so every pair is met exactly once.
-__device__ __forceinline__ void pivot_pair(int r, int j, int& p, int& q) {
-  if (r < 8) { p = j; q = 8 + ((j + r) & 7); return; }
-  int a, b;
-  rr_pair(8, r - 8, j >> 1, a, b);
-  const int off = (j & 1) << 3;
-  p = off + (a < b ? a : b);
-  q = off + (a < b ? b : a);
+// ---------------------------------------------------------------------------------------------- pivot solve
+// Tournament of one full sweep of a 16x16 pivot (Brent-Luk): positions 0..15, pair j = positions (2j, 2j+1); after
+// every round the data moves to position kPi(x) (position 0 stays, the other 15 rotate), so that after 15 rounds every
+// pair has met exactly once and everything is back where it started.  The addressing of a round is therefore static.
+__device__ __forceinline__ int kPi(int x) {
+  if (x == 0) return 0;
+  if (x == 1) return 2;
+  if (x == 14) return 15;
+  return (x & 1) ? x - 2 : x + 2;
 }
 
 // Jacobi rotation annihilating a_pq (classical choice |angle| <= pi/4, "Jacobi method"), written with two
@@ -87,31 +91,49 @@ __device__ __forceinline__ void rotation(double app, double aqq, double apq, dou
 }
 
 // One warp: load S = A[IJ,IJ], run one full sweep (15 rounds of 8 simultaneous rotations), write S back, leave the
-// accumulated 16x16 rotation product in the slot's Q.  Lane (k0 = lane>>3, j = lane&7) owns the 2x2 blocks
+// accumulated 16x16 rotation product in Q (identity on entry; rows are storage rows).  Returns (warp-uniform)
+// whether anything was rotated.  Lane (k0 = lane>>3, j = lane&7) owns the 2x2 blocks
 // (row pair k0, column pair j) and (row pair k0+4, column pair j) of S and rows k0, k0+4, k0+8, k0+12 of Q; one
-// round = S <- R^T S R, Q <- Q R with R the product of the round's 8 disjoint rotations, one __syncwarp per round.
-__device__ void inner_solve(const Smem& sm, int ld, int slot, int I, int J, double tol, int lane, int warp) {
-  double* S = sm.S + warp * 16 * LDSS;  // warp < min(nslots, kWarps)
-  double* Q = sm.Q + slot * 16 * LDQ;
+// round = S <- R^T S R, Q <- Q R with R the product of the round's 8 disjoint rotations, results stored at the
+// positions of the next round.
+__device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, double* __restrict__ S, double* __restrict__ Q, int I,
+                            int J, double tol, int lane) {
   for (int e = lane; e < 256; e += 32) {
     int a = e >> 4, b = e & 15;
     int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-    S[a * LDSS + b] = sm.A[(size_t)r * ld + swz(r, c)];
+    S[a * LDSS + b] = A[(size_t)r * ld + swz(r, c)];
   }
   __syncwarp();
   const int j = lane & 7, k0 = lane >> 3;
   const double tol2 = tol * tol;
+  // static addresses: loads at (row pair, column pair), stores at the permuted positions
+  const double* ldD = S + (2 * j) * LDSS + 2 * j;
+  const double* ldA = S + (2 * k0) * LDSS + 2 * j;
+  const double* ldB = S + (2 * k0 + 8) * LDSS + 2 * j;
+  const int qx = k0 << 2;  // Q column swizzle of this lane's storage rows: (k0 + 4u) & 3 == k0
+  const double* ldQ = Q + k0 * LDQ + ((2 * j) ^ qx);
+  const int cp = kPi(2 * j), cq = kPi(2 * j + 1);
+  double* stA0 = S + kPi(2 * k0) * LDSS;
+  double* stA1 = S + kPi(2 * k0 + 1) * LDSS;
+  double* stB0 = S + kPi(2 * k0 + 8) * LDSS;
+  double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
+  double* stQp = Q + k0 * LDQ + (cp ^ qx);
+  double* stQq = Q + k0 * LDQ + (cq ^ qx);
+  const bool diagA = (k0 == j), diagB = (k0 + 4 == j);
   bool any = false;
 #pragma unroll 1
   for (int r = 0; r < 15; ++r) {
-    const uchar2 pj = sm.pq[r * 8 + j], pa = sm.pq[r * 8 + k0], pb = sm.pq[r * 8 + k0 + 4];
-    const int p = pj.x, q = pj.y;
-    const double app = S[p * LDSS + p], aqq = S[q * LDSS + q], apq = S[p * LDSS + q];
-    double ba[4], bb[4], qx[4], qy[4];
-    ba[0] = S[pa.x * LDSS + p]; ba[1] = S[pa.x * LDSS + q]; ba[2] = S[pa.y * LDSS + p]; ba[3] = S[pa.y * LDSS + q];
-    bb[0] = S[pb.x * LDSS + p]; bb[1] = S[pb.x * LDSS + q]; bb[2] = S[pb.y * LDSS + p]; bb[3] = S[pb.y * LDSS + q];
+    const double2 d0 = *reinterpret_cast<const double2*>(ldD);
+    const double2 d1 = *reinterpret_cast<const double2*>(ldD + LDSS);
+    const double2 a0 = *reinterpret_cast<const double2*>(ldA);
+    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDSS);
+    const double2 b0 = *reinterpret_cast<const double2*>(ldB);
+    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDSS);
+    double2 qv[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { qx[u] = Q[(k0 + 4 * u) * LDQ + p]; qy[u] = Q[(k0 + 4 * u) * LDQ + q]; }
+    for (int u = 0; u < 4; ++u) qv[u] = *reinterpret_cast<const double2*>(ldQ + 4 * u * LDQ);
+    __syncwarp();  // every lane has read its inputs before anybody stores
+    const double app = d0.x, apq = d0.y, aqq = d1.y;
     // pivot test |a_pq| > tol sqrt(|a_pp a_qq|), squared
     const bool doit = apq * apq > tol2 * fabs(app * aqq);
     double c, s, t;
@@ -121,25 +143,25 @@ __device__ void inner_solve(const Smem& sm, int ld, int slot, int I, int J, doub
     const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
     const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
     {  // block (k0, j)
-      double x00 = c * ba[0] - s * ba[1], x01 = s * ba[0] + c * ba[1];
-      double x10 = c * ba[2] - s * ba[3], x11 = s * ba[2] + c * ba[3];
+      double x00 = c * a0.x - s * a0.y, x01 = s * a0.x + c * a0.y;
+      double x10 = c * a1.x - s * a1.y, x11 = s * a1.x + c * a1.y;
       double y00 = ca * x00 - sa * x10, y10 = sa * x00 + ca * x10;
       double y01 = ca * x01 - sa * x11, y11 = sa * x01 + ca * x11;
-      if (k0 == j && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
-      S[pa.x * LDSS + p] = y00; S[pa.x * LDSS + q] = y01; S[pa.y * LDSS + p] = y10; S[pa.y * LDSS + q] = y11;
+      if (diagA && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
+      stA0[cp] = y00; stA0[cq] = y01; stA1[cp] = y10; stA1[cq] = y11;
     }
     {  // block (k0 + 4, j)
-      double x00 = c * bb[0] - s * bb[1], x01 = s * bb[0] + c * bb[1];
-      double x10 = c * bb[2] - s * bb[3], x11 = s * bb[2] + c * bb[3];
+      double x00 = c * b0.x - s * b0.y, x01 = s * b0.x + c * b0.y;
+      double x10 = c * b1.x - s * b1.y, x11 = s * b1.x + c * b1.y;
       double y00 = cb * x00 - sb * x10, y10 = sb * x00 + cb * x10;
       double y01 = cb * x01 - sb * x11, y11 = sb * x01 + cb * x11;
-      if (k0 + 4 == j && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
-      S[pb.x * LDSS + p] = y00; S[pb.x * LDSS + q] = y01; S[pb.y * LDSS + p] = y10; S[pb.y * LDSS + q] = y11;
+      if (diagB && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
+      stB0[cp] = y00; stB0[cq] = y01; stB1[cp] = y10; stB1[cq] = y11;
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      Q[(k0 + 4 * u) * LDQ + p] = c * qx[u] - s * qy[u];
-      Q[(k0 + 4 * u) * LDQ + q] = s * qx[u] + c * qy[u];
+      stQp[4 * u * LDQ] = c * qv[u].x - s * qv[u].y;
+      stQq[4 * u * LDQ] = s * qv[u].x + c * qv[u].y;
     }
     __syncwarp();
   }
@@ -148,16 +170,13 @@ __device__ void inner_solve(const Smem& sm, int ld, int slot, int I, int J, doub
     for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
       int a = e >> 4, b = e & 15;
       int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-      sm.A[(size_t)r * ld + swz(r, c)] = a <= b ? S[a * LDSS + b] : S[b * LDSS + a];
+      A[(size_t)r * ld + swz(r, c)] = a <= b ? S[a * LDSS + b] : S[b * LDSS + a];
     }
   }
-  if (lane == 0) {
-    sm.rot[slot] = anyw ? 1 : 0;
-    if (anyw) atomicAdd(&sm.ctr[1], 1);
-  }
+  return anyw;
 }
 
-// ---------------------------------------------------------------------------------------------- phase 2
+// ---------------------------------------------------------------------------------------------- apply
 // T = A[P1,P2] <- Q1^T T Q2 (P = rows/cols of the slot's one or two blocks), mirrored into A[P2,P1].
 __device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const double* __restrict__ Q1,
                                            const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
@@ -187,7 +206,7 @@ __device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const
         if (c < n2) {
 #pragma unroll
           for (int r = 0; r < 2; ++r) {
-            double a = Q2[(8 * c + 4 * r + t) * LDQ + 8 * mi + g];
+            double a = Q2[(8 * c + 4 * r + t) * LDQ + ((8 * mi + g) ^ (t << 2))];
 #pragma unroll
             for (int ni = 0; ni < 2; ++ni)
               if (ni < n1) dmma(ut[mi][ni], a, r ? tf[ni][c].y : tf[ni][c].x);
@@ -208,7 +227,7 @@ __device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const
         if (c < n1) {
 #pragma unroll
           for (int r = 0; r < 2; ++r) {
-            double a = Q1[(8 * c + 4 * r + t) * LDQ + 8 * mi + g];
+            double a = Q1[(8 * c + 4 * r + t) * LDQ + ((8 * mi + g) ^ (t << 2))];
 #pragma unroll
             for (int nj = 0; nj < 2; ++nj)
               if (nj < n2) dmma(out[mi][nj], a, ut[nj][c][r]);
@@ -239,7 +258,7 @@ __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const do
 #pragma unroll
     for (int r = 0; r < 2; ++r)
 #pragma unroll
-      for (int ni = 0; ni < 2; ++ni) bq[c][r][ni] = (c < nbk && ni < nbk) ? Q[(8 * c + 4 * r + t) * LDQ + 8 * ni + g] : 0.0;
+      for (int ni = 0; ni < 2; ++ni) bq[c][r][ni] = (c < nbk && ni < nbk) ? Q[(8 * c + 4 * r + t) * LDQ + ((8 * ni + g) ^ (t << 2))] : 0.0;
   for (int rb = rb0; rb < rb1; ++rb) {
     const int row = 8 * rb + g;
     double2 vf[2];
@@ -247,7 +266,7 @@ __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const do
     for (int c = 0; c < 2; ++c)
       if (c < nbk) {
         int col = 8 * cb[c] + 2 * t;
-        vf[c] = *reinterpret_cast<const double2*>(V + (size_t)row * ld + swz(row, col));
+        vf[c] = *reinterpret_cast<const double2*>(V + (size_t)row * ld + col);
       }
     double out[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
@@ -263,7 +282,7 @@ __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const do
     for (int ni = 0; ni < 2; ++ni)
       if (ni < nbk) {
         int col = 8 * cb[ni] + 2 * t;
-        *reinterpret_cast<double2*>(V + (size_t)row * ld + swz(row, col)) = make_double2(out[ni][0], out[ni][1]);
+        *reinterpret_cast<double2*>(V + (size_t)row * ld + col) = make_double2(out[ni][0], out[ni][1]);
       }
   }
 }
@@ -274,46 +293,78 @@ struct JacobiParams {
   double* W;
   double* C;
   int* info;
-  double* gwork;  // kGlobal: per-CTA workspace 2*np*ld doubles
-  int n, batch, nb, np, ld, m, nslots, max_sweeps;
+  double* gwork;   // per-CTA global workspace: [A np*ld][V np*ldv] (kGlobal) then [Q 2*nslots*16*LDQ] (q_global)
+  size_t gstride;  // doubles per CTA
+  int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
   double tol;
 };
 
 constexpr int kVRowBlocksPerItem = 2;
 
-template <bool kGlobal>
+// One warp prepares slot sn of step tn: identity into its Q (buffer bn), and for a real pair the critical tile of the
+// running step t (buffer bc) followed by the pivot solve.
+__device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams& P, int tn, int sn, int bn, bool has_cur,
+                                             int t, int bc, int parity, int lane, int widx) {
+  const int m = P.m, nb = P.nb, nslots = P.nslots, ld = P.ld;
+  double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
+  for (int e = lane; e < 256; e += 32) {
+    const int sr = e >> 4, c = e & 15;
+    Qn[sr * LDQ + (c ^ ((sr & 3) << 2))] = (qrow(c) == sr) ? 1.0 : 0.0;
+  }
+  int I, J;
+  slot_blocks(m, nb, tn, sn, I, J);
+  bool rotated = false;
+  if (J >= 0) {
+    if (has_cur) {
+      int s1 = rr_slot_of(m, t, I), s2 = rr_slot_of(m, t, J);
+      if (s1 > s2) { int x = s1; s1 = s2; s2 = x; }
+      if (sm.rot[bc * nslots + s1] | sm.rot[bc * nslots + s2]) {
+        int I1, J1, I2, J2;
+        slot_blocks(m, nb, t, s1, I1, J1);
+        slot_blocks(m, nb, t, s2, I2, J2);
+        const double* Qc = sm.Q + (size_t)bc * nslots * kQSlot;
+        apply_tile(sm.A, ld, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
+      }
+    }
+    __syncwarp();
+    rotated = inner_solve(sm.A, ld, sm.S + widx * 16 * LDSS, Qn, I, J, P.tol, lane);
+  }
+  if (lane == 0) {
+    sm.rot[bn * nslots + sn] = rotated ? 1 : 0;
+    if (rotated) atomicAdd(&sm.ctr[2 + parity], 1);
+  }
+}
+
+template <bool kGlobal, bool kQGlobal>
 __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = P.n, np = P.np, ld = P.ld, nslots = P.nslots, m = P.m;
+  const int n = P.n, np = P.np, ld = P.ld, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
   Smem sm;
   {
     double* d = reinterpret_cast<double*>(smem_raw);
+    double* g = P.gwork + (size_t)blockIdx.x * P.gstride;
     if (kGlobal) {
-      sm.A = P.gwork + (size_t)blockIdx.x * 2 * np * ld;
-      sm.V = sm.A + (size_t)np * ld;
+      sm.A = g; g += (size_t)np * ld;
+      sm.V = g; g += (size_t)np * ldv;
     } else {
       sm.A = d; d += (size_t)np * ld;
-      sm.V = d; d += (size_t)np * ld;
+      sm.V = d; d += (size_t)np * ldv;
     }
-    sm.Q = d; d += (size_t)nslots * 16 * LDQ;
-    sm.S = d; d += (nslots < kWarps ? nslots : kWarps) * 16 * LDSS;
+    if (kQGlobal) sm.Q = g;
+    else { sm.Q = d; d += (size_t)2 * nslots * kQSlot; }
+    sm.S = d; d += (nslots < kPivotWarps ? nslots : kPivotWarps) * 16 * LDSS;
     sm.wsort = d; d += np;
     int* ip = reinterpret_cast<int*>(d);
-    sm.slotI = ip; ip += nslots;
-    sm.slotJ = ip; ip += nslots;
-    sm.rot = ip; ip += nslots;
+    sm.rot = ip; ip += 2 * nslots;
     sm.src = ip; ip += np;
-    sm.ctr = ip; ip += 4;
-    sm.pq = reinterpret_cast<uchar2*>(ip);
+    sm.ctr = ip;
   }
-  if (tid < 120) {
-    int p, q;
-    pivot_pair(tid >> 3, tid & 7, p, q);
-    sm.pq[tid] = make_uchar2((unsigned char)p, (unsigned char)q);
-  }
+  // Pivot solves are latency bound and suffer when DMMAs of the update queue the same FP64 pipe: they run on the
+  // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
+  const int widx = ((warp & 3) < kPivotSmsp) ? (warp >> 2) * kPivotSmsp + (warp & 3) : -1;
   const int ntiles = nslots * (nslots - 1) / 2;
-  const int nvgrp = (P.nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
+  const int nvgrp = (nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
   const int nitems = ntiles + nslots * nvgrp;
 
   for (int mat = blockIdx.x; mat < P.batch; mat += gridDim.x) {
@@ -323,60 +374,80 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
       int r = e / np, c = e - r * np;
       double a = (r < n && c < n) ? H[(size_t)r * n + c] : 0.0;
       sm.A[(size_t)r * ld + swz(r, c)] = a;
-      sm.V[(size_t)r * ld + swz(r, c)] = (r == c) ? 1.0 : 0.0;
+      sm.V[(size_t)r * ldv + c] = (r == c) ? 1.0 : 0.0;
     }
-    int sweeps = 0;
+    if (tid < 4) sm.ctr[tid] = 0;
+    __syncthreads();
+    // prologue: pivots of (sweep 0, step 0) into Q buffer 0
+    if (widx >= 0)
+      for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot(sm, P, 0, sn, 0, false, 0, 0, 0, lane, widx);
+    __syncthreads();
+    int sweeps = 0, buf = 0, gstep = 0;
     bool converged = false;
-    while (sweeps < P.max_sweeps) {
-      __syncthreads();
-      if (tid == 0) sm.ctr[1] = 0;
-      for (int step = 0; step < m - 1; ++step) {
-        // slots of this step, Q = identity
-        for (int s = tid; s < nslots; s += kThreads) {
-          int a, b;
-          rr_pair(m, step, s, a, b);
-          int I = a < b ? a : b, J = a < b ? b : a;
-          if (J >= P.nb) J = -1;
-          if (I >= P.nb) { I = J; J = -1; }  // cannot happen for m <= nb+1, kept for safety
-          sm.slotI[s] = I; sm.slotJ[s] = J; sm.rot[s] = 0;
+    for (;;) {
+      const int par = sweeps & 1;
+      for (int step = 0; step < m - 1; ++step, ++gstep) {
+        const bool last = (step == m - 2);
+        if (last && sm.ctr[2 + par] == 0) { converged = true; break; }  // nothing rotated in this sweep
+        const bool do_next = !(last && sweeps + 1 >= P.max_sweeps);
+        const int tn = last ? 0 : step + 1;
+        const int parn = last ? (par ^ 1) : par;
+        if (tid == 0) {
+          sm.ctr[(gstep + 1) & 1] = 0;
+          if (step == 0) sm.ctr[2 + (par ^ 1)] = 0;
         }
-        for (int e = tid; e < nslots * 16 * LDQ; e += kThreads) {
-          int rr = (e / LDQ) & 15, cc = e % LDQ;
-          sm.Q[e] = (cc < 16 && qrow(cc) == rr) ? 1.0 : 0.0;
-        }
-        if (tid == 0) sm.ctr[0] = 0;
-        __syncthreads();
-        for (int s = warp; s < nslots; s += kWarps)
-          if (sm.slotJ[s] >= 0) inner_solve(sm, ld, s, sm.slotI[s], sm.slotJ[s], P.tol, lane, warp);
-        __syncthreads();
-        // dynamic queue over tiles (s1 < s2) and V items
+#ifdef WPCD_PROFILE
+        long long tk0 = clock64();
+#endif
+        // pivots of the next step (critical tile first), overlapped with the rest of this step's updates
+        if (do_next && widx >= 0)
+          for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot(sm, P, tn, sn, buf ^ 1, true, step, buf, parn, lane, widx);
+#ifdef WPCD_PROFILE
+        if (blockIdx.x == 0 && tid == 32) WPCD_PROF_ADD(1, clock64() - tk0);
+        long long tk1 = clock64();
+#endif
+        const int* rot = sm.rot + buf * nslots;
+        const double* Qc = sm.Q + (size_t)buf * nslots * kQSlot;
+        int* queue = sm.ctr + (gstep & 1);
         for (;;) {
           int it = 0;
-          if (lane == 0) it = atomicAdd(&sm.ctr[0], 1);
+          if (lane == 0) it = atomicAdd(queue, 1);
           it = __shfl_sync(0xffffffffu, it, 0);
           if (it >= nitems) break;
           if (it < ntiles) {
-            // unrank (s1 < s2)
-            int s1 = 0, rem = it;
+            int s1 = 0, rem = it;  // unrank (s1 < s2)
             while (rem >= nslots - 1 - s1) { rem -= nslots - 1 - s1; ++s1; }
-            int s2 = s1 + 1 + rem;
-            if (sm.rot[s1] | sm.rot[s2])
-              apply_tile(sm.A, ld, sm.Q + s1 * 16 * LDQ, sm.Q + s2 * 16 * LDQ, sm.slotI[s1], sm.slotJ[s1], sm.slotI[s2],
-                         sm.slotJ[s2], lane);
+            const int s2 = s1 + 1 + rem;
+            if (!(rot[s1] | rot[s2])) continue;
+            if (do_next && critical_slot(m, nb, step, tn, s1, s2) >= 0) continue;  // done by the pivot warp
+            int I1, J1, I2, J2;
+            slot_blocks(m, nb, step, s1, I1, J1);
+            slot_blocks(m, nb, step, s2, I2, J2);
+            if (I1 < 0 || I2 < 0) continue;
+            apply_tile(sm.A, ld, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
           } else {
-            int v = it - ntiles;
-            int s = v / nvgrp, grp = v - s * nvgrp;
-            if (sm.rot[s]) {
-              int rb0 = grp * kVRowBlocksPerItem, rb1 = rb0 + kVRowBlocksPerItem;
-              if (rb1 > P.nb) rb1 = P.nb;
-              apply_V(sm.V, ld, sm.Q + s * 16 * LDQ, sm.slotI[s], sm.slotJ[s], rb0, rb1, lane);
-            }
+            const int v = it - ntiles;
+            const int s = v / nvgrp, grp = v - s * nvgrp;
+            if (!rot[s]) continue;
+            int I, J;
+            slot_blocks(m, nb, step, s, I, J);
+            int rb0 = grp * kVRowBlocksPerItem, rb1 = rb0 + kVRowBlocksPerItem;
+            if (rb1 > nb) rb1 = nb;
+            apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rb0, rb1, lane);
           }
         }
+#ifdef WPCD_PROFILE
+        if (blockIdx.x == 0 && tid == 480) WPCD_PROF_ADD(3, clock64() - tk1);
+        if (blockIdx.x == 0 && tid == 32) WPCD_PROF_ADD(4, clock64() - tk1);
+#endif
         __syncthreads();
+#ifdef WPCD_PROFILE
+        if (blockIdx.x == 0 && tid == 0) { WPCD_PROF_ADD(0, clock64() - tk0); WPCD_PROF_ADD(2, 1); }
+#endif
+        buf ^= 1;
       }
       ++sweeps;
-      if (sm.ctr[1] == 0) { converged = true; break; }
+      if (converged || sweeps >= P.max_sweeps) break;
     }
     // eigenvalues = diagonal; rank sort ascending (ties by index); gather columns
     __syncthreads();
@@ -398,66 +469,105 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
     for (int e = tid; e < n * n; e += kThreads) {
       int i = e / n, k = e - i * n;
       int c = sm.src[k];
-      Co[e] = sm.V[(size_t)i * ld + swz(i, c)];
+      Co[e] = sm.V[(size_t)i * ldv + c];
     }
     if (tid == 0) P.info[mat] = converged ? sweeps : -1;
   }
 }
 
-struct Geometry { int nb, np, ld, m, nslots; size_t smem_fixed, smem_mat; };
+struct Geometry {
+  int nb, np, ld, ldv, m, nslots;
+  size_t smem_fixed, smem_q, smem_mat;  // bytes
+  bool mat_global, q_global;
+  size_t gstride;  // doubles of global workspace per CTA
+  size_t smem;     // dynamic shared memory of the launch
+};
 
-Geometry geometry(int n) {
+Geometry geometry(const WpcdHandle* h, int n) {
   Geometry g;
   g.nb = (n + 7) / 8;
   if (g.nb < 2) g.nb = 2;
   g.np = 8 * g.nb;
   g.ld = (g.np + 15) / 16 * 16;
+  g.ldv = (g.np % 16 == 8) ? g.np : g.np + 8;  // == 8 mod 16: conflict-free row-fragment access without swizzle
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
+  if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
-  g.smem_fixed = (size_t)g.nslots * 16 * LDQ * 8 + (size_t)(g.nslots < kWarps ? g.nslots : kWarps) * 16 * LDSS * 8 + (size_t)g.np * 8 +
-                 (size_t)(3 * g.nslots + g.np + 4) * 4 + 240 + 64;
-  g.smem_mat = (size_t)2 * g.np * g.ld * 8;
+  const int nS = g.nslots < kPivotWarps ? g.nslots : kPivotWarps;
+  g.smem_fixed = (size_t)nS * 16 * LDSS * 8 + (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
+  g.smem_q = (size_t)2 * g.nslots * kQSlot * 8;
+  g.smem_mat = ((size_t)g.np * g.ld + (size_t)g.np * g.ldv) * 8;
+  const size_t cap = (size_t)h->max_smem_optin;
+  g.mat_global = g.smem_fixed + g.smem_q + g.smem_mat > cap;
+  g.q_global = g.mat_global && (g.smem_fixed + g.smem_q > cap);
+  g.gstride = (g.mat_global ? g.smem_mat / 8 : 0) + (g.q_global ? g.smem_q / 8 : 0);
+  g.smem = g.smem_fixed + (g.q_global ? 0 : g.smem_q) + (g.mat_global ? 0 : g.smem_mat);
   return g;
 }
 
-// CTAs of the global-workspace path: two per SM while all their workspaces together stay well inside the 126 MB L2.
+// CTAs of the global-workspace path: two per SM while all their workspaces together stay well inside the 126 MB L2
+// (and two CTAs' shared memory fits one SM).
 int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
-  int per_sm = ((size_t)2 * h->num_sms * g.smem_mat <= ((size_t)80 << 20)) ? 2 : 1;
-  int grid = per_sm * h->num_sms;
+  const bool two = ((size_t)2 * h->num_sms * g.gstride * 8 <= ((size_t)80 << 20)) && (2 * (g.smem + 1024) <= (size_t)h->max_smem_optin);
+  const int grid = (two ? 2 : 1) * h->num_sms;
   return batch < grid ? batch : grid;
 }
 
 }  // namespace
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
-  Geometry g = geometry(n);
-  if (g.smem_fixed + g.smem_mat <= (size_t)h->max_smem_optin) return 0;
-  int grid = global_grid(h, g, batch);
-  return (size_t)grid * g.smem_mat;
+  Geometry g = geometry(h, n);
+  if (!g.mat_global) return 0;
+  return (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
 
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                        double tol, int max_sweeps, void* d_work, size_t work_bytes, cudaStream_t st) {
-  Geometry g = geometry(n);
+  Geometry g = geometry(h, n);
+  if (g.smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   JacobiParams P;
-  P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gwork = static_cast<double*>(d_work);
-  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.m = g.m; P.nslots = g.nslots;
+  P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gwork = static_cast<double*>(d_work); P.gstride = g.gstride;
+  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
-  const bool in_smem = g.smem_fixed + g.smem_mat <= (size_t)h->max_smem_optin;
   int rc;
-  if (in_smem) {
-    size_t smem = g.smem_fixed + g.smem_mat;
-    rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "jacobi attr");
+  if (!g.mat_global) {
+    rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
     if (rc) return rc;
-    k_jacobi<false><<<batch, kThreads, smem, st>>>(P);
+    k_jacobi<false, false><<<batch, kThreads, g.smem, st>>>(P);
   } else {
-    if (g.smem_fixed > (size_t)h->max_smem_optin) return WPCD_ESIZE;
-    int grid = global_grid(h, g, batch);
-    if (work_bytes < (size_t)grid * g.smem_mat) return WPCD_EWORK;
-    rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem_fixed), "jacobi attr");
-    if (rc) return rc;
-    k_jacobi<true><<<grid, kThreads, g.smem_fixed, st>>>(P);
+    const int grid = global_grid(h, g, batch);
+    if (work_bytes < (size_t)grid * g.gstride * 8) return WPCD_EWORK;
+    if (g.q_global) {
+      rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
+      if (rc) return rc;
+      k_jacobi<true, true><<<grid, kThreads, g.smem, st>>>(P);
+    } else {
+      rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
+      if (rc) return rc;
+      k_jacobi<true, false><<<grid, kThreads, g.smem, st>>>(P);
+    }
   }
   return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch");
 }
+
+// Test hooks (host only): the block tournament of jacobi_schedule.cuh, see include/wpcd.h.
+extern "C" int wpcd_jacobi_schedule(int m, int nb, int t, int s, int* I, int* J) {
+  if (m < 6 || (m & 1) || t < 0 || t >= m - 1 || s < 0 || s >= m / 2 || !I || !J) return WPCD_EINVAL;
+  slot_blocks(m, nb, t, s, *I, *J);
+  return WPCD_OK;
+}
+extern "C" int wpcd_jacobi_critical_slot(int m, int nb, int t, int tn, int s1, int s2) {
+  if (m < 6 || (m & 1) || s1 < 0 || s2 <= s1 || s2 >= m / 2) return WPCD_EINVAL;
+  return critical_slot(m, nb, t, tn, s1, s2);
+}
+
+#ifdef WPCD_PROFILE
+extern "C" int wpcd_debug_read_prof(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, wpcd_prof, sizeof(long long) * 8);
+}
+extern "C" int wpcd_debug_clear_prof() {
+  long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  return (int)cudaMemcpyToSymbol(wpcd_prof, z, sizeof(z));
+}
+#endif

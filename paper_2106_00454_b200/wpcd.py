@@ -6,7 +6,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libwpcd.so")
+# WPCD_LIBRARY selects another build of the same C ABI (e.g. one compiled with -DWPCD_PROFILE)
+_LIBPATH = os.environ.get("WPCD_LIBRARY") or os.path.join(_HERE, "libwpcd.so")
 
 MAX_TERMS = 4
 MAX_CHANNELS = 16
