@@ -100,8 +100,9 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
 
 /* Step (ii), Eq. 21.  Batched real-symmetric eigendecomposition by two-sided block-Jacobi (8-wide blocks paired in
  * a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered Jacobi sweep inside one warp; the
- * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products).  n <= 112: one CTA per
- * matrix, matrix and eigenvectors resident in shared memory; larger n: same algorithm through a global workspace.
+ * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products; the pivots of the next step
+ * are solved while the current step's updates run).  n <= 104: one CTA per matrix, matrix and eigenvectors resident
+ * in shared memory; larger n: same algorithm through a global workspace kept L2 resident.
  *   d_A    : [batch][n][n] input (only read; must be symmetric)
  *   d_W    : [batch][n] eigenvalues ascending
  *   d_C    : [batch][n][n] eigenvectors, column k belongs to d_W[k]  (C_ij = <x_i|z_j>)
@@ -131,6 +132,15 @@ int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_
  *   d_S     : optional (may be NULL) S-matrix, same layout as d_T */
 int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
                       const double* d_dE, double* d_delta, double* d_S, void* stream);
+
+/* Test hooks (host only, no GPU needed): the block tournament that wpcd_diag_batched runs (csrc/jacobi_schedule.cuh).
+ * m = number of players (8-wide blocks, even, >= 6; players >= nb are padding), a sweep has m-1 steps of m/2 slots.
+ *   wpcd_jacobi_schedule      : blocks (I < J) of slot s at step t; J = -1 single block, I = J = -1 empty slot.
+ *   wpcd_jacobi_critical_slot : if the tile of slots (s1 < s2) at step t holds the off-diagonal block of a real
+ *                               pivot of step tn, that pivot's slot at step tn, else -1 (WPCD_EINVAL on bad input).
+ * Invariants (tests/test_abi_cpu.py): every pair of blocks meets exactly once per sweep; at most one pivot per tile. */
+int wpcd_jacobi_schedule(int m, int nb, int t, int s, int* I, int* J);
+int wpcd_jacobi_critical_slot(int m, int nb, int t, int tn, int s1, int s2);
 
 #ifdef __cplusplus
 }

@@ -49,3 +49,50 @@ def test_binding_does_not_import_oracle():
         src = open(os.path.join(ROOT, "paper_2106_00454_b200", fn)).read()
         assert not re.search(r"^\s*(from|import)\s+\.*oracle", src, flags=re.M), fn
         assert "liboracle" not in src, fn
+
+
+def test_jacobi_block_tournament_invariants():
+    """Host logic of wpcd_diag_batched's schedule through the C-ABI test hooks: in a sweep every pair of real blocks
+    meets exactly once, every block sits in at most one slot per step, and the pipelining rule holds -- every real
+    pivot of the next step is fed by exactly one tile of the running step and no tile feeds two pivots."""
+    from paper_2106_00454_b200 import build
+    lib = ctypes.CDLL(build.build())
+    I, J = ctypes.c_int(), ctypes.c_int()
+    for nb in (2, 3, 5, 6, 7, 13, 25, 26, 50, 100):
+        m = max(6, nb + (nb & 1))
+        met = set()
+        for t in range(m - 1):
+            slots, seen = [], set()
+            for s in range(m // 2):
+                assert lib.wpcd_jacobi_schedule(m, nb, t, s, ctypes.byref(I), ctypes.byref(J)) == 0
+                slots.append((I.value, J.value))
+                for b in (I.value, J.value):
+                    if b >= 0:
+                        assert 0 <= b < nb and b not in seen
+                        seen.add(b)
+                if J.value >= 0:
+                    assert I.value < J.value and (I.value, J.value) not in met
+                    met.add((I.value, J.value))
+            assert seen == set(range(nb))                       # every real block sits somewhere
+            tn = (t + 1) % (m - 1)
+            nxt = []
+            for s in range(m // 2):
+                lib.wpcd_jacobi_schedule(m, nb, tn, s, ctypes.byref(I), ctypes.byref(J))
+                nxt.append((I.value, J.value))
+            fed = {}
+            for s1 in range(m // 2):
+                for s2 in range(s1 + 1, m // 2):
+                    cs = lib.wpcd_jacobi_critical_slot(m, nb, t, tn, s1, s2)
+                    blocks1 = {b for b in slots[s1] if b >= 0}
+                    blocks2 = {b for b in slots[s2] if b >= 0}
+                    # brute force: real pivots of step tn with one block in each of the two slots
+                    want = [k for k, (a, b) in enumerate(nxt)
+                            if b >= 0 and ((a in blocks1 and b in blocks2) or (a in blocks2 and b in blocks1))]
+                    assert len(want) <= 1
+                    assert cs == (want[0] if want else -1), (nb, t, s1, s2, cs, want)
+                    if cs >= 0:
+                        assert cs not in fed
+                        fed[cs] = (s1, s2)
+            assert set(fed) == {k for k, (a, b) in enumerate(nxt) if b >= 0}
+        assert met == {(a, b) for a in range(nb) for b in range(a + 1, nb)}
+    assert lib.wpcd_jacobi_schedule(4, 4, 0, 0, ctypes.byref(I), ctypes.byref(J)) == -1   # m < 6 rejected

@@ -66,6 +66,13 @@ def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguc
     assert np.array_equal(g["H"][s, c], g["H"][s, c].T), (label, "H symmetric")
     assert g["info"][s, c] >= 1, (label, "info", g["info"][s, c])
     errW = hp.check_eig(g["W"][s, c], ref["W"], normH)
+    if errW > hp.TOL_EIG_REL:
+        # DESIGN.md section 3 "eigenvalue arbitration": at large n the fp64 oracle's own rounding error on the smallest
+        # eigenvalues exceeds 1e-11; the 80-bit run of the same oracle algorithm decides.
+        from oracle import oracle as o
+        W_ld = o.jacobi_ld(ch["H"])[0]
+        errW, err_oracle = hp.check_eig(g["W"][s, c], W_ld, normH), hp.check_eig(ref["W"], W_ld, normH)
+        print(label, "eig arbitration vs long double: gpu", errW, "fp64 oracle", err_oracle)
     assert errW <= hp.TOL_EIG_REL, (label, "eig", errW)
     C = g["C"][s, c]
     assert np.abs(C.T @ C - np.eye(n)).max() < 1e-12, (label, "orth")
