@@ -77,17 +77,30 @@ __device__ __forceinline__ int kPi(int x) {
   return (x & 1) ? x - 2 : x + 2;
 }
 
+// 1/sqrt(x) for normal x > 0 without the library routine's special-case branch: MUFU.RSQ64H seed (2^-22) and one
+// third-order correction y (1 + e/2 + 3e^2/8), e = 1 - x y^2, i.e. full double precision.  x = 0 gives inf.
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(x, -(y * y), 1.0);
+  return fma(fma(e, 0.375, 0.5), y * e, y);
+}
+
 // Jacobi rotation annihilating a_pq (classical choice |angle| <= pi/4, "Jacobi method"), written with two
 // reciprocal square roots and no division:  with d = a_qq - a_pp, b = 2 a_pq, h = sqrt(d^2 + b^2):
 //   cos 2phi = |d|/h,  c = sqrt((1 + cos 2phi)/2),  s = sgn(d) (b/h)/(2c),  t = s/c.
-__device__ __forceinline__ void rotation(double app, double aqq, double apq, double& c, double& s, double& t) {
+// Pivot test |a_pq| > tol sqrt(|a_pp a_qq|) (squared); below it the identity is returned.
+__device__ __forceinline__ bool rotation(double app, double aqq, double apq, double tol2, double& c, double& s, double& t) {
+  const bool doit = apq * apq > tol2 * fabs(app * aqq);
   const double d = aqq - app, b = apq + apq;
-  const double rh = rsqrt(fma(d, d, b * b));
+  const double rh = rsqrt_nr(fma(d, d, b * b));
   const double c2 = fma(0.5 * fabs(d), rh, 0.5);
-  const double rc = rsqrt(c2);
-  c = c2 * rc;
-  s = copysign(0.5, d) * b * rh * rc;
-  t = s * rc;
+  const double rc = rsqrt_nr(c2);
+  const double bh = copysign(0.5, d) * b * rh;
+  c = doit ? c2 * rc : 1.0;
+  s = doit ? bh * rc : 0.0;
+  t = doit ? bh * rc * rc : 0.0;
+  return doit;
 }
 
 // One warp: load S = A[IJ,IJ], run one full sweep (15 rounds of 8 simultaneous rotations), write S back, leave the
@@ -120,11 +133,25 @@ __device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, doub
   double* stQp = Q + k0 * LDQ + (cp ^ qx);
   double* stQq = Q + k0 * LDQ + (cq ^ qx);
   const bool diagA = (k0 == j), diagB = (k0 + 4 == j);
+  // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
+  // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
+  // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
+  // right after this round's update, so that the next rotation (a long dependent chain) overlaps this round's stores.
+  //   j:      0      1      2..6            7
+  //   x, y:   0,3    1,5    2j-2, 2j+3      12,14
+  const int src_pp = j > 0 ? j - 1 : 0, src_qq = j < 7 ? j + 1 : 7;
+  const int own_src = (int)((0x170F061D140B0201ull >> (8 * j)) & 0xff);  // lanes 1,2,11,20,29,6,15,23
+  const int own_sel = lane == 2 ? 1 : ((lane == 6 || lane == 15) ? 2 : (lane == 23 ? 3 : 0));  // yA01,yA11,yB01,yB00
+  double app, aqq, apq, c, s, t;
+  {
+    const double2 d0 = *reinterpret_cast<const double2*>(S + (2 * j) * LDSS + 2 * j);
+    const double2 d1 = *reinterpret_cast<const double2*>(S + (2 * j + 1) * LDSS + 2 * j);
+    app = d0.x; apq = d0.y; aqq = d1.y;
+  }
+  bool doit = rotation(app, aqq, apq, tol2, c, s, t);
   bool any = false;
 #pragma unroll 1
   for (int r = 0; r < 15; ++r) {
-    const double2 d0 = *reinterpret_cast<const double2*>(ldD);
-    const double2 d1 = *reinterpret_cast<const double2*>(ldD + LDSS);
     const double2 a0 = *reinterpret_cast<const double2*>(ldA);
     const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDSS);
     const double2 b0 = *reinterpret_cast<const double2*>(ldB);
@@ -133,36 +160,39 @@ __device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, doub
 #pragma unroll
     for (int u = 0; u < 4; ++u) qv[u] = *reinterpret_cast<const double2*>(ldQ + 4 * u * LDQ);
     __syncwarp();  // every lane has read its inputs before anybody stores
-    const double app = d0.x, apq = d0.y, aqq = d1.y;
-    // pivot test |a_pq| > tol sqrt(|a_pp a_qq|), squared
-    const bool doit = apq * apq > tol2 * fabs(app * aqq);
-    double c, s, t;
-    rotation(app, aqq, apq, c, s, t);
-    if (!doit) { c = 1.0; s = 0.0; t = 0.0; }
     any |= doit;
     const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
     const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
-    {  // block (k0, j)
-      double x00 = c * a0.x - s * a0.y, x01 = s * a0.x + c * a0.y;
-      double x10 = c * a1.x - s * a1.y, x11 = s * a1.x + c * a1.y;
-      double y00 = ca * x00 - sa * x10, y10 = sa * x00 + ca * x10;
-      double y01 = ca * x01 - sa * x11, y11 = sa * x01 + ca * x11;
-      if (diagA && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
-      stA0[cp] = y00; stA0[cq] = y01; stA1[cp] = y10; stA1[cq] = y11;
-    }
-    {  // block (k0 + 4, j)
-      double x00 = c * b0.x - s * b0.y, x01 = s * b0.x + c * b0.y;
-      double x10 = c * b1.x - s * b1.y, x11 = s * b1.x + c * b1.y;
-      double y00 = cb * x00 - sb * x10, y10 = sb * x00 + cb * x10;
-      double y01 = cb * x01 - sb * x11, y11 = sb * x01 + cb * x11;
-      if (diagB && doit) { y00 = app - t * apq; y11 = aqq + t * apq; y01 = 0.0; y10 = 0.0; }
-      stB0[cp] = y00; stB0[cq] = y01; stB1[cp] = y10; stB1[cq] = y11;
-    }
+    const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
+    // block (k0, j)
+    double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
+    double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
+    double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
+    double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
+    if (diagA && doit) { ya00 = dtop; ya11 = dbot; ya01 = 0.0; ya10 = 0.0; }
+    // block (k0 + 4, j)
+    double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
+    double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
+    double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
+    double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
+    if (diagB && doit) { yb00 = dtop; yb11 = dbot; yb01 = 0.0; yb10 = 0.0; }
+    // next round's pivot by shuffle
+    const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
+    double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
+    double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
+    const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
+    if (j == 0) appn = dtop;
+    if (j == 7) aqqn = dtop;
+    // this round's stores, at the positions of the next round
+    stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
+    stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       stQp[4 * u * LDQ] = c * qv[u].x - s * qv[u].y;
       stQq[4 * u * LDQ] = s * qv[u].x + c * qv[u].y;
     }
+    app = appn; aqq = aqqn; apq = apqn;
+    doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
     __syncwarp();
   }
   const bool anyw = __any_sync(0xffffffffu, any);
