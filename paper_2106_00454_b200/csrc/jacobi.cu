@@ -38,7 +38,7 @@ constexpr int kWarps = kThreads / 32;
 constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), columns XOR-swizzled by the storage row
 constexpr int LDSS = 18;  // row stride of the warp-private 16x16 pivot block (even: 16-byte aligned row pairs)
 constexpr int kQSlot = 16 * LDQ;
-constexpr int kPivotSmsp = 2;                          // SM sub-partitions reserved for the pivot solves
+constexpr int kPivotSmsp = 4;                          // SM sub-partitions reserved for the pivot solves
 constexpr int kPivotWarps = kWarps / 4 * kPivotSmsp;   // warps that solve pivots
 
 // A: XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
@@ -119,8 +119,16 @@ __device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, doub
   __syncwarp();
   const int j = lane & 7, k0 = lane >> 3;
   const double tol2 = tol * tol;
+  {  // early exit: no pair of this pivot passes the rotation test (the usual case in the last sweeps)
+    bool need = false;
+    for (int e = lane; e < 256; e += 32) {
+      const int a = e >> 4, b = e & 15;
+      const double x = S[a * LDSS + b];
+      need |= (a < b) && (x * x > tol2 * fabs(S[a * LDSS + a] * S[b * LDSS + b]));
+    }
+    if (!__any_sync(0xffffffffu, need)) return false;
+  }
   // static addresses: loads at (row pair, column pair), stores at the permuted positions
-  const double* ldD = S + (2 * j) * LDSS + 2 * j;
   const double* ldA = S + (2 * k0) * LDSS + 2 * j;
   const double* ldB = S + (2 * k0 + 8) * LDSS + 2 * j;
   const int qx = k0 << 2;  // Q column swizzle of this lane's storage rows: (k0 + 4u) & 3 == k0
