@@ -55,6 +55,50 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
 // row sr sits at c ^ ((sr & 3) << 2), which makes the B-fragment loads bank-conflict free with LDQ = 16.
 __device__ __forceinline__ int qrow(int k) { return (k & 8) | ((k & 1) << 2) | ((k >> 1) & 3); }
 
+// View of the symmetric working matrix A.
+//   kHalf = false: full np x ld array, XOR-swizzled, both triangles kept up to date (mirror stores).
+//   kHalf = true : only the blocks (rb <= cb) are stored, 64 contiguous doubles each (row-major 8x8); a block below the
+//                  diagonal is read/written through its transpose.  Halves the footprint: n = 200 fits shared memory.
+template <bool kHalf>
+struct AView {
+  double* p;
+  int ld, nb;
+  __device__ __forceinline__ size_t blk(int rb, int cb) const { return (size_t)(rb * nb - ((rb * (rb - 1)) >> 1) + (cb - rb)) << 6; }
+  __device__ __forceinline__ double get(int r, int c) const {
+    if (!kHalf) return p[(size_t)r * ld + swz(r, c)];
+    const int rb = r >> 3, cb = c >> 3;
+    return rb <= cb ? p[blk(rb, cb) + ((r & 7) << 3) + (c & 7)] : p[blk(cb, rb) + ((c & 7) << 3) + (r & 7)];
+  }
+  // element (r,c) of a symmetric update where the caller visits BOTH (r,c) and (c,r)
+  __device__ __forceinline__ void put(int r, int c, double v) const {
+    if (!kHalf) { p[(size_t)r * ld + swz(r, c)] = v; return; }
+    const int rb = r >> 3, cb = c >> 3;
+    if (rb <= cb) p[blk(rb, cb) + ((r & 7) << 3) + (c & 7)] = v;
+  }
+  // fragment of the off-diagonal block (rb != cb): rows 8rb+g, columns 8cb+2t, 8cb+2t+1
+  __device__ __forceinline__ double2 load_frag(int rb, int cb, int g, int t) const {
+    if (!kHalf) {
+      const int r = 8 * rb + g, c = 8 * cb + 2 * t;
+      return *reinterpret_cast<const double2*>(p + (size_t)r * ld + swz(r, c));
+    }
+    if (rb < cb) return *reinterpret_cast<const double2*>(p + blk(rb, cb) + (g << 3) + 2 * t);
+    const double* q = p + blk(cb, rb) + (t << 4) + g;
+    return make_double2(q[0], q[8]);
+  }
+  __device__ __forceinline__ void store_frag(int rb, int cb, int g, int t, double v0, double v1) const {
+    if (!kHalf) {
+      const int r = 8 * rb + g, c = 8 * cb + 2 * t;
+      *reinterpret_cast<double2*>(p + (size_t)r * ld + swz(r, c)) = make_double2(v0, v1);
+      p[(size_t)c * ld + swz(c, r)] = v0;
+      p[(size_t)(c + 1) * ld + swz(c + 1, r)] = v1;
+      return;
+    }
+    if (rb < cb) { *reinterpret_cast<double2*>(p + blk(rb, cb) + (g << 3) + 2 * t) = make_double2(v0, v1); return; }
+    double* q = p + blk(cb, rb) + (t << 4) + g;
+    q[0] = v0; q[8] = v1;
+  }
+};
+
 struct Smem {
   double* A;     // [np][ld] swizzled, full symmetric (shared or global)
   double* V;     // [np][ldv] plain (shared or global)
@@ -109,12 +153,13 @@ __device__ __forceinline__ bool rotation(double app, double aqq, double apq, dou
 // (row pair k0, column pair j) and (row pair k0+4, column pair j) of S and rows k0, k0+4, k0+8, k0+12 of Q; one
 // round = S <- R^T S R, Q <- Q R with R the product of the round's 8 disjoint rotations, results stored at the
 // positions of the next round.
-__device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, double* __restrict__ S, double* __restrict__ Q, int I,
+template <bool kHalf>
+__device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __restrict__ S, double* __restrict__ Q, int I,
                             int J, double tol, int lane) {
   for (int e = lane; e < 256; e += 32) {
     int a = e >> 4, b = e & 15;
     int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-    S[a * LDSS + b] = A[(size_t)r * ld + swz(r, c)];
+    S[a * LDSS + b] = A.get(r, c);
   }
   __syncwarp();
   const int j = lane & 7, k0 = lane >> 3;
@@ -208,15 +253,133 @@ __device__ __forceinline__ bool inner_solve(double* __restrict__ A, int ld, doub
     for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
       int a = e >> 4, b = e & 15;
       int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-      A[(size_t)r * ld + swz(r, c)] = a <= b ? S[a * LDSS + b] : S[b * LDSS + a];
+      A.put(r, c, a <= b ? S[a * LDSS + b] : S[b * LDSS + a]);
     }
   }
   return anyw;
 }
 
+// Variant of the pivot solve that keeps Q in registers (its columns travel between the lanes of a k0 group by
+// shuffle) and uses the slot's own 16x16 Q array as the scratch for S; Q overwrites it at the end.  Used where shared
+// memory has no room for separate pivot scratch (n = 105..200).
+template <bool kHalf>
+__device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* __restrict__ S, int I, int J, double tol,
+                                                 int lane) {
+  constexpr int LDSS = 16;  // S is the slot's 16 x LDQ array
+  for (int e = lane; e < 256; e += 32) {
+    int a = e >> 4, b = e & 15;
+    int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
+    S[a * LDSS + b] = A.get(r, c);
+  }
+  __syncwarp();
+  const int j = lane & 7, k0 = lane >> 3;
+  const double tol2 = tol * tol;
+  bool need = false;  // early exit: no pair of this pivot passes the rotation test (the usual case in the last sweeps)
+  for (int e = lane; e < 256; e += 32) {
+    const int a = e >> 4, b = e & 15;
+    const double x = S[a * LDSS + b];
+    need |= (a < b) && (x * x > tol2 * fabs(S[a * LDSS + a] * S[b * LDSS + b]));
+  }
+  need = __any_sync(0xffffffffu, need);
+  // static addresses: loads at (row pair, column pair), stores at the permuted positions
+  const double* ldA = S + (2 * k0) * LDSS + 2 * j;
+  const double* ldB = S + (2 * k0 + 8) * LDSS + 2 * j;
+  const int cp = kPi(2 * j), cq = kPi(2 * j + 1);
+  double* stA0 = S + kPi(2 * k0) * LDSS;
+  double* stA1 = S + kPi(2 * k0 + 1) * LDSS;
+  double* stB0 = S + kPi(2 * k0 + 8) * LDSS;
+  double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
+  const bool diagA = (k0 == j), diagB = (k0 + 4 == j);
+  // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
+  // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
+  // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
+  // right after this round's update, so that the next rotation (a long dependent chain) overlaps this round's stores.
+  //   j:      0      1      2..6            7
+  //   x, y:   0,3    1,5    2j-2, 2j+3      12,14
+  const int src_pp = j > 0 ? j - 1 : 0, src_qq = j < 7 ? j + 1 : 7;
+  const int own_src = (int)((0x170F061D140B0201ull >> (8 * j)) & 0xff);  // lanes 1,2,11,20,29,6,15,23
+  const int own_sel = lane == 2 ? 1 : ((lane == 6 || lane == 15) ? 2 : (lane == 23 ? 3 : 0));  // yA01,yA11,yB01,yB00
+  const int grp = lane & ~7;  // Q columns travel inside the 8 lanes of a k0 group
+  double qt[4], qb[4];        // Q[storage row k0 + 4u][position 2j], [position 2j + 1]; identity: logical row k sits in row qrow(k)
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    qt[u] = (qrow(2 * j) == k0 + 4 * u) ? 1.0 : 0.0;
+    qb[u] = (qrow(2 * j + 1) == k0 + 4 * u) ? 1.0 : 0.0;
+  }
+  double app = 1.0, aqq = 1.0, apq = 0.0, c, s, t;
+  if (need) {
+    const double2 d0 = *reinterpret_cast<const double2*>(S + (2 * j) * LDSS + 2 * j);
+    const double2 d1 = *reinterpret_cast<const double2*>(S + (2 * j + 1) * LDSS + 2 * j);
+    app = d0.x; apq = d0.y; aqq = d1.y;
+  }
+  bool doit = rotation(app, aqq, apq, tol2, c, s, t);
+  bool any = false;
+#pragma unroll 1
+  for (int r = 0; r < (need ? 15 : 0); ++r) {
+    const double2 a0 = *reinterpret_cast<const double2*>(ldA);
+    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDSS);
+    const double2 b0 = *reinterpret_cast<const double2*>(ldB);
+    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDSS);
+    __syncwarp();  // every lane has read its inputs before anybody stores
+    any |= doit;
+    const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
+    const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
+    const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
+    // block (k0, j)
+    double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
+    double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
+    double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
+    double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
+    if (diagA && doit) { ya00 = dtop; ya11 = dbot; ya01 = 0.0; ya10 = 0.0; }
+    // block (k0 + 4, j)
+    double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
+    double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
+    double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
+    double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
+    if (diagB && doit) { yb00 = dtop; yb11 = dbot; yb01 = 0.0; yb10 = 0.0; }
+    // next round's pivot by shuffle
+    const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
+    double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
+    double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
+    const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
+    if (j == 0) appn = dtop;
+    if (j == 7) aqqn = dtop;
+    // this round's stores, at the positions of the next round
+    stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
+    stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
+    // Q <- Q R, then the columns move: top_j <- top_{j-1} (top_1 <- bot_0, top_0 stays), bot_j <- bot_{j+1} (bot_7 <- top_7)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const double nt = c * qt[u] - s * qb[u], nb = s * qt[u] + c * qb[u];
+      const double mt = __shfl_sync(0xffffffffu, j == 0 ? nb : nt, grp | src_pp);
+      const double mb = __shfl_sync(0xffffffffu, nb, grp | src_qq);
+      qt[u] = j == 0 ? nt : mt;
+      qb[u] = j == 7 ? nt : mb;
+    }
+    app = appn; aqq = aqqn; apq = apqn;
+    doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
+    __syncwarp();
+  }
+  const bool anyw = __any_sync(0xffffffffu, any);
+  if (anyw) {
+    for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
+      int a = e >> 4, b = e & 15;
+      int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
+      A.put(r, c, a <= b ? S[a * LDSS + b] : S[b * LDSS + a]);
+    }
+  }
+  __syncwarp();
+  // Q over the scratch, in the layout of the DMMA B fragments: storage row sr, column c at c ^ ((sr & 3) << 2)
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+    *reinterpret_cast<double2*>(S + (k0 + 4 * u) * LDQ + ((2 * j) ^ (k0 << 2))) = make_double2(qt[u], qb[u]);
+  return anyw;
+}
+
 // ---------------------------------------------------------------------------------------------- apply
 // T = A[P1,P2] <- Q1^T T Q2 (P = rows/cols of the slot's one or two blocks), mirrored into A[P2,P1].
-__device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const double* __restrict__ Q1,
+template <bool kHalf>
+__device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* __restrict__ Q1,
                                            const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int n1 = J1 >= 0 ? 2 : 1, n2 = J2 >= 0 ? 2 : 1;
@@ -226,10 +389,7 @@ __device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const
   for (int ni = 0; ni < 2; ++ni)
 #pragma unroll
     for (int c = 0; c < 2; ++c)
-      if (ni < n1 && c < n2) {
-        int r = 8 * rb[ni] + g, col = 8 * cb[c] + 2 * t;
-        tf[ni][c] = *reinterpret_cast<const double2*>(A + (size_t)r * ld + swz(r, col));
-      }
+      if (ni < n1 && c < n2) tf[ni][c] = A.load_frag(rb[ni], cb[c], g, t);
   // step A: U^T = Q2^T T^T ;  ut[mi][ni] holds U[8ni+2t+{0,1}][8mi+g]
   double ut[2][2][2];
 #pragma unroll
@@ -276,12 +436,7 @@ __device__ __forceinline__ void apply_tile(double* __restrict__ A, int ld, const
   for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
     for (int nj = 0; nj < 2; ++nj)
-      if (mi < n1 && nj < n2) {
-        int r = 8 * rb[mi] + g, col = 8 * cb[nj] + 2 * t;
-        *reinterpret_cast<double2*>(A + (size_t)r * ld + swz(r, col)) = make_double2(out[mi][nj][0], out[mi][nj][1]);
-        A[(size_t)col * ld + swz(col, r)] = out[mi][nj][0];
-        A[(size_t)(col + 1) * ld + swz(col + 1, r)] = out[mi][nj][1];
-      }
+      if (mi < n1 && nj < n2) A.store_frag(rb[mi], cb[nj], g, t, out[mi][nj][0], out[mi][nj][1]);
 }
 
 // V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
@@ -331,7 +486,7 @@ struct JacobiParams {
   double* W;
   double* C;
   int* info;
-  double* gwork;   // per-CTA global workspace: [A np*ld][V np*ldv] (kGlobal) then [Q 2*nslots*16*LDQ] (q_global)
+  double* gwork;   // per-CTA global workspace: [A np*ld] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
   size_t gstride;  // doubles per CTA
   int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
   double tol;
@@ -341,16 +496,20 @@ constexpr int kVRowBlocksPerItem = 2;
 
 // One warp prepares slot sn of step tn: identity into its Q (buffer bn), and for a real pair the critical tile of the
 // running step t (buffer bc) followed by the pivot solve.
+template <int kMode>
 __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams& P, int tn, int sn, int bn, bool has_cur,
                                              int t, int bc, int parity, int lane, int widx) {
-  const int m = P.m, nb = P.nb, nslots = P.nslots, ld = P.ld;
+  constexpr bool kHalf = (kMode == 1);
+  const AView<kHalf> A{sm.A, P.ld, P.nb};
+  const int m = P.m, nb = P.nb, nslots = P.nslots;
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
-  for (int e = lane; e < 256; e += 32) {
-    const int sr = e >> 4, c = e & 15;
-    Qn[sr * LDQ + (c ^ ((sr & 3) << 2))] = (qrow(c) == sr) ? 1.0 : 0.0;
-  }
   int I, J;
   slot_blocks(m, nb, tn, sn, I, J);
+  if (kMode != 1 || J < 0)  // identity (the register variant of the pivot solve writes its own Q)
+    for (int e = lane; e < 256; e += 32) {
+      const int sr = e >> 4, c = e & 15;
+      Qn[sr * LDQ + (c ^ ((sr & 3) << 2))] = (qrow(c) == sr) ? 1.0 : 0.0;
+    }
   bool rotated = false;
   if (J >= 0) {
     if (has_cur) {
@@ -361,11 +520,12 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
         slot_blocks(m, nb, t, s1, I1, J1);
         slot_blocks(m, nb, t, s2, I2, J2);
         const double* Qc = sm.Q + (size_t)bc * nslots * kQSlot;
-        apply_tile(sm.A, ld, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
+        apply_tile(A, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
       }
     }
     __syncwarp();
-    rotated = inner_solve(sm.A, ld, sm.S + widx * 16 * LDSS, Qn, I, J, P.tol, lane);
+    if (kMode == 1) rotated = inner_solve_qreg(A, Qn, I, J, P.tol, lane);
+    else rotated = inner_solve(A, sm.S + widx * 16 * LDSS, Qn, I, J, P.tol, lane);
   }
   if (lane == 0) {
     sm.rot[bn * nslots + sn] = rotated ? 1 : 0;
@@ -373,8 +533,13 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   }
 }
 
-template <bool kGlobal, bool kQGlobal>
+// kMode 0: A (full), V, Q, pivot scratch in shared memory (n <= 104)
+//       1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
+//       2: A (full), V in the global workspace, Q and pivot scratch in shared memory
+//       3: as 2 with Q in the global workspace too (very large n)
+template <int kMode>
 __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
+  constexpr bool kHalf = (kMode == 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n = P.n, np = P.np, ld = P.ld, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
@@ -382,16 +547,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
   {
     double* d = reinterpret_cast<double*>(smem_raw);
     double* g = P.gwork + (size_t)blockIdx.x * P.gstride;
-    if (kGlobal) {
-      sm.A = g; g += (size_t)np * ld;
-      sm.V = g; g += (size_t)np * ldv;
-    } else {
+    if (kMode == 0) {
       sm.A = d; d += (size_t)np * ld;
       sm.V = d; d += (size_t)np * ldv;
+    } else if (kMode == 1) {
+      sm.A = d; d += (size_t)(nb * (nb + 1) / 2) * 64;
+      sm.V = g; g += (size_t)np * ldv;
+    } else {
+      sm.A = g; g += (size_t)np * ld;
+      sm.V = g; g += (size_t)np * ldv;
     }
-    if (kQGlobal) sm.Q = g;
+    if (kMode == 3) sm.Q = g;
     else { sm.Q = d; d += (size_t)2 * nslots * kQSlot; }
-    sm.S = d; d += (nslots < kPivotWarps ? nslots : kPivotWarps) * 16 * LDSS;
+    sm.S = d;
+    if (kMode != 1) d += (nslots < kPivotWarps ? nslots : kPivotWarps) * 16 * LDSS;
     sm.wsort = d; d += np;
     int* ip = reinterpret_cast<int*>(d);
     sm.rot = ip; ip += 2 * nslots;
@@ -401,6 +570,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
   // Pivot solves are latency bound and suffer when DMMAs of the update queue the same FP64 pipe: they run on the
   // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
   const int widx = ((warp & 3) < kPivotSmsp) ? (warp >> 2) * kPivotSmsp + (warp & 3) : -1;
+  const AView<kHalf> Av{sm.A, ld, nb};
   const int ntiles = nslots * (nslots - 1) / 2;
   const int nvgrp = (nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
   const int nitems = ntiles + nslots * nvgrp;
@@ -411,14 +581,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
     for (int e = tid; e < np * np; e += kThreads) {
       int r = e / np, c = e - r * np;
       double a = (r < n && c < n) ? H[(size_t)r * n + c] : 0.0;
-      sm.A[(size_t)r * ld + swz(r, c)] = a;
+      Av.put(r, c, a);
       sm.V[(size_t)r * ldv + c] = (r == c) ? 1.0 : 0.0;
     }
     if (tid < 4) sm.ctr[tid] = 0;
     __syncthreads();
     // prologue: pivots of (sweep 0, step 0) into Q buffer 0
     if (widx >= 0)
-      for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot(sm, P, 0, sn, 0, false, 0, 0, 0, lane, widx);
+      for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot<kMode>(sm, P, 0, sn, 0, false, 0, 0, 0, lane, widx);
     __syncthreads();
     int sweeps = 0, buf = 0, gstep = 0;
     bool converged = false;
@@ -439,7 +609,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
 #endif
         // pivots of the next step (critical tile first), overlapped with the rest of this step's updates
         if (do_next && widx >= 0)
-          for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot(sm, P, tn, sn, buf ^ 1, true, step, buf, parn, lane, widx);
+          for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot<kMode>(sm, P, tn, sn, buf ^ 1, true, step, buf, parn, lane, widx);
 #ifdef WPCD_PROFILE
         if (blockIdx.x == 0 && tid == 32) WPCD_PROF_ADD(1, clock64() - tk0);
         long long tk1 = clock64();
@@ -462,7 +632,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
             slot_blocks(m, nb, step, s1, I1, J1);
             slot_blocks(m, nb, step, s2, I2, J2);
             if (I1 < 0 || I2 < 0) continue;
-            apply_tile(sm.A, ld, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
+            apply_tile(Av, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
           } else {
             const int v = it - ntiles;
             const int s = v / nvgrp, grp = v - s * nvgrp;
@@ -489,7 +659,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
     }
     // eigenvalues = diagonal; rank sort ascending (ties by index); gather columns
     __syncthreads();
-    for (int k = tid; k < n; k += kThreads) sm.wsort[k] = sm.A[(size_t)k * ld + swz(k, k)];
+    for (int k = tid; k < n; k += kThreads) sm.wsort[k] = Av.get(k, k);
     __syncthreads();
     for (int k = tid; k < n; k += kThreads) {
       double wk = sm.wsort[k];
@@ -515,10 +685,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
 
 struct Geometry {
   int nb, np, ld, ldv, m, nslots;
-  size_t smem_fixed, smem_q, smem_mat;  // bytes
-  bool mat_global, q_global;
+  int mode;        // k_jacobi<mode>
   size_t gstride;  // doubles of global workspace per CTA
-  size_t smem;     // dynamic shared memory of the launch
+  size_t smem;     // dynamic shared memory of the launch (bytes)
 };
 
 Geometry geometry(const WpcdHandle* h, int n) {
@@ -532,30 +701,40 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
   const int nS = g.nslots < kPivotWarps ? g.nslots : kPivotWarps;
-  g.smem_fixed = (size_t)nS * 16 * LDSS * 8 + (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
-  g.smem_q = (size_t)2 * g.nslots * kQSlot * 8;
-  g.smem_mat = ((size_t)g.np * g.ld + (size_t)g.np * g.ldv) * 8;
+  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
+  const size_t scratch = (size_t)nS * 16 * LDSS * 8;
+  const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
+  const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
-  g.mat_global = g.smem_fixed + g.smem_q + g.smem_mat > cap;
-  g.q_global = g.mat_global && (g.smem_fixed + g.smem_q > cap);
-  g.gstride = (g.mat_global ? g.smem_mat / 8 : 0) + (g.q_global ? g.smem_q / 8 : 0);
-  g.smem = g.smem_fixed + (g.q_global ? 0 : g.smem_q) + (g.mat_global ? 0 : g.smem_mat);
+  if (misc + scratch + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + scratch + q + a_full + v; g.gstride = 0; }
+  else if (misc + q + a_half <= cap) { g.mode = 1; g.smem = misc + q + a_half; g.gstride = v / 8; }
+  else if (misc + scratch + q <= cap) { g.mode = 2; g.smem = misc + scratch + q; g.gstride = (a_full + v) / 8; }
+  else { g.mode = 3; g.smem = misc + scratch; g.gstride = (a_full + v + q) / 8; }
   return g;
 }
 
-// CTAs of the global-workspace path: two per SM while all their workspaces together stay well inside the 126 MB L2
-// (and two CTAs' shared memory fits one SM).
+// CTAs of the workspace paths: two per SM only while two CTAs' shared memory fits one SM and all workspaces together
+// stay well inside L2 (measured: a 100 MB working set already spills to HBM -- the 126 MB L2 is split over two dies);
+// otherwise one per SM.
 int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
-  const bool two = ((size_t)2 * h->num_sms * g.gstride * 8 <= ((size_t)80 << 20)) && (2 * (g.smem + 1024) <= (size_t)h->max_smem_optin);
+  const bool two = ((size_t)2 * h->num_sms * g.gstride * 8 <= ((size_t)48 << 20)) && (2 * (g.smem + 1024) <= (size_t)h->max_smem_optin);
   const int grid = (two ? 2 : 1) * h->num_sms;
   return batch < grid ? batch : grid;
+}
+
+template <int kMode>
+int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cudaStream_t st) {
+  int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<kMode>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "jacobi attr");
+  if (rc) return rc;
+  k_jacobi<kMode><<<grid, kThreads, smem, st>>>(P);
+  return WPCD_OK;
 }
 
 }  // namespace
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
   Geometry g = geometry(h, n);
-  if (!g.mat_global) return 0;
+  if (g.mode == 0) return 0;
   return (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
 
@@ -568,24 +747,16 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
+  const int grid = g.mode == 0 ? batch : global_grid(h, g, batch);
+  if (g.mode != 0 && work_bytes < (size_t)grid * g.gstride * 8) return WPCD_EWORK;
   int rc;
-  if (!g.mat_global) {
-    rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
-    if (rc) return rc;
-    k_jacobi<false, false><<<batch, kThreads, g.smem, st>>>(P);
-  } else {
-    const int grid = global_grid(h, g, batch);
-    if (work_bytes < (size_t)grid * g.gstride * 8) return WPCD_EWORK;
-    if (g.q_global) {
-      rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
-      if (rc) return rc;
-      k_jacobi<true, true><<<grid, kThreads, g.smem, st>>>(P);
-    } else {
-      rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem), "jacobi attr");
-      if (rc) return rc;
-      k_jacobi<true, false><<<grid, kThreads, g.smem, st>>>(P);
-    }
+  switch (g.mode) {
+    case 0: rc = launch_mode<0>(h, P, grid, g.smem, st); break;
+    case 1: rc = launch_mode<1>(h, P, grid, g.smem, st); break;
+    case 2: rc = launch_mode<2>(h, P, grid, g.smem, st); break;
+    default: rc = launch_mode<3>(h, P, grid, g.smem, st); break;
   }
+  if (rc) return rc;
   return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch");
 }
 
