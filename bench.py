@@ -24,6 +24,9 @@ sys.path.insert(0, ROOT)
 from paper_2106_00454_b200 import inputs as inp  # noqa: E402
 
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+# DRAM traffic of one Jacobi launch at the bench workload (4096 matrices) from the committed ncu --set full capture
+# (profiles/r1_jacobi_ncu.md), keyed by n; algorithmic minimum = read H + write C + W = 16 n^2 + 8 n bytes per matrix.
+NCU_DRAM_BYTES = {100: 0.617683e9, 200: 3.687615e9}
 METRIC = "channel-solves/s (fp64 H diag + on-shell T at all E)"
 CHANNELS = [(0, 0), (1, 1)]   # single 1S0 (n=N) and coupled 3S1-3D1 (n=2N)
 
@@ -103,7 +106,7 @@ def run_reference(args):
     if rank != 0:
         return
     cores = os.cpu_count() or 1
-    n_each = max(cores, 8)
+    n_each = 16 * max(cores, 8)
     for _ in range(args.warmup):
         oracle_sample(args.N, args.nE, max(cores // 4, 1), cores)
     t0 = time.perf_counter()
@@ -215,7 +218,7 @@ def run_ours(args):
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
-            n_each = max(cores, 8)
+            n_each = 64 * max(cores, 8)          # about 10-20 s of CPU work on the box's cores
             k, dt = oracle_sample(N, nE, n_each, cores)
             cpu = {"value": k / dt, "unit": "channel-solves/s", "cores": cores, "kind": "oracle",
                    "sample": f"{n_each} samples x (1S0 + 3S1-3D1) of the same workload, one solve per thread, {dt:.1f} s"}
@@ -229,7 +232,8 @@ def run_ours(args):
                         "d2h_bytes_per_step": pipe.d2h_bytes(), "ms_per_step": ms_e2e / args.steps},
                 "gpu_launches": pipe.launches_per_step * args.steps,
                 "roofline": {"bound": "alu", "kernel": f"k_jacobi ({dom}, n={n})", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
-                             "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
+                             "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(n),
+                             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_jacobi_ncu.md",
                              "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DMMA microbenchmark measured 37.1)",
                              "flops_model": "6 n^3 x rotating sweeps x batch (SURVEY 8(d))"},
                 "stages_ms": stage_ms, "jacobi": jac, "cpu_baseline": cpu}
