@@ -488,11 +488,51 @@ struct JacobiParams {
   int* info;
   double* gwork;   // per-CTA global workspace: [A np*ld] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
   size_t gstride;  // doubles per CTA
+  const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
   int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
   double tol;
 };
 
 constexpr int kVRowBlocksPerItem = 2;
+
+// Schedule tables (one copy per launch, read through the L1): the tournament needs integer divisions that would
+// otherwise be redone for every work item.
+//   slot[t][s]  = I | J << 16                 blocks of slot s at step t (0xFFFF = none)
+//   feed[t][s]  = s1 | s2 << 16               slots (s1 < s2) of the PREVIOUS step whose tile feeds the pivot of slot s
+//   tile[t][k]  = s1 | s2 << 12 | crit << 24  k-th tile of step t (s1 < s2); crit: it feeds a pivot of the next step
+__global__ void k_schedule(int m, int nb, int* __restrict__ tab) {
+  const int nslots = m / 2, ntiles = nslots * (nslots - 1) / 2, t = blockIdx.x;
+  const int tp = (t + m - 2) % (m - 1), tn = (t + 1) % (m - 1);
+  int* slot = tab + t * nslots;
+  int* feed = tab + (m - 1) * nslots + t * nslots;
+  int* tile = tab + 2 * (m - 1) * nslots + t * ntiles;
+  for (int s = threadIdx.x; s < nslots; s += blockDim.x) {
+    int I, J;
+    slot_blocks(m, nb, t, s, I, J);
+    slot[s] = (I & 0xFFFF) | ((J & 0xFFFF) << 16);
+    int f = 0;
+    if (J >= 0) {
+      int s1 = rr_slot_of(m, tp, I), s2 = rr_slot_of(m, tp, J);
+      if (s1 > s2) { int x = s1; s1 = s2; s2 = x; }
+      f = s1 | (s2 << 16);
+    }
+    feed[s] = f;
+  }
+  for (int k = threadIdx.x; k < ntiles; k += blockDim.x) {
+    int s1 = 0, rem = k;  // unrank (s1 < s2)
+    while (rem >= nslots - 1 - s1) { rem -= nslots - 1 - s1; ++s1; }
+    const int s2 = s1 + 1 + rem;
+    const int crit = critical_slot(m, nb, t, tn, s1, s2) >= 0 ? 1 : 0;
+    tile[k] = s1 | (s2 << 12) | (crit << 24);
+  }
+}
+
+__device__ __forceinline__ void decode_slot(int x, int& I, int& J) {
+  I = x & 0xFFFF; J = (x >> 16) & 0xFFFF;
+  if (I == 0xFFFF) I = -1;
+  if (J == 0xFFFF) J = -1;
+}
+
 
 // One warp prepares slot sn of step tn: identity into its Q (buffer bn), and for a real pair the critical tile of the
 // running step t (buffer bc) followed by the pivot solve.
@@ -501,10 +541,10 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
                                              int t, int bc, int parity, int lane, int widx) {
   constexpr bool kHalf = (kMode == 1);
   const AView<kHalf> A{sm.A, P.ld, P.nb};
-  const int m = P.m, nb = P.nb, nslots = P.nslots;
+  const int m = P.m, nslots = P.nslots;
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
   int I, J;
-  slot_blocks(m, nb, tn, sn, I, J);
+  decode_slot(__ldg(P.tab + tn * nslots + sn), I, J);
   if (kMode != 1 || J < 0)  // identity (the register variant of the pivot solve writes its own Q)
     for (int e = lane; e < 256; e += 32) {
       const int sr = e >> 4, c = e & 15;
@@ -513,12 +553,12 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   bool rotated = false;
   if (J >= 0) {
     if (has_cur) {
-      int s1 = rr_slot_of(m, t, I), s2 = rr_slot_of(m, t, J);
-      if (s1 > s2) { int x = s1; s1 = s2; s2 = x; }
+      const int f = __ldg(P.tab + (m - 1) * nslots + tn * nslots + sn);
+      const int s1 = f & 0xFFFF, s2 = f >> 16;
       if (sm.rot[bc * nslots + s1] | sm.rot[bc * nslots + s2]) {
         int I1, J1, I2, J2;
-        slot_blocks(m, nb, t, s1, I1, J1);
-        slot_blocks(m, nb, t, s2, I2, J2);
+        decode_slot(__ldg(P.tab + t * nslots + s1), I1, J1);
+        decode_slot(__ldg(P.tab + t * nslots + s2), I2, J2);
         const double* Qc = sm.Q + (size_t)bc * nslots * kQSlot;
         apply_tile(A, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
       }
@@ -617,20 +657,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
         const int* rot = sm.rot + buf * nslots;
         const double* Qc = sm.Q + (size_t)buf * nslots * kQSlot;
         int* queue = sm.ctr + (gstep & 1);
+        const int* tab_slot = P.tab + step * nslots;
+        const int* tab_tile = P.tab + 2 * (m - 1) * nslots + step * ntiles;
         for (;;) {
           int it = 0;
           if (lane == 0) it = atomicAdd(queue, 1);
           it = __shfl_sync(0xffffffffu, it, 0);
           if (it >= nitems) break;
           if (it < ntiles) {
-            int s1 = 0, rem = it;  // unrank (s1 < s2)
-            while (rem >= nslots - 1 - s1) { rem -= nslots - 1 - s1; ++s1; }
-            const int s2 = s1 + 1 + rem;
+            const int e = __ldg(tab_tile + it);
+            const int s1 = e & 0xFFF, s2 = (e >> 12) & 0xFFF;
             if (!(rot[s1] | rot[s2])) continue;
-            if (do_next && critical_slot(m, nb, step, tn, s1, s2) >= 0) continue;  // done by the pivot warp
+            if (do_next && (e >> 24)) continue;  // feeds a pivot of the next step: done by that pivot's warp
             int I1, J1, I2, J2;
-            slot_blocks(m, nb, step, s1, I1, J1);
-            slot_blocks(m, nb, step, s2, I2, J2);
+            decode_slot(__ldg(tab_slot + s1), I1, J1);
+            decode_slot(__ldg(tab_slot + s2), I2, J2);
             if (I1 < 0 || I2 < 0) continue;
             apply_tile(Av, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
           } else {
@@ -638,7 +679,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
             const int s = v / nvgrp, grp = v - s * nvgrp;
             if (!rot[s]) continue;
             int I, J;
-            slot_blocks(m, nb, step, s, I, J);
+            decode_slot(__ldg(tab_slot + s), I, J);
             int rb0 = grp * kVRowBlocksPerItem, rb1 = rb0 + kVRowBlocksPerItem;
             if (rb1 > nb) rb1 = nb;
             apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rb0, rb1, lane);
@@ -684,6 +725,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
 }
 
 struct Geometry {
+  size_t tab_bytes;  // schedule tables at the head of the workspace
   int nb, np, ld, ldv, m, nslots;
   int mode;        // k_jacobi<mode>
   size_t gstride;  // doubles of global workspace per CTA
@@ -700,6 +742,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
+  g.tab_bytes = (((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255;
   const int nS = g.nslots < kPivotWarps ? g.nslots : kPivotWarps;
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
   const size_t scratch = (size_t)nS * 16 * LDSS * 8;
@@ -734,8 +777,8 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
   Geometry g = geometry(h, n);
-  if (g.mode == 0) return 0;
-  return (size_t)global_grid(h, g, batch) * g.gstride * 8;
+  if (g.mode == 0) return g.tab_bytes;
+  return g.tab_bytes + (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
 
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
@@ -743,12 +786,15 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   Geometry g = geometry(h, n);
   if (g.smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   JacobiParams P;
-  P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gwork = static_cast<double*>(d_work); P.gstride = g.gstride;
+  P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gstride = g.gstride;
+  P.tab = static_cast<const int*>(d_work);
+  P.gwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + g.tab_bytes);
   P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   const int grid = g.mode == 0 ? batch : global_grid(h, g, batch);
-  if (g.mode != 0 && work_bytes < (size_t)grid * g.gstride * 8) return WPCD_EWORK;
+  if (work_bytes < g.tab_bytes + (g.mode != 0 ? (size_t)grid * g.gstride * 8 : 0)) return WPCD_EWORK;
+  k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work));
   int rc;
   switch (g.mode) {
     case 0: rc = launch_mode<0>(h, P, grid, g.smem, st); break;

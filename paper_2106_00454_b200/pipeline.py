@@ -61,8 +61,8 @@ class Pipeline:
 
     @property
     def launches_per_step(self):
-        # k_grid, k_basis, k_combine per kind; k_jacobi, k_bins, k_onshell, k_phase per kind
-        return 2 + len(self.kind) * 5
+        # k_grid, k_basis, k_combine per kind; k_schedule, k_jacobi, k_bins, k_onshell, k_phase per kind
+        return 2 + len(self.kind) * 6
 
     def solve_device(self, events=None):
         """One pass of the whole hot path with inputs resident in HBM.  events: optional dict name -> (start, end)
