@@ -378,11 +378,10 @@ __device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* 
 
 // ---------------------------------------------------------------------------------------------- apply
 // T = A[P1,P2] <- Q1^T T Q2 (P = rows/cols of the slot's one or two blocks), mirrored into A[P2,P1].
-template <bool kHalf>
-__device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* __restrict__ Q1,
-                                           const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
+template <bool kHalf, int n1, int n2>
+__device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double* __restrict__ Q1,
+                                             const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
   const int g = lane >> 2, t = lane & 3;
-  const int n1 = J1 >= 0 ? 2 : 1, n2 = J2 >= 0 ? 2 : 1;
   const int rb[2] = {I1, J1}, cb[2] = {I2, J2};
   double2 tf[2][2];
 #pragma unroll
@@ -437,6 +436,16 @@ __device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* 
 #pragma unroll
     for (int nj = 0; nj < 2; ++nj)
       if (mi < n1 && nj < n2) A.store_frag(rb[mi], cb[nj], g, t, out[mi][nj][0], out[mi][nj][1]);
+}
+
+// the usual case (two full slots) gets code without predication
+template <bool kHalf>
+__device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* __restrict__ Q1,
+                                           const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
+  if (J1 >= 0 && J2 >= 0) apply_tile_n<kHalf, 2, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else if (J1 >= 0) apply_tile_n<kHalf, 2, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else if (J2 >= 0) apply_tile_n<kHalf, 1, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else apply_tile_n<kHalf, 1, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
 }
 
 // V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
@@ -614,6 +623,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
   const int ntiles = nslots * (nslots - 1) / 2;
   const int nvgrp = (nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
   const int nitems = ntiles + nslots * nvgrp;
+  const float rnvgrp = 1.0f / (float)nvgrp;
 
   for (int mat = blockIdx.x; mat < P.batch; mat += gridDim.x) {
     const double* H = P.H + (size_t)mat * n * n;
@@ -676,7 +686,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
             apply_tile(Av, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
           } else {
             const int v = it - ntiles;
-            const int s = v / nvgrp, grp = v - s * nvgrp;
+            const int s = (int)(((float)v + 0.5f) * rnvgrp), grp = v - s * nvgrp;
             if (!rot[s]) continue;
             int I, J;
             decode_slot(__ldg(tab_slot + s), I, J);
