@@ -449,10 +449,10 @@ __device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* 
 }
 
 // V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
-__device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                        int rb0, int rb1, int lane) {
+template <int nbk>
+__device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
+                                          int rb0, int rb1, int lane) {
   const int g = lane >> 2, t = lane & 3;
-  const int nbk = J >= 0 ? 2 : 1;
   const int cb[2] = {I, J};
   double bq[2][2][2];
 #pragma unroll
@@ -487,6 +487,12 @@ __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const do
         *reinterpret_cast<double2*>(V + (size_t)row * ld + col) = make_double2(out[ni][0], out[ni][1]);
       }
   }
+}
+
+__device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
+                                        int rb0, int rb1, int lane) {
+  if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rb0, rb1, lane);
+  else apply_V_n<1>(V, ld, Q, I, J, rb0, rb1, lane);
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
