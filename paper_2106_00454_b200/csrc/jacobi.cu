@@ -185,7 +185,6 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
   double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
   double* stQp = Q + k0 * LDQ + (cp ^ qx);
   double* stQq = Q + k0 * LDQ + (cq ^ qx);
-  const bool diagA = (k0 == j), diagB = (k0 + 4 == j);
   // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
   // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
   // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
@@ -222,13 +221,11 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
     double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
     double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
     double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
-    if (diagA && doit) { ya00 = dtop; ya11 = dbot; ya01 = 0.0; ya10 = 0.0; }
     // block (k0 + 4, j)
     double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
     double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
     double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
     double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
-    if (diagB && doit) { yb00 = dtop; yb11 = dbot; yb01 = 0.0; yb10 = 0.0; }
     // next round's pivot by shuffle
     const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
     double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
@@ -289,7 +286,6 @@ __device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* 
   double* stA1 = S + kPi(2 * k0 + 1) * LDSS;
   double* stB0 = S + kPi(2 * k0 + 8) * LDSS;
   double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
-  const bool diagA = (k0 == j), diagB = (k0 + 4 == j);
   // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
   // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
   // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
@@ -330,13 +326,11 @@ __device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* 
     double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
     double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
     double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
-    if (diagA && doit) { ya00 = dtop; ya11 = dbot; ya01 = 0.0; ya10 = 0.0; }
     // block (k0 + 4, j)
     double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
     double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
     double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
     double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
-    if (diagB && doit) { yb00 = dtop; yb11 = dbot; yb01 = 0.0; yb10 = 0.0; }
     // next round's pivot by shuffle
     const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
     double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
