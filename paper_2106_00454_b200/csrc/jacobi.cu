@@ -36,8 +36,8 @@ __device__ long long wpcd_prof[8];
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
 constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), columns XOR-swizzled by the storage row
-constexpr int LDSS = 18;  // row stride of the warp-private 16x16 pivot block (even: 16-byte aligned row pairs)
 constexpr int kQSlot = 16 * LDQ;
+constexpr int kFullEvery = 4;  // a full 16x16 pivot sweep every 4th step of the block tournament, cross-only sweeps between
 constexpr int kPivotSmsp = 4;                          // SM sub-partitions reserved for the pivot solves
 constexpr int kPivotWarps = kWarps / 4 * kPivotSmsp;   // warps that solve pivots
 
@@ -103,7 +103,6 @@ struct Smem {
   double* A;     // [np][ld] swizzled, full symmetric (shared or global)
   double* V;     // [np][ldv] plain (shared or global)
   double* Q;     // [2][nslots][16][LDQ] (shared or global), double buffered over the steps
-  double* S;     // [min(nslots,kWarps)][16][LDSS]
   double* wsort; // [np]
   int* rot;      // [2][nslots] slot rotated something
   int* src;      // [np]
@@ -147,208 +146,116 @@ __device__ __forceinline__ bool rotation(double app, double aqq, double apq, dou
   return doit;
 }
 
-// One warp: load S = A[IJ,IJ], run one full sweep (15 rounds of 8 simultaneous rotations), write S back, leave the
-// accumulated 16x16 rotation product in Q (identity on entry; rows are storage rows).  Returns (warp-uniform)
-// whether anything was rotated.  Lane (k0 = lane>>3, j = lane&7) owns the 2x2 blocks
-// (row pair k0, column pair j) and (row pair k0+4, column pair j) of S and rows k0, k0+4, k0+8, k0+12 of Q; one
-// round = S <- R^T S R, Q <- Q R with R the product of the round's 8 disjoint rotations, results stored at the
-// positions of the next round.
-template <bool kHalf>
-__device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __restrict__ S, double* __restrict__ Q, int I,
-                            int J, double tol, int lane) {
-  for (int e = lane; e < 256; e += 32) {
-    int a = e >> 4, b = e & 15;
-    int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-    S[a * LDSS + b] = A.get(r, c);
-  }
-  __syncwarp();
-  const int j = lane & 7, k0 = lane >> 3;
-  const double tol2 = tol * tol;
-  {  // early exit: no pair of this pivot passes the rotation test (the usual case in the last sweeps)
-    bool need = false;
-    for (int e = lane; e < 256; e += 32) {
-      const int a = e >> 4, b = e & 15;
-      const double x = S[a * LDSS + b];
-      need |= (a < b) && (x * x > tol2 * fabs(S[a * LDSS + a] * S[b * LDSS + b]));
-    }
-    if (!__any_sync(0xffffffffu, need)) return false;
-  }
-  // static addresses: loads at (row pair, column pair), stores at the permuted positions
-  const double* ldA = S + (2 * k0) * LDSS + 2 * j;
-  const double* ldB = S + (2 * k0 + 8) * LDSS + 2 * j;
-  const int qx = k0 << 2;  // Q column swizzle of this lane's storage rows: (k0 + 4u) & 3 == k0
-  const double* ldQ = Q + k0 * LDQ + ((2 * j) ^ qx);
-  const int cp = kPi(2 * j), cq = kPi(2 * j + 1);
-  double* stA0 = S + kPi(2 * k0) * LDSS;
-  double* stA1 = S + kPi(2 * k0 + 1) * LDSS;
-  double* stB0 = S + kPi(2 * k0 + 8) * LDSS;
-  double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
-  double* stQp = Q + k0 * LDQ + (cp ^ qx);
-  double* stQq = Q + k0 * LDQ + (cq ^ qx);
-  // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
-  // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
-  // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
-  // right after this round's update, so that the next rotation (a long dependent chain) overlaps this round's stores.
-  //   j:      0      1      2..6            7
-  //   x, y:   0,3    1,5    2j-2, 2j+3      12,14
-  const int src_pp = j > 0 ? j - 1 : 0, src_qq = j < 7 ? j + 1 : 7;
-  const int own_src = (int)((0x170F061D140B0201ull >> (8 * j)) & 0xff);  // lanes 1,2,11,20,29,6,15,23
-  const int own_sel = lane == 2 ? 1 : ((lane == 6 || lane == 15) ? 2 : (lane == 23 ? 3 : 0));  // yA01,yA11,yB01,yB00
-  double app, aqq, apq, c, s, t;
-  {
-    const double2 d0 = *reinterpret_cast<const double2*>(S + (2 * j) * LDSS + 2 * j);
-    const double2 d1 = *reinterpret_cast<const double2*>(S + (2 * j + 1) * LDSS + 2 * j);
-    app = d0.x; apq = d0.y; aqq = d1.y;
-  }
-  bool doit = rotation(app, aqq, apq, tol2, c, s, t);
-  bool any = false;
-#pragma unroll 1
-  for (int r = 0; r < 15; ++r) {
-    const double2 a0 = *reinterpret_cast<const double2*>(ldA);
-    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDSS);
-    const double2 b0 = *reinterpret_cast<const double2*>(ldB);
-    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDSS);
-    double2 qv[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) qv[u] = *reinterpret_cast<const double2*>(ldQ + 4 * u * LDQ);
-    __syncwarp();  // every lane has read its inputs before anybody stores
-    any |= doit;
-    const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
-    const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
-    const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
-    // block (k0, j)
-    double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
-    double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
-    double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
-    double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
-    // block (k0 + 4, j)
-    double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
-    double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
-    double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
-    double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
-    // next round's pivot by shuffle
-    const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
-    double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
-    double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
-    const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
-    if (j == 0) appn = dtop;
-    if (j == 7) aqqn = dtop;
-    // this round's stores, at the positions of the next round
-    stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
-    stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      stQp[4 * u * LDQ] = c * qv[u].x - s * qv[u].y;
-      stQq[4 * u * LDQ] = s * qv[u].x + c * qv[u].y;
-    }
-    app = appn; aqq = aqqn; apq = apqn;
-    doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
-    __syncwarp();
-  }
-  const bool anyw = __any_sync(0xffffffffu, any);
-  if (anyw) {
-    for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
-      int a = e >> 4, b = e & 15;
-      int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-      A.put(r, c, a <= b ? S[a * LDSS + b] : S[b * LDSS + a]);
-    }
-  }
-  return anyw;
-}
+// Cross-only tournament: the even positions (block I) stay, the odd ones (block J) move on by one pair, so that 8
+// rounds meet the 64 pairs (i in I, j in J) exactly once and everything is back where it started.
+__device__ __forceinline__ int kPiCross(int x) { return (x & 1) ? (((x >> 1) + 1) & 7) * 2 + 1 : x; }
 
-// Variant of the pivot solve that keeps Q in registers (its columns travel between the lanes of a k0 group by
-// shuffle) and uses the slot's own 16x16 Q array as the scratch for S; Q overwrites it at the end.  Used where shared
-// memory has no room for separate pivot scratch (n = 105..200).
+// Pivot solve.  One warp: load S = A[IJ,IJ] into the scratch (position 2i = i-th index of block I, 2i+1 = i-th of J),
+// run one sweep -- full: 15 rounds of 8 simultaneous rotations over all 120 pairs (Brent-Luk); cross: 8 rounds over
+// the 64 pairs between the two blocks -- write S back, and write the accumulated 16x16 rotation product over the
+// scratch (which is the slot's Q array) in the layout of the DMMA B fragments.  Returns (warp-uniform) whether
+// anything was rotated.  Lane (k0 = lane>>3, j = lane&7) owns the 2x2 blocks (row pair k0, column pair j) and (row
+// pair k0+4, column pair j) of S, which go through shared memory every round (static addresses: the data moves to the
+// next round's positions, not the pairing), and storage rows k0, k0+4, k0+8, k0+12 of Q at column pair j, which stay
+// in registers (the columns travel between the lanes of a k0 group by shuffle).  One round = S <- R^T S R, Q <- Q R
+// with R the product of the round's 8 disjoint rotations.  The next round's pivots (a_pp, a_qq, a_pq) are fetched by
+// shuffle right after the update, so that the next rotation (a long dependent chain) overlaps this round's stores.
 template <bool kHalf>
-__device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* __restrict__ S, int I, int J, double tol,
-                                                 int lane) {
-  constexpr int LDSS = 16;  // S is the slot's 16 x LDQ array
-  for (int e = lane; e < 256; e += 32) {
-    int a = e >> 4, b = e & 15;
-    int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-    S[a * LDSS + b] = A.get(r, c);
-  }
-  __syncwarp();
-  const int j = lane & 7, k0 = lane >> 3;
-  const double tol2 = tol * tol;
-  bool need = false;  // early exit: no pair of this pivot passes the rotation test (the usual case in the last sweeps)
+__device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __restrict__ S, int I, int J, double tol,
+                                            bool full, int lane) {
+  constexpr int LDS_ = 16;  // S is the slot's 16 x LDQ array: a row = all 32 banks
   for (int e = lane; e < 256; e += 32) {
     const int a = e >> 4, b = e & 15;
-    const double x = S[a * LDSS + b];
-    need |= (a < b) && (x * x > tol2 * fabs(S[a * LDSS + a] * S[b * LDSS + b]));
+    const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c = 8 * ((b & 1) ? J : I) + (b >> 1);
+    S[a * LDS_ + b] = A.get(r, c);
+  }
+  __syncwarp();
+  const int j = lane & 7, k0 = lane >> 3;
+  const double tol2 = tol * tol;
+  bool need = false;  // early exit: no pair of this sweep passes the rotation test (the usual case in the last sweeps)
+  for (int e = lane; e < 256; e += 32) {
+    const int a = e >> 4, b = e & 15;
+    const double x = S[a * LDS_ + b];
+    need |= (a < b) && (full || ((a ^ b) & 1)) && (x * x > tol2 * fabs(S[a * LDS_ + a] * S[b * LDS_ + b]));
   }
   need = __any_sync(0xffffffffu, need);
   // static addresses: loads at (row pair, column pair), stores at the permuted positions
-  const double* ldA = S + (2 * k0) * LDSS + 2 * j;
-  const double* ldB = S + (2 * k0 + 8) * LDSS + 2 * j;
-  const int cp = kPi(2 * j), cq = kPi(2 * j + 1);
-  double* stA0 = S + kPi(2 * k0) * LDSS;
-  double* stA1 = S + kPi(2 * k0 + 1) * LDSS;
-  double* stB0 = S + kPi(2 * k0 + 8) * LDSS;
-  double* stB1 = S + kPi(2 * k0 + 9) * LDSS;
-  // Look-ahead: the pivot (a_pp, a_qq, a_pq) of pair j in the NEXT round sits, before the move, at rows/columns
-  // x = kPi^-1(2j), y = kPi^-1(2j+1): the two diagonal entries come from the rotations of pairs x/2 and y/2, the
-  // off-diagonal entry from one entry of the block (x/2, y/2), owned by lane own_src.  They are fetched by shuffle
-  // right after this round's update, so that the next rotation (a long dependent chain) overlaps this round's stores.
+  const double* ldA = S + (2 * k0) * LDS_ + 2 * j;
+  const double* ldB = S + (2 * k0 + 8) * LDS_ + 2 * j;
+  const int cp = full ? kPi(2 * j) : kPiCross(2 * j), cq = full ? kPi(2 * j + 1) : kPiCross(2 * j + 1);
+  double* stA0 = S + (full ? kPi(2 * k0) : kPiCross(2 * k0)) * LDS_;
+  double* stA1 = S + (full ? kPi(2 * k0 + 1) : kPiCross(2 * k0 + 1)) * LDS_;
+  double* stB0 = S + (full ? kPi(2 * k0 + 8) : kPiCross(2 * k0 + 8)) * LDS_;
+  double* stB1 = S + (full ? kPi(2 * k0 + 9) : kPiCross(2 * k0 + 9)) * LDS_;
+  // Look-ahead sources.  Full tournament: the next pivot of pair j sits, before the move, at rows/columns
   //   j:      0      1      2..6            7
   //   x, y:   0,3    1,5    2j-2, 2j+3      12,14
-  const int src_pp = j > 0 ? j - 1 : 0, src_qq = j < 7 ? j + 1 : 7;
-  const int own_src = (int)((0x170F061D140B0201ull >> (8 * j)) & 0xff);  // lanes 1,2,11,20,29,6,15,23
-  const int own_sel = lane == 2 ? 1 : ((lane == 6 || lane == 15) ? 2 : (lane == 23 ? 3 : 0));  // yA01,yA11,yB01,yB00
-  const int grp = lane & ~7;  // Q columns travel inside the 8 lanes of a k0 group
-  double qt[4], qb[4];        // Q[storage row k0 + 4u][position 2j], [position 2j + 1]; identity: logical row k sits in row qrow(k)
+  // (diagonal entries from the rotations of pairs x/2, y/2; off-diagonal entry owned by lanes 1,2,11,20,29,6,15,23).
+  // Cross tournament: x = 2j (own pair), y = 2((j-1)&7)+1: entry (0,1) of block (row pair j, column pair j-1).
+  const int grp = lane & ~7;
+  const int src_pp = full ? (j > 0 ? j - 1 : 0) : j;
+  const int src_qq = full ? (j < 7 ? j + 1 : 7) : ((j + 7) & 7);
+  const bool fix0 = full && j == 0, fix7 = full && j == 7;
+  const int own_src = full ? (int)((0x170F061D140B0201ull >> (8 * j)) & 0xff) : 8 * (j & 3) + ((j + 7) & 7);
+  int own_sel;  // which of its entries a lane supplies: 0 yA01, 1 yA11, 2 yB01, 3 yB00
+  if (full) own_sel = lane == 2 ? 1 : ((lane == 6 || lane == 15) ? 2 : (lane == 23 ? 3 : 0));
+  else own_sel = (((j + 1) & 7) < 4) ? 0 : 2;
+  // Q[storage row k0 + 4u][position 2j], [position 2j + 1]; identity: local row k sits in storage row qrow(k), and
+  // position 2i (2i+1) is local column i (8+i)
+  double qt[4], qb[4];
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
-    qt[u] = (qrow(2 * j) == k0 + 4 * u) ? 1.0 : 0.0;
-    qb[u] = (qrow(2 * j + 1) == k0 + 4 * u) ? 1.0 : 0.0;
+    qt[u] = (qrow(j) == k0 + 4 * u) ? 1.0 : 0.0;
+    qb[u] = (qrow(8 + j) == k0 + 4 * u) ? 1.0 : 0.0;
   }
   double app = 1.0, aqq = 1.0, apq = 0.0, c, s, t;
   if (need) {
-    const double2 d0 = *reinterpret_cast<const double2*>(S + (2 * j) * LDSS + 2 * j);
-    const double2 d1 = *reinterpret_cast<const double2*>(S + (2 * j + 1) * LDSS + 2 * j);
+    const double2 d0 = *reinterpret_cast<const double2*>(S + (2 * j) * LDS_ + 2 * j);
+    const double2 d1 = *reinterpret_cast<const double2*>(S + (2 * j + 1) * LDS_ + 2 * j);
     app = d0.x; apq = d0.y; aqq = d1.y;
   }
   bool doit = rotation(app, aqq, apq, tol2, c, s, t);
   bool any = false;
+  const int nrounds = need ? (full ? 15 : 8) : 0;
 #pragma unroll 1
-  for (int r = 0; r < (need ? 15 : 0); ++r) {
+  for (int r = 0; r < nrounds; ++r) {
     const double2 a0 = *reinterpret_cast<const double2*>(ldA);
-    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDSS);
+    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDS_);
     const double2 b0 = *reinterpret_cast<const double2*>(ldB);
-    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDSS);
+    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDS_);
     __syncwarp();  // every lane has read its inputs before anybody stores
     any |= doit;
     const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
     const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
     const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
     // block (k0, j)
-    double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
-    double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
-    double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
-    double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
+    const double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
+    const double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
+    const double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
+    const double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
     // block (k0 + 4, j)
-    double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
-    double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
-    double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
-    double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
+    const double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
+    const double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
+    const double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
+    const double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
     // next round's pivot by shuffle
     const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
-    double appn = __shfl_sync(0xffffffffu, j == 0 ? dbot : dtop, src_pp);
+    double appn = __shfl_sync(0xffffffffu, fix0 ? dbot : dtop, src_pp);
     double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
     const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
-    if (j == 0) appn = dtop;
-    if (j == 7) aqqn = dtop;
+    if (fix0) appn = dtop;
+    if (fix7) aqqn = dtop;
     // this round's stores, at the positions of the next round
     stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
     stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
-    // Q <- Q R, then the columns move: top_j <- top_{j-1} (top_1 <- bot_0, top_0 stays), bot_j <- bot_{j+1} (bot_7 <- top_7)
+    // Q <- Q R, then the columns move like the positions
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const double nt = c * qt[u] - s * qb[u], nb = s * qt[u] + c * qb[u];
-      const double mt = __shfl_sync(0xffffffffu, j == 0 ? nb : nt, grp | src_pp);
+      const double mt = __shfl_sync(0xffffffffu, fix0 ? nb : nt, grp | src_pp);
       const double mb = __shfl_sync(0xffffffffu, nb, grp | src_qq);
-      qt[u] = j == 0 ? nt : mt;
-      qb[u] = j == 7 ? nt : mb;
+      qt[u] = fix0 ? nt : mt;
+      qb[u] = fix7 ? nt : mb;
     }
     app = appn; aqq = aqqn; apq = apqn;
     doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
@@ -357,16 +264,18 @@ __device__ __forceinline__ bool inner_solve_qreg(const AView<kHalf>& A, double* 
   const bool anyw = __any_sync(0xffffffffu, any);
   if (anyw) {
     for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
-      int a = e >> 4, b = e & 15;
-      int r = 8 * (a < 8 ? I : J) + (a & 7), c = 8 * (b < 8 ? I : J) + (b & 7);
-      A.put(r, c, a <= b ? S[a * LDSS + b] : S[b * LDSS + a]);
+      const int a = e >> 4, b = e & 15;
+      const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c2 = 8 * ((b & 1) ? J : I) + (b >> 1);
+      A.put(r, c2, a <= b ? S[a * LDS_ + b] : S[b * LDS_ + a]);
     }
   }
   __syncwarp();
-  // Q over the scratch, in the layout of the DMMA B fragments: storage row sr, column c at c ^ ((sr & 3) << 2)
+  // Q over the scratch: storage row sr, local column c at c ^ ((sr & 3) << 2); position 2j -> column j, 2j+1 -> 8+j
 #pragma unroll
-  for (int u = 0; u < 4; ++u)
-    *reinterpret_cast<double2*>(S + (k0 + 4 * u) * LDQ + ((2 * j) ^ (k0 << 2))) = make_double2(qt[u], qb[u]);
+  for (int u = 0; u < 4; ++u) {
+    S[(k0 + 4 * u) * LDQ + (j ^ (k0 << 2))] = qt[u];
+    S[(k0 + 4 * u) * LDQ + ((8 + j) ^ (k0 << 2))] = qb[u];
+  }
   return anyw;
 }
 
@@ -554,7 +463,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
   int I, J;
   decode_slot(__ldg(P.tab + tn * nslots + sn), I, J);
-  if (kMode != 1 || J < 0)  // identity (the register variant of the pivot solve writes its own Q)
+  if (J < 0)  // no pivot: identity (a pivot solve writes its own Q)
     for (int e = lane; e < 256; e += 32) {
       const int sr = e >> 4, c = e & 15;
       Qn[sr * LDQ + (c ^ ((sr & 3) << 2))] = (qrow(c) == sr) ? 1.0 : 0.0;
@@ -573,8 +482,10 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
       }
     }
     __syncwarp();
-    if (kMode == 1) rotated = inner_solve_qreg(A, Qn, I, J, P.tol, lane);
-    else rotated = inner_solve(A, sm.S + widx * 16 * LDSS, Qn, I, J, P.tol, lane);
+    // full sweep of the pivot every kFullEvery-th step (every block then sits in a pivot at >= 1 full step per sweep,
+    // so every pair is still met in every sweep); always for small matrices, where padding leaves few real pivots
+    const bool full = (tn % kFullEvery) == 0 || P.nb < 8;
+    rotated = inner_solve(A, Qn, I, J, P.tol, full, lane);
   }
   if (lane == 0) {
     sm.rot[bn * nslots + sn] = rotated ? 1 : 0;
@@ -582,9 +493,9 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   }
 }
 
-// kMode 0: A (full), V, Q, pivot scratch in shared memory (n <= 104)
+// kMode 0: A (full), V, Q in shared memory (n <= 104); the pivot scratch is always the slot's own Q array
 //       1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
-//       2: A (full), V in the global workspace, Q and pivot scratch in shared memory
+//       2: A (full), V in the global workspace, Q in shared memory
 //       3: as 2 with Q in the global workspace too (very large n)
 template <int kMode>
 __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
@@ -608,8 +519,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
     }
     if (kMode == 3) sm.Q = g;
     else { sm.Q = d; d += (size_t)2 * nslots * kQSlot; }
-    sm.S = d;
-    if (kMode != 1) d += (nslots < kPivotWarps ? nslots : kPivotWarps) * 16 * LDSS;
     sm.wsort = d; d += np;
     int* ip = reinterpret_cast<int*>(d);
     sm.rot = ip; ip += 2 * nslots;
@@ -753,16 +662,14 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
   g.tab_bytes = (((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255;
-  const int nS = g.nslots < kPivotWarps ? g.nslots : kPivotWarps;
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
-  const size_t scratch = (size_t)nS * 16 * LDSS * 8;
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
-  if (misc + scratch + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + scratch + q + a_full + v; g.gstride = 0; }
+  if (misc + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + q + a_full + v; g.gstride = 0; }
   else if (misc + q + a_half <= cap) { g.mode = 1; g.smem = misc + q + a_half; g.gstride = v / 8; }
-  else if (misc + scratch + q <= cap) { g.mode = 2; g.smem = misc + scratch + q; g.gstride = (a_full + v) / 8; }
-  else { g.mode = 3; g.smem = misc + scratch; g.gstride = (a_full + v + q) / 8; }
+  else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
+  else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
   return g;
 }
 
