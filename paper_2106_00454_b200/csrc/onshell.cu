@@ -171,6 +171,105 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
   }
 }
 
+// Variant for n <= kI1MaxN: the rows of VC come from the eigen-identity (VC)_ik = C_ik (eps_k - e_i), which follows
+// from H C = C D with H0 diagonal (coupled: e_{i mod N}); no V C product, only the on-shell rows of C are read (straight
+// from global memory, coalesced along k), V_ii from the diagonal of H.  The identity inherits the eigen-residual
+// eps ||H|| instead of eps ||V||: at n <= 200 the phase shifts move by < 6e-10 degrees against the direct product
+// (DESIGN.md section 6), so it is gated by size and the direct kernel above stays the path for larger n.
+constexpr int kI1MaxN = 200;
+
+__global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int N = P.N, n = P.n, nc = P.nc, nE = P.nE;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kOnThreads / 32;
+  double* sW = reinterpret_cast<double*>(smem_raw);  // [n]
+  double* sLo = sW + n;                                // [n]
+  double* sHi = sLo + n;                               // [n]
+  __shared__ int s_nb;
+  const size_t mat = blockIdx.x;
+  const double* H = P.H + mat * (size_t)n * n;
+  const double* C = P.C + mat * (size_t)n * n;
+  const double* W = P.W + mat * (size_t)n;
+  double* T = P.T + mat * (size_t)nE * nc * nc * 2;
+  if (tid == 0) s_nb = 0;
+  for (int k = tid; k < n; k += kOnThreads) sW[k] = W[k];
+  __syncthreads();
+  {
+    int cnt = 0;
+    for (int k = tid; k < n; k += kOnThreads) cnt += sW[k] < 0.0;
+    if (cnt) atomicAdd(&s_nb, cnt);
+  }
+  __syncthreads();
+  const int nbd = s_nb;
+  for (int k = tid; k < n; k += kOnThreads) {
+    double lo = 0.0, hi = 0.0;
+    if (k >= nbd) {
+      int br = (k - nbd) % nc, i = (k - nbd) / nc;
+      int mbr = (n - nbd - br + nc - 1) / nc;  // states in this branch
+      double w = sW[k];
+      lo = i == 0 ? 0.0 : 0.5 * (sW[k - nc] + w);
+      if (i < mbr - 1) hi = 0.5 * (w + sW[k + nc]);
+      else if (mbr == 1) hi = 2.0 * w;
+      else {
+        double lop = i == 1 ? 0.0 : 0.5 * (sW[k - 2 * nc] + sW[k - nc]);
+        hi = w + 0.5 * (lo - lop);
+      }
+    }
+    sLo[k] = lo; sHi[k] = hi;
+  }
+  __syncthreads();
+  for (int e = warp; e < nE; e += nwarps) {
+    const int b = P.bin[e];
+    if (b < 0) {
+      if (lane < nc * nc * 2) T[(size_t)e * nc * nc * 2 + lane] = 0.0;
+      continue;
+    }
+    const double E = P.Ecm[e], e0b = P.e0[b];
+    const double* c0 = C + (size_t)b * n;
+    const double* c1 = C + (size_t)((nc - 1) * N + b) * n;  // == c0 for uncoupled
+    double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
+    for (int k = lane; k < n; k += 32) {
+      double gr, gi = 0.0;
+      if (k < nbd) gr = 1.0 / (E - sW[k]);
+      else {
+        double lo = sLo[k], hi = sHi[k], wdt = hi - lo;
+        gr = log(fabs((E - lo) / (E - hi))) / wdt;
+        if (E >= lo && E < hi) gi = -WPCD_PI / wdt;
+      }
+      const double w = sW[k] - e0b;
+      const double a = c0[k] * w;
+      re00 = fma(a * a, gr, re00); im00 = fma(a * a, gi, im00);
+      if (nc == 2) {
+        const double bb = c1[k] * w;
+        re01 = fma(a * bb, gr, re01); im01 = fma(a * bb, gi, im01);
+        re11 = fma(bb * bb, gr, re11); im11 = fma(bb * bb, gi, im11);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      re00 += __shfl_xor_sync(0xffffffffu, re00, o); im00 += __shfl_xor_sync(0xffffffffu, im00, o);
+      if (nc == 2) {
+        re01 += __shfl_xor_sync(0xffffffffu, re01, o); im01 += __shfl_xor_sync(0xffffffffu, im01, o);
+        re11 += __shfl_xor_sync(0xffffffffu, re11, o); im11 += __shfl_xor_sync(0xffffffffu, im11, o);
+      }
+    }
+    if (lane == 0) {
+      const double* h0 = H + (size_t)b * n;  // row (0, b) of H; V = H - diag(e0)
+      if (nc == 1) {
+        T[(size_t)e * 2] = (h0[b] - e0b) + re00;
+        T[(size_t)e * 2 + 1] = im00;
+      } else {
+        const double* h1 = H + (size_t)(N + b) * n;  // row (1, b)
+        double* t = T + (size_t)e * 8;
+        t[0] = (h0[b] - e0b) + re00;     t[1] = im00;
+        t[2] = h0[N + b] + re01;         t[3] = im01;
+        t[4] = h1[b] + re01;             t[5] = im01;
+        t[6] = (h1[N + b] - e0b) + re11; t[7] = im11;
+      }
+    }
+  }
+}
+
 __global__ void k_phase(int coupled, size_t total, int nE, const double* __restrict__ T, const int* __restrict__ bin,
                         const double* __restrict__ dE, double* __restrict__ delta, double* __restrict__ S) {
   size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -225,6 +324,10 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   size_t smem = (size_t)(3 * P.n + 2 * P.R * P.nc * P.n) * 8;
   if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   k_bins<<<1, 256, 0, st>>>(N, nE, d_Eedge, d_Ecm, d_bin, static_cast<int*>(d_work));
+  if (P.n <= kI1MaxN) {
+    k_onshell_i1<<<batch, kOnThreads, (size_t)3 * P.n * 8, st>>>(P);
+    return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
+  }
   int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
   if (rc) return rc;
   k_onshell<<<batch, kOnThreads, smem, st>>>(P);
