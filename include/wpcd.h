@@ -98,17 +98,20 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
                         int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl,
                         double* d_e0, double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, void* stream);
 
-/* Step (ii), Eq. 21.  Batched real-symmetric eigendecomposition by two-sided block-Jacobi (8-wide blocks paired in
- * a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered Jacobi sweep inside one warp; the
+/* Step (ii), Eq. 21.  Batched real-symmetric eigendecomposition by two-sided block-Jacobi, one CTA per matrix: 8-wide
+ * blocks paired in a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered (Brent-Luk) Jacobi
+ * sweep inside one warp -- all 120 pairs every 4th step, the 64 pairs between the two blocks otherwise; the
  * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products; the pivots of the next step
- * are solved while the current step's updates run).  n <= 104: one CTA per matrix, matrix and eigenvectors resident
- * in shared memory; larger n: same algorithm through a global workspace kept L2 resident.
+ * are solved while the current step's updates run.  n <= 104: matrix and eigenvectors resident in shared memory;
+ * n <= 200: the matrix (upper 8x8 blocks) in shared memory, the eigenvectors in an L2-resident workspace; larger n:
+ * both through the workspace.
  *   d_A    : [batch][n][n] input (only read; must be symmetric)
  *   d_W    : [batch][n] eigenvalues ascending
  *   d_C    : [batch][n][n] eigenvectors, column k belongs to d_W[k]  (C_ij = <x_i|z_j>)
  *   d_info : [batch] sweeps used (>= 1), or -1 if not converged in max_sweeps
  *   tol    : a pivot is rotated iff |a_pq| > tol sqrt(|a_pp a_qq|); convergence = a full sweep without rotation.
- *            tol <= 0 selects the default 2^-52. */
+ *            tol <= 0 selects the default 2^-52.
+ *   d_work : wpcd_diag_workspace_bytes(n, batch) bytes (never 0: the schedule tables live there) */
 int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                       double tol, int max_sweeps, void* d_work, size_t work_bytes, void* stream);
 
@@ -117,7 +120,8 @@ int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double*
  *   coupled  : T^{ab}(E) = V_{(a i)(b i)} + sum_k (VC)_{(a i)k} g_k(E) (VC)_{(b i)k},  a,b in {0,1}
  * with g_k(E) = [ln|(E-lo_k)/(E-hi_k)| - i pi 1{lo_k <= E < hi_k}]/(hi_k - lo_k) (readings G2, C11), edges from
  * Eq. 23 as printed (C5), negative eigenvalues = bound states, positive eigenvalues of coupled channels alternate
- * between two branches by rank (C6).  VC = (H - diag(e0)) C is formed for the on-shell rows only.
+ * between two branches by rank (C6).  VC = (H - diag(e0)) C is formed for the on-shell rows only; for n <= 200 through
+ * the identity (VC)_ik = C_ik (eps_k - e_i) (H C = C D, H0 diagonal), which needs no product at all.
  *   d_H, d_W, d_C : as given to / returned by wpcd_diag_batched (n = N or 2N)
  *   d_Ecm  : [nE] c.m. energies, MeV;  mode: 0 = point-wise resolvent (only mode implemented)
  *   d_T    : [batch][nE][2] (re,im) or [batch][nE][2][2][2] for coupled;  zero where E is outside the grid

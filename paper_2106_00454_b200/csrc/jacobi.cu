@@ -583,6 +583,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
           if (lane == 0) it = atomicAdd(queue, 1);
           it = __shfl_sync(0xffffffffu, it, 0);
           if (it >= nitems) break;
+          if (kMode == 1) {  // V lives in global memory, A in shared: interleave the (L2-latency bound) V items with the tiles
+            const int nv = nitems - ntiles, nmix = 2 * (ntiles < nv ? ntiles : nv);
+            if (it < nmix) it = (it & 1) ? ntiles + (it >> 1) : (it >> 1);
+            else if (nv < ntiles) it -= nv;  // the remaining tiles (remaining V items keep their index)
+          }
           if (it < ntiles) {
             const int e = __ldg(tab_tile + it);
             const int s1 = e & 0xFFF, s2 = (e >> 12) & 0xFFF;
