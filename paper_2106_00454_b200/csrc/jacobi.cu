@@ -107,6 +107,7 @@ struct Smem {
   int* rot;      // [2][nslots] slot rotated something
   int* src;      // [np]
   int* ctr;      // [0..1] work queues (step parity), [2..3] rotations per sweep (sweep parity)
+  const int* tab; // slot and feed tables [2][m-1][nslots]: shared-memory copy (modes 0, 1) or k_schedule's global ones
 };
 
 // ---------------------------------------------------------------------------------------------- pivot solve
@@ -462,7 +463,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   const int m = P.m, nslots = P.nslots;
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
   int I, J;
-  decode_slot(__ldg(P.tab + tn * nslots + sn), I, J);
+  decode_slot(sm.tab[tn * nslots + sn], I, J);
   if (J < 0)  // no pivot: identity (a pivot solve writes its own Q)
     for (int e = lane; e < 256; e += 32) {
       const int sr = e >> 4, c = e & 15;
@@ -471,12 +472,12 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   bool rotated = false;
   if (J >= 0) {
     if (has_cur) {
-      const int f = __ldg(P.tab + (m - 1) * nslots + tn * nslots + sn);
+      const int f = sm.tab[(m - 1) * nslots + tn * nslots + sn];
       const int s1 = f & 0xFFFF, s2 = f >> 16;
       if (sm.rot[bc * nslots + s1] | sm.rot[bc * nslots + s2]) {
         int I1, J1, I2, J2;
-        decode_slot(__ldg(P.tab + t * nslots + s1), I1, J1);
-        decode_slot(__ldg(P.tab + t * nslots + s2), I2, J2);
+        decode_slot(sm.tab[t * nslots + s1], I1, J1);
+        decode_slot(sm.tab[t * nslots + s2], I2, J2);
         const double* Qc = sm.Q + (size_t)bc * nslots * kQSlot;
         apply_tile(A, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
       }
@@ -523,8 +524,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
     int* ip = reinterpret_cast<int*>(d);
     sm.rot = ip; ip += 2 * nslots;
     sm.src = ip; ip += np;
-    sm.ctr = ip;
+    sm.ctr = ip; ip += 4;
+    if (kMode <= 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
+      for (int e = tid; e < 2 * (m - 1) * nslots; e += kThreads) ip[e] = P.tab[e];
+      sm.tab = ip;
+    } else {
+      sm.tab = P.tab;
+    }
   }
+  __syncthreads();
   // Pivot solves are latency bound and suffer when DMMAs of the update queue the same FP64 pipe: they run on the
   // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
   const int widx = ((warp & 3) < kPivotSmsp) ? (warp >> 2) * kPivotSmsp + (warp & 3) : -1;
@@ -576,7 +584,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
         const int* rot = sm.rot + buf * nslots;
         const double* Qc = sm.Q + (size_t)buf * nslots * kQSlot;
         int* queue = sm.ctr + (gstep & 1);
-        const int* tab_slot = P.tab + step * nslots;
+        const int* tab_slot = sm.tab + step * nslots;
         const int* tab_tile = P.tab + 2 * (m - 1) * nslots + step * ntiles;
         for (;;) {
           int it = 0;
@@ -594,8 +602,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
             if (!(rot[s1] | rot[s2])) continue;
             if (do_next && (e >> 24)) continue;  // feeds a pivot of the next step: done by that pivot's warp
             int I1, J1, I2, J2;
-            decode_slot(__ldg(tab_slot + s1), I1, J1);
-            decode_slot(__ldg(tab_slot + s2), I2, J2);
+            decode_slot(tab_slot[s1], I1, J1);
+            decode_slot(tab_slot[s2], I2, J2);
             if (I1 < 0 || I2 < 0) continue;
             apply_tile(Av, Qc + (size_t)s1 * kQSlot, Qc + (size_t)s2 * kQSlot, I1, J1, I2, J2, lane);
           } else {
@@ -603,7 +611,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
             const int s = (int)(((float)v + 0.5f) * rnvgrp), grp = v - s * nvgrp;
             if (!rot[s]) continue;
             int I, J;
-            decode_slot(__ldg(tab_slot + s), I, J);
+            decode_slot(tab_slot[s], I, J);
             int rb0 = grp * kVRowBlocksPerItem, rb1 = rb0 + kVRowBlocksPerItem;
             if (rb1 > nb) rb1 = nb;
             apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rb0, rb1, lane);
@@ -668,11 +676,12 @@ Geometry geometry(const WpcdHandle* h, int n) {
   g.nslots = g.m / 2;
   g.tab_bytes = (((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255;
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
+  const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
-  if (misc + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + q + a_full + v; g.gstride = 0; }
-  else if (misc + q + a_half <= cap) { g.mode = 1; g.smem = misc + q + a_half; g.gstride = v / 8; }
+  if (misc + tabs + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + tabs + q + a_full + v; g.gstride = 0; }
+  else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
   else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
   else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
   return g;
