@@ -33,13 +33,9 @@ __device__ long long wpcd_prof[8];
 #define WPCD_PROF_ADD(k, v) atomicAdd((unsigned long long*)&wpcd_prof[k], (unsigned long long)(v))
 #endif
 
-constexpr int kThreads = 512;
-constexpr int kWarps = kThreads / 32;
 constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), columns XOR-swizzled by the storage row
 constexpr int kQSlot = 16 * LDQ;
 constexpr int kFullEvery = 4;  // a full 16x16 pivot sweep every 4th step of the block tournament, cross-only sweeps between
-constexpr int kPivotSmsp = 4;                          // SM sub-partitions reserved for the pivot solves
-constexpr int kPivotWarps = kWarps / 4 * kPivotSmsp;   // warps that solve pivots
 
 // A: XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
 __device__ __forceinline__ int swz(int r, int c) { return c ^ (((r & 6) << 1) ^ ((r & 1) << 3)); }
@@ -498,8 +494,11 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 //       1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
 //       2: A (full), V in the global workspace, Q in shared memory
 //       3: as 2 with Q in the global workspace too (very large n)
-template <int kMode>
-__global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
+// kThr: 512 threads (one CTA per SM), or 256 / 128 (two / four CTAs per SM) where shared memory allows and a step has
+// no more pivots than the CTA has warps: several matrices in flight per SM fill each other's pivot-chain bubbles.
+template <int kMode, int kThr>
+__global__ void __launch_bounds__(kThr, 512 / kThr) k_jacobi(JacobiParams P) {
+  constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
   constexpr bool kHalf = (kMode == 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -535,7 +534,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
   __syncthreads();
   // Pivot solves are latency bound and suffer when DMMAs of the update queue the same FP64 pipe: they run on the
   // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
-  const int widx = ((warp & 3) < kPivotSmsp) ? (warp >> 2) * kPivotSmsp + (warp & 3) : -1;
+  const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
   const AView<kHalf> Av{sm.A, ld, nb};
   const int ntiles = nslots * (nslots - 1) / 2;
   const int nvgrp = (nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
@@ -659,7 +658,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_jacobi(JacobiParams P) {
 struct Geometry {
   size_t tab_bytes;  // schedule tables at the head of the workspace
   int nb, np, ld, ldv, m, nslots;
-  int mode;        // k_jacobi<mode>
+  int mode;        // k_jacobi<mode, threads>
+  int threads;
   size_t gstride;  // doubles of global workspace per CTA
   size_t smem;     // dynamic shared memory of the launch (bytes)
 };
@@ -680,27 +680,30 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
-  if (misc + tabs + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + tabs + q + a_full + v; g.gstride = 0; }
+  g.threads = 512;
+  const size_t smem1 = misc + tabs + q + a_half;
+  if (g.nslots <= 4 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 128; g.smem = smem1; g.gstride = v / 8; }
+  else if (g.nslots <= 8 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 256; g.smem = smem1; g.gstride = v / 8; }
+  else if (misc + tabs + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + tabs + q + a_full + v; g.gstride = 0; }
   else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
   else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
   else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
   return g;
 }
 
-// CTAs of the workspace paths: two per SM only while two CTAs' shared memory fits one SM and all workspaces together
-// stay well inside L2 (measured: a 100 MB working set already spills to HBM -- the 126 MB L2 is split over two dies);
-// otherwise one per SM.
+// CTAs of the workspace paths: as many as fit an SM (512 / threads: registers are 128 per thread), each with its own
+// workspace.  All workspaces together must stay inside L2 (measured: a 100 MB working set already spills to HBM -- the
+// 126 MB L2 is split over two dies); the mode-1 sets are 25-50 MB.
 int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
-  const bool two = ((size_t)2 * h->num_sms * g.gstride * 8 <= ((size_t)48 << 20)) && (2 * (g.smem + 1024) <= (size_t)h->max_smem_optin);
-  const int grid = (two ? 2 : 1) * h->num_sms;
+  const int grid = (512 / g.threads) * h->num_sms;
   return batch < grid ? batch : grid;
 }
 
-template <int kMode>
+template <int kMode, int kThr>
 int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cudaStream_t st) {
-  int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<kMode>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "jacobi attr");
+  int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_jacobi<kMode, kThr>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "jacobi attr");
   if (rc) return rc;
-  k_jacobi<kMode><<<grid, kThreads, smem, st>>>(P);
+  k_jacobi<kMode, kThr><<<grid, kThr, smem, st>>>(P);
   return WPCD_OK;
 }
 
@@ -728,10 +731,14 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work));
   int rc;
   switch (g.mode) {
-    case 0: rc = launch_mode<0>(h, P, grid, g.smem, st); break;
-    case 1: rc = launch_mode<1>(h, P, grid, g.smem, st); break;
-    case 2: rc = launch_mode<2>(h, P, grid, g.smem, st); break;
-    default: rc = launch_mode<3>(h, P, grid, g.smem, st); break;
+    case 0: rc = launch_mode<0, 512>(h, P, grid, g.smem, st); break;
+    case 1:
+      rc = g.threads == 128   ? launch_mode<1, 128>(h, P, grid, g.smem, st)
+           : g.threads == 256 ? launch_mode<1, 256>(h, P, grid, g.smem, st)
+                              : launch_mode<1, 512>(h, P, grid, g.smem, st);
+      break;
+    case 2: rc = launch_mode<2, 512>(h, P, grid, g.smem, st); break;
+    default: rc = launch_mode<3, 512>(h, P, grid, g.smem, st); break;
   }
   if (rc) return rc;
   return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch");
