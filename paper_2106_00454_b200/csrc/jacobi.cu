@@ -33,7 +33,7 @@ __device__ long long wpcd_prof[8];
 #define WPCD_PROF_ADD(k, v) atomicAdd((unsigned long long*)&wpcd_prof[k], (unsigned long long)(v))
 #endif
 
-constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), columns XOR-swizzled by the storage row
+constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), column pairs XOR-swizzled by the storage row
 constexpr int kQSlot = 16 * LDQ;
 constexpr int kFullEvery = 4;  // a full 16x16 pivot sweep every 4th step of the block tournament, cross-only sweeps between
 
@@ -48,7 +48,9 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
 
 // Q layout: logical row k sits in storage row qrow(k) -- within each group of 8 rows the order is 0,2,4,6,1,3,5,7 so
 // that the k-chunks {8c+2t+r : t=0..3} used by the MMAs are 4 consecutive storage rows -- and column c of storage
-// row sr sits at c ^ ((sr & 3) << 2), which makes the B-fragment loads bank-conflict free with LDQ = 16.
+// row sr sits at 2 ((c & 7) ^ 2 (sr & 3)) + (c >> 3): columns g and 8+g are adjacent (one 16-byte load feeds both
+// column blocks of an MMA step) and the fragment loads are bank-conflict free with LDQ = 16.
+__device__ __forceinline__ int qoff(int sr, int c) { return sr * LDQ + 2 * ((c & 7) ^ (2 * (sr & 3))) + (c >> 3); }
 __device__ __forceinline__ int qrow(int k) { return (k & 8) | ((k & 1) << 2) | ((k >> 1) & 3); }
 
 // View of the symmetric working matrix A.
@@ -267,11 +269,10 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
     }
   }
   __syncwarp();
-  // Q over the scratch: storage row sr, local column c at c ^ ((sr & 3) << 2); position 2j -> column j, 2j+1 -> 8+j
+  // Q over the scratch (layout qoff): position 2j -> local column j, 2j+1 -> 8+j, which are adjacent
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
-    S[(k0 + 4 * u) * LDQ + (j ^ (k0 << 2))] = qt[u];
-    S[(k0 + 4 * u) * LDQ + ((8 + j) ^ (k0 << 2))] = qb[u];
+    *reinterpret_cast<double2*>(S + qoff(k0 + 4 * u, j)) = make_double2(qt[u], qb[u]);
   }
   return anyw;
 }
@@ -289,6 +290,15 @@ __device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double
 #pragma unroll
     for (int c = 0; c < 2; ++c)
       if (ni < n1 && c < n2) tf[ni][c] = A.load_frag(rb[ni], cb[c], g, t);
+  // Q fragments: one 16-byte load gives the entries of columns g and 8+g of storage row 8c+4r+t
+  double2 q2[2][2], q1[2][2];
+#pragma unroll
+  for (int c = 0; c < 2; ++c)
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      if (c < n2) q2[c][r] = *reinterpret_cast<const double2*>(Q2 + qoff(8 * c + 4 * r + t, g));
+      if (c < n1) q1[c][r] = *reinterpret_cast<const double2*>(Q1 + qoff(8 * c + 4 * r + t, g));
+    }
   // step A: U^T = Q2^T T^T ;  ut[mi][ni] holds U[8ni+2t+{0,1}][8mi+g]
   double ut[2][2][2];
 #pragma unroll
@@ -303,7 +313,7 @@ __device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double
         if (c < n2) {
 #pragma unroll
           for (int r = 0; r < 2; ++r) {
-            double a = Q2[(8 * c + 4 * r + t) * LDQ + ((8 * mi + g) ^ (t << 2))];
+            const double a = mi ? q2[c][r].y : q2[c][r].x;
 #pragma unroll
             for (int ni = 0; ni < 2; ++ni)
               if (ni < n1) dmma(ut[mi][ni], a, r ? tf[ni][c].y : tf[ni][c].x);
@@ -324,7 +334,7 @@ __device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double
         if (c < n1) {
 #pragma unroll
           for (int r = 0; r < 2; ++r) {
-            double a = Q1[(8 * c + 4 * r + t) * LDQ + ((8 * mi + g) ^ (t << 2))];
+            const double a = mi ? q1[c][r].y : q1[c][r].x;
 #pragma unroll
             for (int nj = 0; nj < 2; ++nj)
               if (nj < n2) dmma(out[mi][nj], a, ut[nj][c][r]);
@@ -354,13 +364,12 @@ __device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const 
                                           int rb0, int rb1, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int cb[2] = {I, J};
-  double bq[2][2][2];
+  double2 bq[2][2];
 #pragma unroll
   for (int c = 0; c < 2; ++c)
 #pragma unroll
     for (int r = 0; r < 2; ++r)
-#pragma unroll
-      for (int ni = 0; ni < 2; ++ni) bq[c][r][ni] = (c < nbk && ni < nbk) ? Q[(8 * c + 4 * r + t) * LDQ + ((8 * ni + g) ^ (t << 2))] : 0.0;
+      if (c < nbk) bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
   for (int rb = rb0; rb < rb1; ++rb) {
     const int row = 8 * rb + g;
     double2 vf[2];
@@ -378,7 +387,7 @@ __device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const 
         for (int r = 0; r < 2; ++r)
 #pragma unroll
           for (int ni = 0; ni < 2; ++ni)
-            if (ni < nbk) dmma(out[ni], r ? vf[c].y : vf[c].x, bq[c][r][ni]);
+            if (ni < nbk) dmma(out[ni], r ? vf[c].y : vf[c].x, ni ? bq[c][r].y : bq[c][r].x);
       }
 #pragma unroll
     for (int ni = 0; ni < 2; ++ni)
@@ -463,7 +472,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   if (J < 0)  // no pivot: identity (a pivot solve writes its own Q)
     for (int e = lane; e < 256; e += 32) {
       const int sr = e >> 4, c = e & 15;
-      Qn[sr * LDQ + (c ^ ((sr & 3) << 2))] = (qrow(c) == sr) ? 1.0 : 0.0;
+      Qn[qoff(sr, c)] = (qrow(c) == sr) ? 1.0 : 0.0;
     }
   bool rotated = false;
   if (J >= 0) {
