@@ -102,9 +102,8 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
  * blocks paired in a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered (Brent-Luk) Jacobi
  * sweep inside one warp -- all 120 pairs every 4th step, the 64 pairs between the two blocks otherwise; the
  * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products; the pivots of the next step
- * are solved while the current step's updates run.  n <= 104: matrix and eigenvectors resident in shared memory;
- * n <= 200: the matrix (upper 8x8 blocks) in shared memory, the eigenvectors in an L2-resident workspace; larger n:
- * both through the workspace.
+ * are solved while the current step's updates run.  n <= 200: the matrix (upper 8x8 blocks) in shared memory, the
+ * eigenvectors in an L2-resident workspace, 1-4 matrices in flight per SM; larger n: both through the workspace.
  *   d_A    : [batch][n][n] input (only read; must be symmetric)
  *   d_W    : [batch][n] eigenvalues ascending
  *   d_C    : [batch][n][n] eigenvectors, column k belongs to d_W[k]  (C_ij = <x_i|z_j>)

@@ -1,21 +1,23 @@
 // jacobi.cu -- step (ii) of the WPCD recipe: H = C D C^T (Eq. 21), batched, fp64.
 //
 // Two-sided BLOCK Jacobi, one CTA per matrix, software-pipelined over the steps of the block tournament.
-//   * The n x n matrix is cut into 8-wide blocks.  A round-robin tournament (jacobi_schedule.cuh) pairs the blocks;
-//     each pair (I,J) is a "slot" with a 16x16 symmetric pivot sub-problem S = A[IJ,IJ].
-//   * Pivot solve (one warp per slot): one full Brent-Luk sweep of S (15 rounds of 8 disjoint rotations, classical
-//     rotation angle, division-free), accumulating the 16x16 orthogonal Q.  It is latency bound.
-//   * Apply (all warps, dynamic work queue): A <- Q^T A Q tile by tile (one tile per slot pair; the mirror image is
-//     stored too) and V <- V Q, as fp64 tensor-core products (mma.sync m8n8k4 = DMMA, which runs at the full FP64
-//     rate of the SM with operands distributed over the warp).  The accumulator fragment of the first product is
-//     re-used directly as the B fragment of the second one (the k index of an MMA may be permuted freely), so a
-//     two-sided tile update needs no shuffle and no shared-memory round trip.
+//   * The n x n matrix is cut into 8-wide blocks.  A round-robin tournament (jacobi_schedule.cuh; tables written once
+//     per launch by k_schedule) pairs the blocks; each pair (I,J) is a "slot" with a 16x16 symmetric pivot
+//     sub-problem S = A[IJ,IJ].
+//   * Pivot solve (one warp per slot): one Brent-Luk sweep of S -- all 120 pairs (15 rounds of 8 disjoint rotations)
+//     every 4th step, the 64 pairs between the two blocks (8 rounds) otherwise -- with the classical rotation angle,
+//     division-free, accumulating the 16x16 orthogonal Q in registers.  A serial chain of rounds: latency/issue bound.
+//   * Apply (all warps, dynamic work queue): A <- Q^T A Q tile by tile (one tile per slot pair) and V <- V Q, as fp64
+//     tensor-core products (mma.sync m8n8k4 = DMMA, same flop rate as DFMA on B200 but operands distributed over the
+//     warp).  The accumulator fragment of the first product is re-used directly as the B fragment of the second one
+//     (the k index of an MMA may be permuted freely): no shuffle, no shared-memory round trip between the two sides.
 //   * Pipeline: the pivot of a slot of step g+1 only needs ONE tile of step g (its "critical" tile) besides the
-//     diagonal blocks.  In phase g the first warps update their critical tile and go straight on to the pivot solve
-//     of step g+1 (into the other Q buffer) while the remaining warps work through the other tiles and the V
-//     updates of step g; one __syncthreads per step.
+//     diagonal blocks.  In phase g a warp updates its critical tile and goes straight on to the pivot solve of step
+//     g+1 (into the other Q buffer), then joins the queue of the other tiles and the V updates of step g; one
+//     __syncthreads per step.
 //   * A sweep = m-1 steps.  Converged when a whole sweep rotates nothing (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
-// n <= 104: A and V live in shared memory; larger n: same code on a per-CTA global workspace kept L2 resident.
+// n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
+// n <= 104 with 256 threads (n <= 56: 128) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
 //
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
@@ -499,10 +501,10 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
   }
 }
 
-// kMode 0: A (full), V, Q in shared memory (n <= 104); the pivot scratch is always the slot's own Q array
-//       1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
+// kMode 1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
 //       2: A (full), V in the global workspace, Q in shared memory
 //       3: as 2 with Q in the global workspace too (very large n)
+// The pivot scratch is always the slot's own Q array.
 // kThr: 512 threads (one CTA per SM), or 256 / 128 (two / four CTAs per SM) where shared memory allows and a step has
 // no more pivots than the CTA has warps: several matrices in flight per SM fill each other's pivot-chain bubbles.
 template <int kMode, int kThr>
@@ -516,10 +518,7 @@ __global__ void __launch_bounds__(kThr, 512 / kThr) k_jacobi(JacobiParams P) {
   {
     double* d = reinterpret_cast<double*>(smem_raw);
     double* g = P.gwork + (size_t)blockIdx.x * P.gstride;
-    if (kMode == 0) {
-      sm.A = d; d += (size_t)np * ld;
-      sm.V = d; d += (size_t)np * ldv;
-    } else if (kMode == 1) {
+    if (kMode == 1) {
       sm.A = d; d += (size_t)(nb * (nb + 1) / 2) * 64;
       sm.V = g; g += (size_t)np * ldv;
     } else {
@@ -533,7 +532,7 @@ __global__ void __launch_bounds__(kThr, 512 / kThr) k_jacobi(JacobiParams P) {
     sm.rot = ip; ip += 2 * nslots;
     sm.src = ip; ip += np;
     sm.ctr = ip; ip += 4;
-    if (kMode <= 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
+    if (kMode == 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
       for (int e = tid; e < 2 * (m - 1) * nslots; e += kThreads) ip[e] = P.tab[e];
       sm.tab = ip;
     } else {
@@ -693,7 +692,6 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t smem1 = misc + tabs + q + a_half;
   if (g.nslots <= 4 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 128; g.smem = smem1; g.gstride = v / 8; }
   else if (g.nslots <= 8 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 256; g.smem = smem1; g.gstride = v / 8; }
-  else if (misc + tabs + q + a_full + v <= cap) { g.mode = 0; g.smem = misc + tabs + q + a_full + v; g.gstride = 0; }
   else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
   else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
   else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
@@ -720,7 +718,6 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
   Geometry g = geometry(h, n);
-  if (g.mode == 0) return g.tab_bytes;
   return g.tab_bytes + (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
 
@@ -735,12 +732,11 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
-  const int grid = g.mode == 0 ? batch : global_grid(h, g, batch);
-  if (work_bytes < g.tab_bytes + (g.mode != 0 ? (size_t)grid * g.gstride * 8 : 0)) return WPCD_EWORK;
+  const int grid = global_grid(h, g, batch);
+  if (work_bytes < g.tab_bytes + (size_t)grid * g.gstride * 8) return WPCD_EWORK;
   k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work));
   int rc;
   switch (g.mode) {
-    case 0: rc = launch_mode<0, 512>(h, P, grid, g.smem, st); break;
     case 1:
       rc = g.threads == 128   ? launch_mode<1, 128>(h, P, grid, g.smem, st)
            : g.threads == 256 ? launch_mode<1, 256>(h, P, grid, g.smem, st)
