@@ -127,6 +127,16 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------- GPU arm
+def max_over_ranks(values, world, device):
+    """Replicas only: the one cross-rank step of the bench is the MAX of the per-rank timings."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -192,10 +202,7 @@ def run_ours(args):
         sampler.stop_flag.set()
         sampler.join()
 
-    tms = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(tms[0]), float(tms[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], world, "cuda")
     solves = pipe.channel_solves * world
     value = solves * args.steps / (ms * 1e-3)
     e2e = solves * args.steps / (ms_e2e * 1e-3)
