@@ -34,6 +34,8 @@ _jac_ld = _sig("orc_jacobi_ld", _i, [_i, _pd, _pd, _pd, _d, _i])
 _edges = _sig("orc_swp_edges", None, [_i, _pd, _pd])
 _res = _sig("orc_resolvent_c", None, [_d, _d, _d, _pd])
 _onT = _sig("orc_onshell_T", None, [_i, _i, _pd, _pd, _pd, _pd, _pd, _i, _pd, _pi])
+_onTavg = _sig("orc_onshell_T_avg", None, [_i, _i, _pd, _pd, _pd, _pd, _pd, _i, _pd, _pi])
+_resavg = _sig("orc_resolvent_avg_c", None, [C.c_double, C.c_double, C.c_double, C.c_double, _i, _pd])
 _ph = _sig("orc_phase_shifts", None, [_i, _i, _pd, _pi, _pd, _pd, _vp])
 _migrid = _sig("orc_mi_grid", None, [_i, _d, _pd, _pd])
 _mi = _sig("orc_mi_solve", None, [_i, _i, _i, _i, _pd, _pd, _d, _d, _d, _d, _d, _d, _i, _d, _pd, _pd])
@@ -132,10 +134,17 @@ def resolvent(E, lo, hi):
     return complex(o[0], o[1])
 
 
-def onshell_T(N, coupled, Eedge, V, W, Cm, Ecm):
+def resolvent_avg(a, b, lo, hi, same_bin):
+    """Average of g(E; lo, hi) over E in [a, b] (Eqs. B.7-B.8, reading G3)."""
+    o = np.empty(2)
+    _resavg(a, b, lo, hi, 1 if same_bin else 0, o)
+    return complex(o[0], o[1])
+
+
+def onshell_T(N, coupled, Eedge, V, W, Cm, Ecm, averaged=False):
     Ecm = _f(Ecm); nE = len(Ecm); nc = 2 if coupled else 1
     T = np.empty((nE, nc, nc, 2)); b = np.empty(nE, dtype=np.int32)
-    _onT(N, 1 if coupled else 0, _f(Eedge), _f(V), _f(W), _f(Cm), Ecm, nE, T, b)
+    (_onTavg if averaged else _onT)(N, 1 if coupled else 0, _f(Eedge), _f(V), _f(W), _f(Cm), Ecm, nE, T, b)
     Tc = T[..., 0] + 1j * T[..., 1]
     return (Tc if coupled else Tc[:, 0, 0]), b
 

@@ -11,7 +11,8 @@
 //   legendre_Q       : vs mpmath.legenq (independent arbitrary-precision evaluation) and the Neumann integral
 //   V_yukawa         : vs adaptive quadrature of the radial (r-space) definition on tiny grids
 //   jacobi           : closed-form 2x2/3x3, rank-one secular equation by bisection (Yamaguchi), invariants, mpmath
-//   resolvent / T    : limits of Eq. B.3-B.6, sum rule, hand-evaluated tiny cases
+//   resolvent / T    : limits of Eq. B.3-B.6, sum rule, hand-evaluated tiny cases; energy-averaged variant (B.7-B.8)
+//                      against numerical quadrature of the point-wise resolvent and the Yamaguchi closed form
 //   phases           : closed forms of Eqs. A.3-A.5 (unit-modulus S built from known angles)
 //   MI solver        : Yamaguchi analytic phase shifts; unitarity
 //   whole WPCD chain : converges to MI as N grows
@@ -348,6 +349,85 @@ void orc_onshell_T(int N, int coupled, const double* Eedge, const double* V, con
           t = cplx(V[(size_t)ra * n + rb], 0.0);
           for (int k = 0; k < nb; ++k) t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] / (E - W[k]);
           for (int k = nb; k < n; ++k) t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] * orc_resolvent(E, lo[k], hi[k]);
+        }
+        size_t o = ((size_t)e * nc * nc + a * nc + b) * 2;
+        T[o] = t.real(); T[o + 1] = t.imag();
+      }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-1: energy-averaged resolvent, Eq. 28 and Eqs. B.7-B.8.
+// The average of g_k(E) (state bin [lo,hi]) over an averaging bin [a,b]:
+//   Re gbar = W/((b-a)(hi-lo)),  W = (b-lo)ln|b-lo| - (b-hi)ln|b-hi| - (a-lo)ln|a-lo| + (a-hi)ln|a-hi|,  x ln|x| -> 0 at 0
+//   Im gbar = -pi/(hi-lo) iff the averaging bin IS the state's bin
+// W is the antiderivative (E-c)ln|E-c| - (E-c) of ln|E-c| taken between a and b for c = lo minus the same for c = hi;
+// it is Eq. B.8 with the overall sign of the printed formula corrected (reading G3: the printed B.7 carries the same
+// sign slip as B.5/B.6, reading G2).
+static double xlnx(double x) { return x == 0.0 ? 0.0 : x * std::log(std::fabs(x)); }
+cplx orc_resolvent_avg(double a, double b, double lo, double hi, int same_bin) {
+  double W = xlnx(b - lo) - xlnx(b - hi) - xlnx(a - lo) + xlnx(a - hi);
+  return cplx(W / ((b - a) * (hi - lo)), same_bin ? -PI / (hi - lo) : 0.0);
+}
+void orc_resolvent_avg_c(double a, double b, double lo, double hi, int same_bin, double* out) {
+  cplx g = orc_resolvent_avg(a, b, lo, hi, same_bin);
+  out[0] = g.real(); out[1] = g.imag();
+}
+
+// Energy-averaged on-shell T: ONE value per on-shell FWP bin i ("if we use energy averaging we only require a single
+// evaluation for each on-shell wave packet"), returned for every requested energy of that bin.
+//   T_ii = V_ii + sum_b (VC)_ib^2 gbar_b + sum_k (VC)_ik^2 gbar_k   (coupled: the 2x2 block as in orc_onshell_T)
+// Readings (A1-A3): the averaging bin of a state of branch beta is the pseudostate bin of the i-th
+// positive state of the SAME branch (k(i) = i in the positive spectrum, Eq. 39 "g_jj(E in D_i)"); only
+// that state gets the -i pi term; a bound state's 1/(E - eps_b) is averaged over branch 0's bin:
+// ln|(b-eps_b)/(a-eps_b)|/(b-a).  If a branch has no i-th state the bin is treated as outside the grid (T = 0).
+void orc_onshell_T_avg(int N, int coupled, const double* Eedge, const double* V, const double* W, const double* C,
+                       const double* Ecm, int nE, double* T, int* bin) {
+  int n = coupled ? 2 * N : N;
+  std::vector<double> VC((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      double s = 0.0;
+      for (int j = 0; j < n; ++j) s += V[(size_t)i * n + j] * C[(size_t)j * n + k];
+      VC[(size_t)i * n + k] = s;
+    }
+  int nb = 0;
+  while (nb < n && W[nb] < 0.0) ++nb;
+  int nbranch = coupled ? 2 : 1;
+  std::vector<std::vector<int>> members(nbranch);
+  for (int k = nb; k < n; ++k) members[(k - nb) % nbranch].push_back(k);
+  std::vector<double> lo(n, 0.0), hi(n, 0.0);
+  for (int br = 0; br < nbranch; ++br) {
+    int m = (int)members[br].size();
+    if (m == 0) continue;
+    std::vector<double> eps(m), edge(m + 1);
+    for (int i = 0; i < m; ++i) eps[i] = W[members[br][i]];
+    orc_swp_edges(m, eps.data(), edge.data());
+    for (int i = 0; i < m; ++i) { lo[members[br][i]] = edge[i]; hi[members[br][i]] = edge[i + 1]; }
+  }
+  int nc = coupled ? 2 : 1;
+  for (int e = 0; e < nE; ++e) {
+    double E = Ecm[e];
+    int ib = -1;
+    for (int i = 0; i < N; ++i)
+      if (E >= Eedge[i] && E < Eedge[i + 1]) { ib = i; break; }
+    bin[e] = ib;
+    bool ok = ib >= 0;
+    for (int br = 0; br < nbranch && ok; ++br) ok = ib < (int)members[br].size();
+    for (int a = 0; a < nc; ++a)
+      for (int b = 0; b < nc; ++b) {
+        cplx t(0.0, 0.0);
+        if (ok) {
+          int ra = a * N + ib, rb = b * N + ib;
+          t = cplx(V[(size_t)ra * n + rb], 0.0);
+          int k0 = members[0][ib];
+          for (int k = 0; k < nb; ++k)
+            t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] *
+                 (std::log(std::fabs((hi[k0] - W[k]) / (lo[k0] - W[k]))) / (hi[k0] - lo[k0]));
+          for (int k = nb; k < n; ++k) {
+            int ki = members[(k - nb) % nbranch][ib];  // the i-th state of k's branch: its bin is the averaging bin
+            t += VC[(size_t)ra * n + k] * VC[(size_t)rb * n + k] * orc_resolvent_avg(lo[ki], hi[ki], lo[k], hi[k], k == ki);
+          }
         }
         size_t o = ((size_t)e * nc * nc + a * nc + b) * 2;
         T[o] = t.real(); T[o + 1] = t.imag();
