@@ -122,7 +122,14 @@ int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double*
  * between two branches by rank (C6).  VC = (H - diag(e0)) C is formed for the on-shell rows only; for n <= 200 through
  * the identity (VC)_ik = C_ik (eps_k - e_i) (H C = C D, H0 diagonal), which needs no product at all.
  *   d_H, d_W, d_C : as given to / returned by wpcd_diag_batched (n = N or 2N)
- *   d_Ecm  : [nE] c.m. energies, MeV;  mode: 0 = point-wise resolvent (only mode implemented)
+ *   d_Ecm  : [nE] c.m. energies, MeV
+ *   mode   : 0 = point-wise resolvent g_k(E) above;
+ *            1 = energy-averaged resolvent, Eq. 28 and B.7-B.8 (sign per reading G3): ONE T per
+ *                on-shell FWP bin i, returned for every energy of that bin.  State k of branch beta is
+ *                averaged over the pseudostate bin [a,b] of the i-th positive state of the same branch:
+ *                Re = W/((b-a)(hi_k-lo_k)), W = (b-lo)ln|b-lo| - (b-hi)ln|b-hi| - (a-lo)ln|a-lo| + (a-hi)ln|a-hi|,
+ *                Im = -pi/(hi_k-lo_k) for that i-th state only; bound states ln|(b-eps)/(a-eps)|/(b-a) over branch 0's
+ *                bin; T = 0 if a branch has no i-th state (readings A1-A3)
  *   d_T    : [batch][nE][2] (re,im) or [batch][nE][2][2][2] for coupled;  zero where E is outside the grid
  *   d_bin  : [nE] FWP bin of each energy (-1 if outside the grid) */
 int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,

@@ -119,11 +119,11 @@ int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_
                    double* d_T, int* d_bin, void* d_work, size_t work_bytes, void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !d_e0 || !d_Eedge || !d_H || !d_W || !d_C || !d_Ecm || !d_T || !d_bin) return WPCD_EINVAL;
-  if (N < 1 || batch < 1 || nE < 1 || mode != 0) return WPCD_EINVAL;
+  if (N < 1 || batch < 1 || nE < 1 || (mode != 0 && mode != 1)) return WPCD_EINVAL;
   size_t need = wpcd_onshell_workspace(N, coupled, batch, nE);
   if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
-  return wpcd_onshell_launch(h, N, coupled ? 1 : 0, batch, d_e0, d_Eedge, d_H, d_W, d_C, d_Ecm, nE, d_T, d_bin, d_work,
-                             work_bytes, static_cast<cudaStream_t>(stream));
+  return wpcd_onshell_launch(h, N, coupled ? 1 : 0, batch, d_e0, d_Eedge, d_H, d_W, d_C, d_Ecm, nE, mode, d_T, d_bin,
+                             d_work, work_bytes, static_cast<cudaStream_t>(stream));
 }
 
 int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,

@@ -14,6 +14,36 @@ namespace {
 
 constexpr int kOnThreads = 256;
 
+__device__ __forceinline__ double xlnx(double x) { return x == 0.0 ? 0.0 : x * log(fabs(x)); }
+
+// Resolvent of state k for the on-shell bin `b` / energy E.
+//   mode 0: point-wise, Eqs. B.5-B.6 (sign per DESIGN.md reading G2); bound states 1/(E - eps).
+//   mode 1: averaged over the pseudostate bin [lo_ki, hi_ki] of the b-th positive state ki of k's own branch, Eq. 28 and
+//           B.7-B.8 (sign per reading G3): W/((hi_ki-lo_ki)(hi_k-lo_k)) - i pi/(hi_k-lo_k) [k = ki];
+//           bound states averaged over branch 0's bin (readings A1-A3).  The caller has checked that every branch has a
+//           b-th state.
+__device__ __forceinline__ void resolvent_k(int mode, double E, int b, int k, int nbd, int nc, const double* sW,
+                                            const double* sLo, const double* sHi, double& gr, double& gi) {
+  gi = 0.0;
+  if (mode == 0) {
+    if (k < nbd) { gr = 1.0 / (E - sW[k]); return; }
+    const double lo = sLo[k], hi = sHi[k], wdt = hi - lo;
+    gr = log(fabs((E - lo) / (E - hi))) / wdt;
+    if (E >= lo && E < hi) gi = -WPCD_PI / wdt;
+    return;
+  }
+  if (k < nbd) {
+    const int k0 = nbd + nc * b;
+    const double A = sLo[k0], B = sHi[k0], w = sW[k];
+    gr = log(fabs((B - w) / (A - w))) / (B - A);
+    return;
+  }
+  const int ki = nbd + (k - nbd) % nc + nc * b;
+  const double A = sLo[ki], B = sHi[ki], lo = sLo[k], hi = sHi[k];
+  gr = (xlnx(B - lo) - xlnx(B - hi) - xlnx(A - lo) + xlnx(A - hi)) / ((B - A) * (hi - lo));
+  if (k == ki) gi = -WPCD_PI / (hi - lo);
+}
+
 __global__ void k_bins(int N, int nE, const double* __restrict__ Eedge, const double* __restrict__ Ecm,
                        int* __restrict__ bin, int* __restrict__ range) {
   __shared__ int smin, smax;
@@ -44,6 +74,7 @@ struct OnshellParams {
   const int* range;
   double* T;
   int N, n, nc, nE, R;  // R = bins per chunk
+  int mode;             // 0 point-wise resolvent (B.5-B.6), 1 energy-averaged (Eq. 28, B.7-B.8)
 };
 
 __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
@@ -90,7 +121,7 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
   }
   // energies outside the grid: T = 0
   for (int e = tid; e < nE; e += kOnThreads)
-    if (P.bin[e] < 0)
+    if (P.bin[e] < 0 || (P.mode == 1 && nbd + nc * P.bin[e] + nc - 1 >= n))
       for (int x = 0; x < nc * nc * 2; ++x) T[(size_t)e * nc * nc * 2 + x] = 0.0;
   const int bmin = P.range[0], bmax = P.range[1];
   for (int b0 = bmin; b0 <= bmax; b0 += R) {
@@ -125,18 +156,14 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
     for (int e = warp; e < nE; e += nwarps) {
       int b = P.bin[e];
       if (b < b0 || b >= b0 + nbins) continue;
+      if (P.mode == 1 && nbd + nc * b + nc - 1 >= n) continue;  // a branch has no b-th state: T = 0 (set above)
       const double E = P.Ecm[e];
       const double* vc0 = sVC + (size_t)((b - b0) * nc) * n;
       const double* vc1 = vc0 + (nc - 1) * n;  // == vc0 for uncoupled
       double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
       for (int k = lane; k < n; k += 32) {
-        double gr, gi = 0.0;
-        if (k < nbd) gr = 1.0 / (E - sW[k]);
-        else {
-          double lo = sLo[k], hi = sHi[k], wdt = hi - lo;
-          gr = log(fabs((E - lo) / (E - hi))) / wdt;
-          if (E >= lo && E < hi) gi = -WPCD_PI / wdt;
-        }
+        double gr, gi;
+        resolvent_k(P.mode, E, b, k, nbd, nc, sW, sLo, sHi, gr, gi);
         double a = vc0[k];
         re00 = fma(a * a, gr, re00); im00 = fma(a * a, gi, im00);
         if (nc == 2) {
@@ -220,7 +247,7 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
   __syncthreads();
   for (int e = warp; e < nE; e += nwarps) {
     const int b = P.bin[e];
-    if (b < 0) {
+    if (b < 0 || (P.mode == 1 && nbd + nc * b + nc - 1 >= n)) {  // outside the grid / a branch has no b-th state
       if (lane < nc * nc * 2) T[(size_t)e * nc * nc * 2 + lane] = 0.0;
       continue;
     }
@@ -229,13 +256,8 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
     const double* c1 = C + (size_t)((nc - 1) * N + b) * n;  // == c0 for uncoupled
     double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
     for (int k = lane; k < n; k += 32) {
-      double gr, gi = 0.0;
-      if (k < nbd) gr = 1.0 / (E - sW[k]);
-      else {
-        double lo = sLo[k], hi = sHi[k], wdt = hi - lo;
-        gr = log(fabs((E - lo) / (E - hi))) / wdt;
-        if (E >= lo && E < hi) gi = -WPCD_PI / wdt;
-      }
+      double gr, gi;
+      resolvent_k(P.mode, E, b, k, nbd, nc, sW, sLo, sHi, gr, gi);
       const double w = sW[k] - e0b;
       const double a = c0[k] * w;
       re00 = fma(a * a, gr, re00); im00 = fma(a * a, gi, im00);
@@ -315,10 +337,10 @@ size_t wpcd_onshell_workspace(int, int, int, int) { return 256; }
 
 int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
                         const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE,
-                        double* d_T, int* d_bin, void* d_work, size_t, cudaStream_t st) {
+                        int mode, double* d_T, int* d_bin, void* d_work, size_t, cudaStream_t st) {
   OnshellParams P;
   P.e0 = d_e0; P.H = d_H; P.W = d_W; P.C = d_C; P.Ecm = d_Ecm; P.bin = d_bin; P.range = static_cast<int*>(d_work);
-  P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE;
+  P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE; P.mode = mode;
   int budget = h->max_smem_optin < 100 * 1024 ? h->max_smem_optin : 100 * 1024;
   P.R = chunk_bins(P.n, P.nc, budget);
   size_t smem = (size_t)(3 * P.n + 2 * P.R * P.nc * P.n) * 8;

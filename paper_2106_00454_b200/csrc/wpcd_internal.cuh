@@ -30,6 +30,6 @@ int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential
 size_t wpcd_onshell_workspace(int N, int coupled, int batch, int nE);
 int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
                         const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE,
-                        double* d_T, int* d_bin, void* d_work, size_t work_bytes, cudaStream_t st);
+                        int mode, double* d_T, int* d_bin, void* d_work, size_t work_bytes, cudaStream_t st);
 int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
                       const double* d_dE, double* d_delta, double* d_S, cudaStream_t st);

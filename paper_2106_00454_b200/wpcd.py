@@ -164,7 +164,8 @@ class Handle:
         return W, Cm, info
 
     # ------------------------------------------------------------------ wpcd_onshell_T
-    def onshell_T(self, N, coupled, e0, Eedge, H, W, Cm, Ecm, stream=None, T=None, bins=None, work=None):
+    def onshell_T(self, N, coupled, e0, Eedge, H, W, Cm, Ecm, stream=None, T=None, bins=None, work=None, mode=0):
+        """mode 0: point-wise resolvent; mode 1: energy-averaged resolvent (one T per on-shell bin)."""
         batch = H.shape[0]; nE = Ecm.shape[0]; dev = H.device
         shape = (batch, nE, 2, 2, 2) if coupled else (batch, nE, 2)
         T = torch.empty(shape, dtype=torch.float64, device=dev) if T is None else T
@@ -173,7 +174,7 @@ class Handle:
         if work is None or work.numel() < wb:
             work = self._work(wb)
         rc = _lib.wpcd_onshell_T(self._h, N, int(coupled), batch, _ptr(e0), _ptr(Eedge), _ptr(H), _ptr(W), _ptr(Cm),
-                                 _ptr(Ecm), nE, 0, _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream))
+                                 _ptr(Ecm), nE, int(mode), _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream))
         self._check(rc, "wpcd_onshell_T")
         return T, bins
 

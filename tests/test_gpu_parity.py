@@ -233,3 +233,40 @@ def test_abi_argument_errors(ctx):
     g = wp.Grid(2, edges, 197.327, 469.46, 8)
     assert lib.wpcd_build_channels(h, C.byref(g), None, None, 1, None, 1, 0, None, None, None, None, None, None, 0, None) == -1
     assert wp._lib.wpcd_strerror(-3) == b"workspace too small"
+
+
+# ----------------------------------------------------------------------------------------------- NEXT-1: averaged resolvent
+@pytest.mark.parametrize("N,kind,lJ", [(50, 0, 0), (100, 1, 1), (64, 1, 2), (120, 1, 1), (210, 0, 0)])
+def test_energy_averaged_T_mode1(ctx, N, kind, lJ):
+    """wpcd_onshell_T(mode=1) (Eq. 28, B.7-B.8) against the oracle's averaged T on the same eigenpairs' inputs:
+    n <= 200 runs the identity kernel, n > 200 the direct one; uncoupled (with a bound state) and coupled channels."""
+    h, torch = ctx["h"], ctx["torch"]
+    tl, Ecm = inp.energies(120)
+    out = h.build_channels(inp.grid_edges(N), [(kind, lJ)], S=1, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+    Hd = out["H_cpl" if kind else "H_unc"]
+    n = Hd.shape[-1]
+    Hb = Hd.reshape(-1, n, n)
+    W, C, info = h.diag_batched(Hb)
+    T, bins = h.onshell_T(N, kind, out["e0"], out["Eedge"], Hb, W, C, _to_dev(ctx, Ecm), mode=1)
+    delta, Sm = h.phase_shifts(kind, T, bins, out["dE"])
+    torch.cuda.synchronize()
+    ch = hp.oracle_channel(N, kind, lJ)
+    from oracle import oracle as o
+    Wr, Cr, _ = o.jacobi(ch["H"])
+    Tr, br = o.onshell_T(N, bool(kind), ch["Eedge"], ch["V"], Wr, Cr, Ecm, averaged=True)
+    dr, Sr = o.phase_shifts(bool(kind), Tr, br, ch["dE"])
+    assert np.array_equal(bins.cpu().numpy(), br)
+    Tg = T.cpu().numpy()[0]; Tg = Tg[..., 0] + 1j * Tg[..., 1]
+    Sg = Sm.cpu().numpy()[0]; Sg = Sg[..., 0] + 1j * Sg[..., 1]
+    scale = np.abs(Tr).max()
+    assert np.abs(Tg - Tr).max() <= 1e-10 * scale, np.abs(Tg - Tr).max() / scale
+    assert np.abs(Sg - Sr).max() <= hp.TOL_S_ABS
+    d = hp.dist180(delta.cpu().numpy()[0], dr)
+    if kind:
+        d = d[:, :2]
+    assert d.max() <= hp.TOL_PHASE_DEG, d.max()
+    # one value per on-shell bin
+    bb = bins.cpu().numpy()
+    for i in np.unique(bb[bb >= 0]):
+        idx = np.where(bb == i)[0]
+        assert np.all(Tg[idx] == Tg[idx[0]])
