@@ -361,6 +361,44 @@ __device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* 
 }
 
 // V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
+// V[rows of row-blocks rb0, rb0+1][P] <- V[..][P] Q for exactly two row blocks: all four 16-byte loads are in flight
+// before the first product (V lives in global memory in every mode: L2 latency).
+template <int nbk>
+__device__ __forceinline__ void apply_V_2(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
+                                          int rb0, int lane) {
+  const int g = lane >> 2, t = lane & 3;
+  const int cb[2] = {I, J};
+  double* v0 = V + (size_t)(8 * rb0 + g) * ld + 2 * t;
+  double* v1 = v0 + (size_t)8 * ld;
+  double2 f0[2], f1[2];
+#pragma unroll
+  for (int c = 0; c < nbk; ++c) {
+    f0[c] = *reinterpret_cast<const double2*>(v0 + 8 * cb[c]);
+    f1[c] = *reinterpret_cast<const double2*>(v1 + 8 * cb[c]);
+  }
+  double2 bq[2][2];
+#pragma unroll
+  for (int c = 0; c < nbk; ++c)
+#pragma unroll
+    for (int r = 0; r < 2; ++r) bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
+  double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll
+  for (int c = 0; c < nbk; ++c)
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int ni = 0; ni < nbk; ++ni) {
+        const double q = ni ? bq[c][r].y : bq[c][r].x;
+        dmma(o0[ni], r ? f0[c].y : f0[c].x, q);
+        dmma(o1[ni], r ? f1[c].y : f1[c].x, q);
+      }
+#pragma unroll
+  for (int ni = 0; ni < nbk; ++ni) {
+    *reinterpret_cast<double2*>(v0 + 8 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
+    *reinterpret_cast<double2*>(v1 + 8 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+  }
+}
+
 template <int nbk>
 __device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
                                           int rb0, int rb1, int lane) {
@@ -402,8 +440,13 @@ __device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const 
 
 __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
                                         int rb0, int rb1, int lane) {
-  if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rb0, rb1, lane);
-  else apply_V_n<1>(V, ld, Q, I, J, rb0, rb1, lane);
+  if (rb1 - rb0 == 2) {
+    if (J >= 0) apply_V_2<2>(V, ld, Q, I, J, rb0, lane);
+    else apply_V_2<1>(V, ld, Q, I, J, rb0, lane);
+  } else {
+    if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rb0, rb1, lane);
+    else apply_V_n<1>(V, ld, Q, I, J, rb0, rb1, lane);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------- the kernel
