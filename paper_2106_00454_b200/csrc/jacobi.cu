@@ -37,7 +37,6 @@ __device__ long long wpcd_prof[8];
 
 constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), column pairs XOR-swizzled by the storage row
 constexpr int kQSlot = 16 * LDQ;
-constexpr int kFullEvery = 4;  // a full 16x16 pivot sweep every 4th step of the block tournament, cross-only sweeps between
 
 // A: XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
 __device__ __forceinline__ int swz(int r, int c) { return c ^ (((r & 6) << 1) ^ ((r & 1) << 3)); }
@@ -459,6 +458,7 @@ struct JacobiParams {
   size_t gstride;  // doubles per CTA
   const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
   int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
+  int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
 };
 
@@ -533,9 +533,9 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
       }
     }
     __syncwarp();
-    // full sweep of the pivot every kFullEvery-th step (every block then sits in a pivot at >= 1 full step per sweep,
+    // full sweep of the pivot every full_every-th step (every block then sits in a pivot at >= 1 full step per sweep,
     // so every pair is still met in every sweep); always for small matrices, where padding leaves few real pivots
-    const bool full = (tn % kFullEvery) == 0 || P.nb < 8;
+    const bool full = (tn % P.full_every) == 0 || P.nb < 8;
     rotated = inner_solve(A, Qn, I, J, P.tol, full, lane);
   }
   if (lane == 0) {
@@ -774,6 +774,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.gwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + g.tab_bytes);
   P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
+  // about four full pivot sweeps per sweep of the tournament (measured: fewer cost extra sweeps, more cost pivot time)
+  P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   const int grid = global_grid(h, g, batch);
   if (work_bytes < g.tab_bytes + (size_t)grid * g.gstride * 8) return WPCD_EWORK;
