@@ -548,10 +548,11 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 //       2: A (full), V in the global workspace, Q in shared memory
 //       3: as 2 with Q in the global workspace too (very large n)
 // The pivot scratch is always the slot's own Q array.
-// kThr: 512 threads (one CTA per SM), or 256 / 128 (two / four CTAs per SM) where shared memory allows and a step has
-// no more pivots than the CTA has warps: several matrices in flight per SM fill each other's pivot-chain bubbles.
+// kThr: 640 threads (one CTA per SM; 20 warps at 96 registers measured faster than 16 at 128 or 24 at 80), or 320 /
+// 160 (two / four CTAs per SM) where shared memory allows and a step has no more pivots than the CTA has warps:
+// several matrices in flight per SM fill each other's pivot-chain bubbles.
 template <int kMode, int kThr>
-__global__ void __launch_bounds__(kThr, 512 / kThr) k_jacobi(JacobiParams P) {
+__global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
   constexpr bool kHalf = (kMode == 1);
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -731,21 +732,21 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
-  g.threads = 512;
+  g.threads = 640;
   const size_t smem1 = misc + tabs + q + a_half;
-  if (g.nslots <= 4 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 128; g.smem = smem1; g.gstride = v / 8; }
-  else if (g.nslots <= 8 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 256; g.smem = smem1; g.gstride = v / 8; }
+  if (g.nslots <= 5 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 160; g.smem = smem1; g.gstride = v / 8; }
+  else if (g.nslots <= 10 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 320; g.smem = smem1; g.gstride = v / 8; }
   else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
   else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
   else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
   return g;
 }
 
-// CTAs of the workspace paths: as many as fit an SM (512 / threads: registers are 128 per thread), each with its own
+// CTAs of the workspace paths: as many as fit an SM (640 / threads: 96 registers per thread), each with its own
 // workspace.  All workspaces together must stay inside L2 (measured: a 100 MB working set already spills to HBM -- the
 // 126 MB L2 is split over two dies); the mode-1 sets are 25-50 MB.
 int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
-  const int grid = (512 / g.threads) * h->num_sms;
+  const int grid = (640 / g.threads) * h->num_sms;
   return batch < grid ? batch : grid;
 }
 
@@ -783,12 +784,12 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   int rc;
   switch (g.mode) {
     case 1:
-      rc = g.threads == 128   ? launch_mode<1, 128>(h, P, grid, g.smem, st)
-           : g.threads == 256 ? launch_mode<1, 256>(h, P, grid, g.smem, st)
-                              : launch_mode<1, 512>(h, P, grid, g.smem, st);
+      rc = g.threads == 160   ? launch_mode<1, 160>(h, P, grid, g.smem, st)
+           : g.threads == 320 ? launch_mode<1, 320>(h, P, grid, g.smem, st)
+                              : launch_mode<1, 640>(h, P, grid, g.smem, st);
       break;
-    case 2: rc = launch_mode<2, 512>(h, P, grid, g.smem, st); break;
-    default: rc = launch_mode<3, 512>(h, P, grid, g.smem, st); break;
+    case 2: rc = launch_mode<2, 640>(h, P, grid, g.smem, st); break;
+    default: rc = launch_mode<3, 640>(h, P, grid, g.smem, st); break;
   }
   if (rc) return rc;
   return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch");
