@@ -17,7 +17,7 @@
 //     __syncthreads per step.
 //   * A sweep = m-1 steps.  Converged when a whole sweep rotates nothing (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
 // n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
-// n <= 104 with 256 threads (n <= 56: 128) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
+// n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
 //
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
