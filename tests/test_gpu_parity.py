@@ -270,3 +270,27 @@ def test_energy_averaged_T_mode1(ctx, N, kind, lJ):
     for i in np.unique(bb[bb >= 0]):
         idx = np.where(bb == i)[0]
         assert np.all(Tg[idx] == Tg[idx[0]])
+
+
+def test_diag_is_run_to_run_deterministic(ctx):
+    """The pipelined kernel hands tiles to warps through a dynamic queue and overlaps the pivot solves of the next step
+    with the updates of the running one; every item touches disjoint data, so repeated runs must agree BIT FOR BIT.
+    (compute-sanitizer is closed on this pool; a data race would show up here as run-to-run differences.)"""
+    h, torch = ctx["h"], ctx["torch"]
+    for N, chans, S in ((100, [(0, 0)], 300), (100, [(1, 1)], 150), (24, [(0, 1)], 600), (150, [(1, 2)], 8)):
+        scales = inp.sample_scales(S, seed=3)
+        out = h.build_channels(inp.grid_edges(N), chans, scales=_to_dev(ctx, scales), S=S, V0=inp.MT_V0, mu=inp.MT_MU,
+                               scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+        H = out["H_cpl" if chans[0][0] else "H_unc"]
+        n = H.shape[-1]
+        Hb = H.reshape(-1, n, n)
+        ref = None
+        for rep in range(3):
+            W, C, info = h.diag_batched(Hb)
+            torch.cuda.synchronize()
+            cur = (W.clone(), C.clone(), info.clone())
+            if ref is None:
+                ref = cur
+            else:
+                assert torch.equal(cur[0], ref[0]) and torch.equal(cur[1], ref[1]) and torch.equal(cur[2], ref[2]), (N, chans, rep)
+        assert (ref[2] >= 1).all()
