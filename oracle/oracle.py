@@ -35,6 +35,7 @@ _edges = _sig("orc_swp_edges", None, [_i, _pd, _pd])
 _res = _sig("orc_resolvent_c", None, [_d, _d, _d, _pd])
 _onT = _sig("orc_onshell_T", None, [_i, _i, _pd, _pd, _pd, _pd, _pd, _i, _pd, _pi])
 _onTavg = _sig("orc_onshell_T_avg", None, [_i, _i, _pd, _pd, _pd, _pd, _pd, _i, _pd, _pi])
+_interp = _sig("orc_interp_phases", None, [_i, _i, _pd, _pd, _pd, _i, _pd])
 _resavg = _sig("orc_resolvent_avg_c", None, [C.c_double, C.c_double, C.c_double, C.c_double, _i, _pd])
 _ph = _sig("orc_phase_shifts", None, [_i, _i, _pd, _pi, _pd, _pd, _vp])
 _migrid = _sig("orc_mi_grid", None, [_i, _d, _pd, _pd])
@@ -132,6 +133,15 @@ def resolvent(E, lo, hi):
     o = np.empty(2)
     _res(E, lo, hi, o)
     return complex(o[0], o[1])
+
+
+def interp_phases(pedge, dmid, q):
+    """Eq. 42: phases at momenta q from the mid-point phases dmid [N] or [N][3] (degrees)."""
+    pedge = _f(pedge); dmid = _f(dmid); q = _f(q)
+    N = len(pedge) - 1; nc = 1 if dmid.ndim == 1 else dmid.shape[1]
+    out = np.empty((len(q), nc))
+    _interp(N, nc, pedge, dmid, q, len(q), out)
+    return out[:, 0] if nc == 1 else out
 
 
 def resolvent_avg(a, b, lo, hi, same_bin):

@@ -565,6 +565,58 @@ void orc_mi_solve(int kind, int coupled, int l_or_J, int nterms, const double* V
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-1, second half: linear interpolation of the phase shifts between the bin mid-points, Eq. 42.
+//   pedge[N+1]   momentum bin edges q_0..q_N (fm^-1); mid-points qbar_i = (q_i + q_{i+1})/2 (Eq. 43 with n = m/2)
+//   dmid[N][nc]  phase shifts at the mid-points in degrees, nc = 1 (delta) or 3 (delta_-, delta_+, eps_J)
+//   q[nq]        target momenta; out[nq][nc] in degrees, principal value (-90, 90]; q outside the grid: NaN
+// As printed: for q in bin i the straight line through (qbar_{i-1}, delta_{i-1}) and (qbar_i, delta_i) (so the upper
+// half of a bin is an extrapolation of that line); bin 0 uses the line of bins 0 and 1 (reading I1).  Before that the
+// mid-point phases are made continuous (reading I2): delta_i is shifted by the multiple of 180 degrees that brings it
+// within 90 degrees of delta_{i-1} (the principal value jumps by 180 at a bound-state transition), and
+// eps_J changes sign with every odd shift of delta_- or delta_+ (S_12 = i sin 2eps e^{i(delta_- + delta_+)}, Eq. A.5).
+static double wrap90(double d) {
+  double r = std::fmod(d + 90.0, 180.0);
+  if (r <= 0.0) r += 180.0;
+  return r - 90.0;  // in (-90, 90]
+}
+void orc_interp_phases(int N, int nc, const double* pedge, const double* dmid, const double* q, int nq, double* out) {
+  std::vector<double> u((size_t)N * nc);
+  std::vector<int> flips(N, 0);
+  for (int c = 0; c < (nc == 3 ? 2 : 1); ++c) {
+    double shift = 0.0;
+    for (int i = 0; i < N; ++i) {
+      double d = dmid[(size_t)i * nc + c] + shift;
+      if (i > 0) {
+        double prev = u[(size_t)(i - 1) * nc + c];
+        while (d - prev > 90.0) { d -= 180.0; shift -= 180.0; }
+        while (d - prev <= -90.0) { d += 180.0; shift += 180.0; }
+      }
+      u[(size_t)i * nc + c] = d;
+      flips[i] += (int)std::llround(shift / 180.0);
+    }
+  }
+  if (nc == 3)
+    for (int i = 0; i < N; ++i) u[(size_t)i * 3 + 2] = (flips[i] & 1) ? -dmid[(size_t)i * 3 + 2] : dmid[(size_t)i * 3 + 2];
+  for (int e = 0; e < nq; ++e) {
+    int ib = -1;
+    for (int i = 0; i < N; ++i)
+      if (q[e] >= pedge[i] && q[e] < pedge[i + 1]) { ib = i; break; }
+    for (int c = 0; c < nc; ++c) {
+      double r = std::nan("");
+      if (ib >= 0 && N >= 2) {
+        int i1 = ib > 0 ? ib : 1, i0 = i1 - 1;
+        double q0 = 0.5 * (pedge[i0] + pedge[i0 + 1]), q1 = 0.5 * (pedge[i1] + pedge[i1 + 1]);
+        double d0 = u[(size_t)i0 * nc + c], d1 = u[(size_t)i1 * nc + c];
+        double slope = (d1 - d0) / (q1 - q0);
+        r = slope * q[e] + (d0 - slope * q0);                     // Eq. 42 as printed
+        if (!(nc == 3 && c == 2)) r = wrap90(r);
+      }
+      out[(size_t)e * nc + c] = r;
+    }
+  }
+}
+
 // Whole chain for a batch of (sample, channel) solves, OpenMP over the batch (used only for timing the oracle as the
 // reported CPU baseline and by tests that need many solves).  Per solve b: H_b (n x n) and V_b are given
 // (assembled by orc_V_yukawa/orc_assemble_H), outputs W, C, T, delta.  Returns max sweeps (or -1).

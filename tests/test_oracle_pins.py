@@ -486,3 +486,63 @@ def test_wpcd_avg_yamaguchi_converges_monotonically():
         exact = np.array([0.5 * math.degrees(np.angle(_yamaguchi_S_exact(2 * E))) for E in Em[sel]])
         errs.append(_dist180(d, exact).max())
     assert errs[0] > errs[1] > errs[2] and errs[0] < 1.5 and errs[2] < 0.4, errs
+
+
+# ---------------------------------------------------------------- NEXT-1: mid-point interpolation (Eqs. 42-43)
+def test_interp_phases_lines_wraps_and_mixing_sign():
+    p = np.array([0.0, 0.5, 1.2, 2.0, 3.5, 5.0])
+    qm = 0.5 * (p[:-1] + p[1:])
+    q = np.array([0.05, 0.3, 0.9, 1.9, 2.0, 3.4, 4.99])
+    # (1) a straight line in q is reproduced exactly (interpolation and the printed extrapolation in the upper half bin)
+    assert np.allclose(o.interp_phases(p, 12.0 - 7.0 * qm, q), 12.0 - 7.0 * q, atol=1e-12)
+    assert np.isnan(o.interp_phases(p, qm, np.array([5.0, -0.1]))).all()           # outside the grid
+    # (2) Eq. 42 by hand for q in bin 2 (0-based): line through the mid-points of bins 1 and 2
+    d = np.array([3.0, -20.0, 35.0, 40.0, 10.0])
+    want = d[1] + (d[2] - d[1]) / (qm[2] - qm[1]) * (1.9 - qm[1])
+    assert abs(o.interp_phases(p, d, np.array([1.9]))[0] - want) < 1e-12
+    want0 = d[0] + (d[1] - d[0]) / (qm[1] - qm[0]) * (0.05 - qm[0])                 # bin 0 uses bins 0 and 1 (reading I1)
+    assert abs(o.interp_phases(p, d, np.array([0.05]))[0] - want0) < 1e-12
+    # (3) a 180-degree branch jump of the principal value is not interpolated across (reading I2):
+    true = 150.0 - 40.0 * qm                                                         # smooth, crosses +90 and -90... wrapped:
+    wrapped = (true + 90.0) % 180.0 - 90.0
+    got = o.interp_phases(p, wrapped, q)
+    exact = ((150.0 - 40.0 * q) + 90.0) % 180.0 - 90.0
+    assert np.allclose((got - exact + 90.0) % 180.0 - 90.0, 0.0, atol=1e-10)
+    assert np.all((got > -90.0) & (got <= 90.0))
+    # (4) coupled: eps_J flips sign with every odd 180-degree shift of delta_- or delta_+ (Eq. A.5)
+    dm = (80.0 + 30.0 * qm + 90.0) % 180.0 - 90.0                                    # delta_- wraps once along the grid
+    dp = 5.0 + 0.0 * qm
+    eps_true = 2.0 + 0.5 * qm
+    k = np.round((80.0 + 30.0 * qm - dm) / 180.0).astype(int)
+    k = k - k[0]                                                                     # shifts relative to the first bin
+    eps_given = np.where(k % 2 == 1, -eps_true, eps_true)
+    out = o.interp_phases(p, np.stack([dm, dp, eps_given], axis=1), q)
+    assert np.allclose(out[:, 2], eps_true[0] / eps_true[0] * (2.0 + 0.5 * q), atol=1e-10)
+    assert np.allclose(out[:, 1], 5.0, atol=1e-12)
+
+
+def test_interp_phases_yamaguchi_beats_the_steps():
+    """Fig. 5 / PAPER.md:385: mid-point interpolation of the energy-averaged phases is close to the exact result at ANY
+    energy, closer than the step-like bin values (whose error adds the half-bin variation of the phase)."""
+    lamA, lamB = inp.yamaguchi_lambda()
+    cE = inp.HBARC ** 2 / (2 * inp.MU)
+    tl = np.linspace(5.0, 350.0, 70)
+    q = np.sqrt(tl / 2 / cE)
+    exact = np.array([0.5 * math.degrees(np.angle(_yamaguchi_S_exact(t))) for t in tl])
+    errs = []
+    for N in (50, 100):
+        p = inp.grid_edges(N)
+        e0, dE, Ee = o.fwp(p)
+        V, G = o.V_yamaguchi(p, lamB, inp.YAMAGUCHI_BETA)
+        H, Vf = o.assemble_H(e0, V)
+        W, C, _ = o.jacobi(H)
+        qm = 0.5 * (p[:-1] + p[1:])
+        T, b = o.onshell_T(N, False, Ee, Vf, W, C, cE * qm ** 2, averaged=True)
+        dmid, _ = o.phase_shifts(False, T, b, dE)
+        Ts, bs = o.onshell_T(N, False, Ee, Vf, W, C, tl / 2, averaged=True)
+        dstep, _ = o.phase_shifts(False, Ts, bs, dE)
+        e_int = _dist180(o.interp_phases(p, dmid, q), exact).max()
+        e_step = _dist180(dstep, exact).max()
+        assert e_int < 0.75 * e_step, (N, e_int, e_step)
+        errs.append(e_int)
+    assert errs[1] < errs[0] < 1.5, errs
