@@ -143,6 +143,18 @@ int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_
 int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
                       const double* d_dE, double* d_delta, double* d_S, void* stream);
 
+/* Eq. 42, the second half of the paper's production variant (energy-averaged T per bin, then linear
+ * interpolation between the bin mid-points): phase shifts at arbitrary momenta from the mid-point values.
+ *   d_pedge     : [N+1] momentum bin edges, fm^-1 (device);  mid-points qbar_i = (p_i + p_{i+1})/2 (Eq. 43, n = m/2)
+ *   d_delta_mid : [batch][N] or [batch][N][3] phases at the mid-points, degrees -- e.g. wpcd_onshell_T(mode 1) and
+ *                 wpcd_phase_shifts evaluated at the N energies cE qbar_i^2
+ *   d_q         : [nq] target momenta, fm^-1;  d_out : [batch][nq] or [batch][nq][3], degrees, delta in (-90, 90]
+ * For q in bin i the line through the mid-points of bins i-1 and i, as printed (bin 0: bins 0 and 1); q outside the grid
+ * gives NaN.  The mid-point phases are first made continuous: delta_i is shifted by the multiple of 180 degrees that
+ * brings it within 90 degrees of delta_{i-1}, eps_J changes sign with every odd shift (readings I1-I2). */
+int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
+                       const double* d_q, int nq, double* d_out, void* stream);
+
 /* Test hooks (host only, no GPU needed): the block tournament that wpcd_diag_batched runs (csrc/jacobi_schedule.cuh).
  * m = number of players (8-wide blocks, even, >= 6; players >= nb are padding), a sweep has m-1 steps of m/2 slots.
  *   wpcd_jacobi_schedule      : blocks (I < J) of slot s at step t; J = -1 single block, I = J = -1 empty slot.

@@ -135,3 +135,11 @@ int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double
 }
 
 }  // extern "C"
+
+int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
+                       const double* d_q, int nq, double* d_out, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !d_pedge || !d_delta_mid || !d_q || !d_out || batch < 1 || N < 1 || nq < 1) return WPCD_EINVAL;
+  return wpcd_interp_launch(h, coupled ? 1 : 0, batch, N, d_pedge, d_delta_mid, d_q, nq, d_out,
+                            static_cast<cudaStream_t>(stream));
+}

@@ -325,6 +325,69 @@ __global__ void k_phase(int coupled, size_t total, int nE, const double* __restr
   }
 }
 
+// Eq. 42: phase shifts at arbitrary momenta from the values at the bin mid-points; one CTA per
+// batch element.  The mid-point phases are first made continuous (shifts by multiples of 180 degrees, eps_J changing
+// sign with every odd shift of delta_- or delta_+; readings I1-I2), sequentially along the grid by one
+// thread per phase, then every target momentum takes the straight line of Eq. 42 as printed.
+__global__ void __launch_bounds__(128) k_interp(int N, int nc, int nq, const double* __restrict__ pedge,
+                                                const double* __restrict__ dmid, const double* __restrict__ q,
+                                                double* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* u = reinterpret_cast<double*>(smem_raw);       // [N][nc] continuous mid-point phases
+  int* flips = reinterpret_cast<int*>(u + (size_t)N * nc);  // [2][N] accumulated 180-degree shifts of delta_-/delta_+
+  const double* d = dmid + (size_t)blockIdx.x * N * nc;
+  double* o = out + (size_t)blockIdx.x * nq * nc;
+  const int tid = threadIdx.x;
+  if (tid < (nc == 3 ? 2 : 1)) {
+    double shift = 0.0;
+    for (int i = 0; i < N; ++i) {
+      double x = d[(size_t)i * nc + tid] + shift;
+      if (i > 0) {
+        const double prev = u[(size_t)(i - 1) * nc + tid];
+        while (x - prev > 90.0) { x -= 180.0; shift -= 180.0; }
+        while (x - prev <= -90.0) { x += 180.0; shift += 180.0; }
+      }
+      u[(size_t)i * nc + tid] = x;
+      flips[tid * N + i] = (int)llrint(shift / 180.0);
+    }
+  }
+  __syncthreads();
+  if (nc == 3)
+    for (int i = tid; i < N; i += blockDim.x) {
+      const double e = d[(size_t)i * 3 + 2];
+      u[(size_t)i * 3 + 2] = ((flips[i] + flips[N + i]) & 1) ? -e : e;
+    }
+  __syncthreads();
+  for (int e = tid; e < nq; e += blockDim.x) {
+    const double qe = q[e];
+    int ib = -1;
+    if (qe >= pedge[0] && qe < pedge[N]) {
+      int lo = 0, hi = N;  // invariant pedge[lo] <= qe < pedge[hi]
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (qe >= pedge[mid]) lo = mid; else hi = mid;
+      }
+      ib = lo;
+    }
+    for (int c = 0; c < nc; ++c) {
+      double r = nan("");
+      if (ib >= 0 && N >= 2) {
+        const int i1 = ib > 0 ? ib : 1, i0 = i1 - 1;
+        const double q0 = 0.5 * (pedge[i0] + pedge[i0 + 1]), q1 = 0.5 * (pedge[i1] + pedge[i1 + 1]);
+        const double d0 = u[(size_t)i0 * nc + c], d1 = u[(size_t)i1 * nc + c];
+        const double slope = (d1 - d0) / (q1 - q0);
+        r = slope * qe + (d0 - slope * q0);
+        if (!(nc == 3 && c == 2)) {
+          r = fmod(r + 90.0, 180.0);
+          if (r <= 0.0) r += 180.0;
+          r -= 90.0;
+        }
+      }
+      o[(size_t)e * nc + c] = r;
+    }
+  }
+}
+
 int chunk_bins(int n, int nc, int max_smem) {
   int R = 16 / nc;  // at most 16 accumulator rows
   while (R > 1 && (size_t)(3 * n + 2 * R * nc * n) * 8 > (size_t)max_smem - 1024) R >>= 1;
@@ -361,4 +424,15 @@ int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const doubl
   size_t total = (size_t)batch * nE;
   k_phase<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(coupled, total, nE, d_T, d_bin, d_dE, d_delta, d_S);
   return wpcd_check_cuda(h, cudaGetLastError(), "phase_shifts launch");
+}
+
+int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
+                       const double* d_q, int nq, double* d_out, cudaStream_t st) {
+  const int nc = coupled ? 3 : 1;
+  const size_t smem = (size_t)N * nc * 8 + (size_t)2 * N * 4;
+  if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
+  int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_interp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "interp attr");
+  if (rc) return rc;
+  k_interp<<<batch, 128, smem, st>>>(N, nc, nq, d_pedge, d_delta_mid, d_q, d_out);
+  return wpcd_check_cuda(h, cudaGetLastError(), "interp_phases launch");
 }

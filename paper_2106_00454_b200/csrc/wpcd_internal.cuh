@@ -33,3 +33,5 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
                         int mode, double* d_T, int* d_bin, void* d_work, size_t work_bytes, cudaStream_t st);
 int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
                       const double* d_dE, double* d_delta, double* d_S, cudaStream_t st);
+int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
+                       const double* d_q, int nq, double* d_out, cudaStream_t st);

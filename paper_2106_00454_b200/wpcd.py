@@ -56,6 +56,8 @@ _lib.wpcd_onshell_T.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _
 _lib.wpcd_onshell_T.restype = _i
 _lib.wpcd_phase_shifts.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.wpcd_phase_shifts.restype = _i
+_lib.wpcd_interp_phases.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _i, _vp, _vp]
+_lib.wpcd_interp_phases.restype = _i
 
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
@@ -177,6 +179,17 @@ class Handle:
                                  _ptr(Ecm), nE, int(mode), _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream))
         self._check(rc, "wpcd_onshell_T")
         return T, bins
+
+    # ------------------------------------------------------------------ wpcd_interp_phases
+    def interp_phases(self, coupled, pedge, delta_mid, q, stream=None, out=None):
+        """Eq. 42: delta_mid [batch][N] (or [batch][N][3]) at the bin mid-points -> phases at momenta q [nq]."""
+        batch, N = delta_mid.shape[0], delta_mid.shape[1]; nq = q.shape[0]; dev = delta_mid.device
+        shape = (batch, nq, 3) if coupled else (batch, nq)
+        out = torch.empty(shape, dtype=torch.float64, device=dev) if out is None else out
+        rc = _lib.wpcd_interp_phases(self._h, int(coupled), batch, N, _ptr(pedge), _ptr(delta_mid), _ptr(q), nq, _ptr(out),
+                                     _stream(stream))
+        self._check(rc, "wpcd_interp_phases")
+        return out
 
     # ------------------------------------------------------------------ wpcd_phase_shifts
     def phase_shifts(self, coupled, T, bins, dE, want_S=True, stream=None, delta=None, S=None):

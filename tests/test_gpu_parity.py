@@ -294,3 +294,49 @@ def test_diag_is_run_to_run_deterministic(ctx):
             else:
                 assert torch.equal(cur[0], ref[0]) and torch.equal(cur[1], ref[1]) and torch.equal(cur[2], ref[2]), (N, chans, rep)
         assert (ref[2] >= 1).all()
+
+
+@pytest.mark.parametrize("N,kind,lJ", [(50, 0, 0), (100, 1, 1), (40, 0, 2)])
+def test_production_variant_averaged_T_then_interpolation(ctx, N, kind, lJ):
+    """The paper's production chain: energy-averaged T at the bin mid-points, phases, then
+    Eq. 42 at arbitrary energies -- GPU (wpcd_onshell_T mode 1 -> wpcd_phase_shifts -> wpcd_interp_phases) against the
+    oracle's chain; plus synthetic mid-point phases with branch jumps fed to both interpolators."""
+    from oracle import oracle as o
+    h, torch = ctx["h"], ctx["torch"]
+    p = inp.grid_edges(N)
+    cE = inp.HBARC ** 2 / (2 * inp.MU)
+    qm = 0.5 * (p[:-1] + p[1:])
+    tl, Ecm = inp.energies(90)
+    q = np.sqrt(Ecm / cE)
+    out = h.build_channels(p, [(kind, lJ)], S=1, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+    Hd = out["H_cpl" if kind else "H_unc"]
+    n = Hd.shape[-1]
+    Hb = Hd.reshape(-1, n, n)
+    W, C, info = h.diag_batched(Hb)
+    T, bins = h.onshell_T(N, kind, out["e0"], out["Eedge"], Hb, W, C, _to_dev(ctx, cE * qm ** 2), mode=1)
+    dmid, _ = h.phase_shifts(kind, T, bins, out["dE"])
+    got = h.interp_phases(kind, _to_dev(ctx, p), dmid, _to_dev(ctx, q))
+    torch.cuda.synchronize()
+    ch = hp.oracle_channel(N, kind, lJ)
+    Wr, Cr, _ = o.jacobi(ch["H"])
+    Tr, br = o.onshell_T(N, bool(kind), ch["Eedge"], ch["V"], Wr, Cr, cE * qm ** 2, averaged=True)
+    dr, _ = o.phase_shifts(bool(kind), Tr, br, ch["dE"])
+    assert np.array_equal(bins.cpu().numpy(), br) and np.array_equal(br, np.arange(N))   # mid-point i lies in bin i
+    # same mid-point inputs to both interpolators: agreement to rounding
+    same = o.interp_phases(p, dmid.cpu().numpy()[0], q)
+    g = got.cpu().numpy()[0]
+    assert np.allclose(g, same, atol=1e-10, rtol=0, equal_nan=True)
+    # whole chain against the oracle's chain, where the mid-point phases themselves agree to 1e-8 (top bins with no
+    # i-th pseudostate give T = 0 on both sides)
+    want = o.interp_phases(p, dr, q)
+    d = hp.dist180(g, want)
+    if kind:
+        d = d[:, :2]
+    assert np.nanmax(d) <= 5 * hp.TOL_PHASE_DEG, np.nanmax(d)
+    # synthetic mid-point phases with principal-value jumps (and, coupled, mixing-angle sign flips)
+    rng = np.random.default_rng(N)
+    smooth = 150.0 * np.cos(3.0 * qm / qm[-1]) + 20.0
+    wrapped = (smooth + 90.0) % 180.0 - 90.0
+    dm = np.stack([wrapped, (0.5 * smooth + 90.0) % 180.0 - 90.0, rng.uniform(-5, 5, N)], axis=1) if kind else wrapped
+    g2 = h.interp_phases(kind, _to_dev(ctx, p), _to_dev(ctx, dm[None]), _to_dev(ctx, q)).cpu().numpy()[0]
+    assert np.allclose(g2, o.interp_phases(p, dm, q), atol=1e-10, rtol=0, equal_nan=True)
