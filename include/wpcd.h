@@ -110,9 +110,14 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
  *   d_info : [batch] sweeps used (>= 1), or -1 if not converged in max_sweeps
  *   tol    : a pivot is rotated iff |a_pq| > tol sqrt(|a_pp a_qq|); convergence = a full sweep without rotation.
  *            tol <= 0 selects the default 2^-52.
+ *   h_rows : optional HOST array of n_ranges (<= 4) half-open row ranges [lo, hi) of C that the caller needs (NULL,
+ *            0 = all rows).  C <- C J acts on the rows independently, so rows outside the ranges (rounded out to
+ *            multiples of 8) are not updated and are returned as ZEROS; the eigenvalues and the wanted rows are
+ *            unaffected.  The on-shell T of the n <= 200 path only reads the rows of the on-shell bins.
  *   d_work : wpcd_diag_workspace_bytes(n, batch) bytes (never 0: the schedule tables live there) */
 int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
-                      double tol, int max_sweeps, void* d_work, size_t work_bytes, void* stream);
+                      double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
+                      void* stream);
 
 /* Steps (iii)-(v).  For every matrix b and energy e: FWP bin i(e) with Eedge_i <= E_e < Eedge_{i+1}, then
  *   uncoupled: T_ii(E) = V_ii + sum_b (VC)_ib^2/(E - eps_b) + sum_k (VC)_ik^2 g_k(E)
@@ -142,6 +147,11 @@ int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_
  *   d_S     : optional (may be NULL) S-matrix, same layout as d_T */
 int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double* d_T, const int* d_bin,
                       const double* d_dE, double* d_delta, double* d_S, void* stream);
+
+/* Host helper (no GPU work): the row ranges of C that wpcd_onshell_T will read for the c.m. energies h_Ecm [nE] (HOST
+ * array) on this grid, to be handed to wpcd_diag_batched as h_rows.  h_rows must hold 8 ints; *n_ranges comes back as
+ * 0 when all rows are needed (the direct-product path of large n). */
+int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, int nE, int* h_rows, int* n_ranges);
 
 /* Eq. 42, the second half of the paper's production variant (energy-averaged T per bin, then linear
  * interpolation between the bin mid-points): phase shifts at arbitrary momenta from the mid-point values.

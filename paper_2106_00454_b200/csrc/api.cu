@@ -103,14 +103,18 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
 }
 
 int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
-                      double tol, int max_sweeps, void* d_work, size_t work_bytes, void* stream) {
+                      double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
+                      void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !d_A || !d_W || !d_C || !d_info || batch < 1 || max_sweeps < 1) return WPCD_EINVAL;
+  if (n_ranges < 0 || n_ranges > 4 || (n_ranges > 0 && !h_rows)) return WPCD_EINVAL;
+  for (int r = 0; r < n_ranges; ++r)
+    if (h_rows[2 * r] < 0 || h_rows[2 * r + 1] > n || h_rows[2 * r] >= h_rows[2 * r + 1]) return WPCD_EINVAL;
   if (n < 2 || n > 4096) return WPCD_ESIZE;
   if (!aligned16(d_A) || !aligned16(d_C) || !aligned16(d_work)) return WPCD_EINVAL;
   size_t need = wpcd_jacobi_workspace(h, n, batch);
   if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
-  return wpcd_jacobi_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, d_work, work_bytes,
+  return wpcd_jacobi_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, h_rows, n_ranges, d_work, work_bytes,
                             static_cast<cudaStream_t>(stream));
 }
 
@@ -142,4 +146,9 @@ int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double
   if (!h || !d_pedge || !d_delta_mid || !d_q || !d_out || batch < 1 || N < 1 || nq < 1) return WPCD_EINVAL;
   return wpcd_interp_launch(h, coupled ? 1 : 0, batch, N, d_pedge, d_delta_mid, d_q, nq, d_out,
                             static_cast<cudaStream_t>(stream));
+}
+
+int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, int nE, int* h_rows, int* n_ranges) {
+  if (!grid || !grid->h_edges || grid->N < 1 || !h_Ecm || nE < 1 || !h_rows || !n_ranges) return WPCD_EINVAL;
+  return wpcd_onshell_rows_host(grid->N, coupled ? 1 : 0, grid->h_edges, grid->hbarc, grid->mu, h_Ecm, nE, h_rows, n_ranges);
 }

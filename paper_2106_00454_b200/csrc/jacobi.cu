@@ -106,6 +106,7 @@ struct Smem {
   int* rot;      // [2][nslots] slot rotated something
   int* src;      // [np]
   int* ctr;      // [0..1] work queues (step parity), [2..3] rotations per sweep (sweep parity)
+  int* act;      // [nb] active row blocks of V (those that hold wanted rows of C)
   const int* tab; // slot and feed tables [2][m-1][nslots]: shared-memory copy (modes 0, 1) or k_schedule's global ones
 };
 
@@ -360,15 +361,15 @@ __device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* 
 }
 
 // V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
-// V[rows of row-blocks rb0, rb0+1][P] <- V[..][P] Q for exactly two row blocks: all four 16-byte loads are in flight
+// V[rows of row-blocks rbA, rbB][P] <- V[..][P] Q for exactly two row blocks: all four 16-byte loads are in flight
 // before the first product (V lives in global memory in every mode: L2 latency).
 template <int nbk>
 __device__ __forceinline__ void apply_V_2(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                          int rb0, int lane) {
+                                          int rbA, int rbB, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int cb[2] = {I, J};
-  double* v0 = V + (size_t)(8 * rb0 + g) * ld + 2 * t;
-  double* v1 = v0 + (size_t)8 * ld;
+  double* v0 = V + (size_t)(8 * rbA + g) * ld + 2 * t;
+  double* v1 = V + (size_t)(8 * rbB + g) * ld + 2 * t;
   double2 f0[2], f1[2];
 #pragma unroll
   for (int c = 0; c < nbk; ++c) {
@@ -437,14 +438,15 @@ __device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const 
   }
 }
 
+// rbB < 0: a single row block
 __device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                        int rb0, int rb1, int lane) {
-  if (rb1 - rb0 == 2) {
-    if (J >= 0) apply_V_2<2>(V, ld, Q, I, J, rb0, lane);
-    else apply_V_2<1>(V, ld, Q, I, J, rb0, lane);
+                                        int rbA, int rbB, int lane) {
+  if (rbB >= 0) {
+    if (J >= 0) apply_V_2<2>(V, ld, Q, I, J, rbA, rbB, lane);
+    else apply_V_2<1>(V, ld, Q, I, J, rbA, rbB, lane);
   } else {
-    if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rb0, rb1, lane);
-    else apply_V_n<1>(V, ld, Q, I, J, rb0, rb1, lane);
+    if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rbA, rbA + 1, lane);
+    else apply_V_n<1>(V, ld, Q, I, J, rbA, rbA + 1, lane);
   }
 }
 
@@ -458,6 +460,7 @@ struct JacobiParams {
   size_t gstride;  // doubles per CTA
   const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
   int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
+  int nranges, row_lo[4], row_hi[4];  // rows of C that are wanted (nranges = 0: all); the others are returned as zeros
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
 };
@@ -576,6 +579,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
     sm.rot = ip; ip += 2 * nslots;
     sm.src = ip; ip += np;
     sm.ctr = ip; ip += 4;
+    sm.act = ip; ip += 2 * nb;  // list of active row blocks, then a flag per row block
     if (kMode == 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
       for (int e = tid; e < 2 * (m - 1) * nslots; e += kThreads) ip[e] = P.tab[e];
       sm.tab = ip;
@@ -588,8 +592,21 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
   const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
   const AView<kHalf> Av{sm.A, ld, nb};
+  if (tid == 0) {  // row blocks of V that hold wanted rows of C (all of them unless row ranges were given)
+    int na = 0;
+    for (int rb = 0; rb < nb; ++rb) {
+      bool want = P.nranges == 0;
+      for (int r = 0; r < P.nranges; ++r) want |= (8 * rb < P.row_hi[r]) && (8 * rb + 8 > P.row_lo[r]);
+      if (want) sm.act[na++] = rb;
+      sm.act[nb + rb] = want ? 1 : 0;
+    }
+    sm.ctr[0] = na;
+  }
+  __syncthreads();
+  const int nact = sm.ctr[0];
+  __syncthreads();
   const int ntiles = nslots * (nslots - 1) / 2;
-  const int nvgrp = (nb + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
+  const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
   const int nitems = ntiles + nslots * nvgrp;
   const float rnvgrp = 1.0f / (float)nvgrp;
 
@@ -663,9 +680,8 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
             if (!rot[s]) continue;
             int I, J;
             decode_slot(tab_slot[s], I, J);
-            int rb0 = grp * kVRowBlocksPerItem, rb1 = rb0 + kVRowBlocksPerItem;
-            if (rb1 > nb) rb1 = nb;
-            apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rb0, rb1, lane);
+            const int rbA = sm.act[2 * grp], rbB = 2 * grp + 1 < nact ? sm.act[2 * grp + 1] : -1;
+            apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rbA, rbB, lane);
           }
         }
 #ifdef WPCD_PROFILE
@@ -701,7 +717,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
     for (int e = tid; e < n * n; e += kThreads) {
       int i = e / n, k = e - i * n;
       int c = sm.src[k];
-      Co[e] = sm.V[(size_t)i * ldv + c];
+      Co[e] = sm.act[nb + (i >> 3)] ? sm.V[(size_t)i * ldv + c] : 0.0;
     }
     if (tid == 0) P.info[mat] = converged ? sweeps : -1;
   }
@@ -727,7 +743,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
   g.tab_bytes = (((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255;
-  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4) * 4 + 64;
+  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
@@ -766,7 +782,8 @@ size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
 }
 
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
-                       double tol, int max_sweeps, void* d_work, size_t work_bytes, cudaStream_t st) {
+                       double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
+                       cudaStream_t st) {
   Geometry g = geometry(h, n);
   if (g.smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   JacobiParams P;
@@ -775,6 +792,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.gwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + g.tab_bytes);
   P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
+  P.nranges = n_ranges;
+  for (int r = 0; r < 4; ++r) { P.row_lo[r] = r < n_ranges ? h_rows[2 * r] : 0; P.row_hi[r] = r < n_ranges ? h_rows[2 * r + 1] : 0; }
   // about four full pivot sweeps per sweep of the tournament (measured: fewer cost extra sweeps, more cost pivot time)
   P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;

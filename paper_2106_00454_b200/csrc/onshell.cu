@@ -436,3 +436,29 @@ int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const doubl
   k_interp<<<batch, 128, smem, st>>>(N, nc, nq, d_pedge, d_delta_mid, d_q, d_out);
   return wpcd_check_cuda(h, cudaGetLastError(), "interp_phases launch");
 }
+
+// Rows of C that wpcd_onshell_T will read for these energies (host arithmetic, same bin rule as k_bins, widened by one
+// bin on either side against rounding): none needed beyond the on-shell bins on the identity path, all rows on the
+// direct path (n_ranges = 0).
+int wpcd_onshell_rows_host(int N, int coupled, const double* h_edges, double hbarc, double mu, const double* h_Ecm, int nE,
+                           int* h_rows, int* n_ranges) {
+  const int n = coupled ? 2 * N : N;
+  *n_ranges = 0;
+  if (n > kI1MaxN) return WPCD_OK;
+  const double cE = hbarc * hbarc / (2.0 * mu);
+  int bmin = N, bmax = -1;
+  for (int e = 0; e < nE; ++e)
+    for (int i = 0; i < N; ++i)
+      if (h_Ecm[e] >= cE * h_edges[i] * h_edges[i] && h_Ecm[e] < cE * h_edges[i + 1] * h_edges[i + 1]) {
+        if (i < bmin) bmin = i;
+        if (i > bmax) bmax = i;
+        break;
+      }
+  if (bmax < 0) { bmin = 0; bmax = 0; }  // no energy on the grid: any row will do
+  bmin = bmin > 0 ? bmin - 1 : 0;
+  bmax = bmax < N - 1 ? bmax + 1 : N - 1;
+  h_rows[0] = bmin; h_rows[1] = bmax + 1;
+  *n_ranges = 1;
+  if (coupled) { h_rows[2] = N + bmin; h_rows[3] = N + bmax + 1; *n_ranges = 2; }
+  return WPCD_OK;
+}

@@ -20,7 +20,8 @@ int wpcd_check_cuda(WpcdHandle* h, cudaError_t e, const char* where);
 // jacobi.cu
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch);
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
-                       double tol, int max_sweeps, void* d_work, size_t work_bytes, cudaStream_t st);
+                       double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
+                       cudaStream_t st);
 // assembly.cu
 size_t wpcd_build_workspace(int N, int n_chan);
 int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
@@ -35,3 +36,5 @@ int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const doubl
                       const double* d_dE, double* d_delta, double* d_S, cudaStream_t st);
 int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
                        const double* d_q, int nq, double* d_out, cudaStream_t st);
+int wpcd_onshell_rows_host(int N, int coupled, const double* h_edges, double hbarc, double mu, const double* h_Ecm, int nE,
+                           int* h_rows, int* n_ranges);

@@ -15,7 +15,8 @@ class Pipeline:
 
     KERNELS_PER_STEP_FIXED = 2  # k_grid, k_basis
 
-    def __init__(self, edges, channels, Ecm, S, potential, n_scale_cols=3, device=0, max_sweeps=30, tol=0.0):
+    def __init__(self, edges, channels, Ecm, S, potential, n_scale_cols=3, device=0, max_sweeps=30, tol=0.0,
+                 onshell_rows_only=True):
         self.h = wpcd.Handle(device)
         self.dev = self.h.device
         self.edges = np.asarray(edges, dtype=np.float64)
@@ -28,6 +29,10 @@ class Pipeline:
         self.n_cpl = len(self.channels) - self.n_unc
         N, f64 = self.N, torch.float64
         self.nE = len(Ecm)
+        # rows of C the on-shell kernel will read (library decides; None = all): C <- C J is row-independent, so the
+        # eigenvector update can skip the rest (wpcd_diag_batched h_rows)
+        self.rows = {k: (self.h.onshell_rows(self.edges, k, np.asarray(Ecm, dtype=np.float64)) if onshell_rows_only else None)
+                     for k in (0, 1)}
         self.Ecm = torch.as_tensor(np.ascontiguousarray(Ecm, dtype=np.float64), device=self.dev)
         self.scales = torch.ones((self.S, n_scale_cols), dtype=f64, device=self.dev)
         self.geo = dict(e0=torch.empty(N, dtype=f64, device=self.dev), dE=torch.empty(N, dtype=f64, device=self.dev),
@@ -77,7 +82,8 @@ class Pipeline:
         for kind, b in self.kind.items():
             tag = "cpl" if kind else "unc"
             rec("diag_" + tag, 0)
-            self.h.diag_batched(b["H"], tol=self.tol, max_sweeps=self.max_sweeps, W=b["W"], Cm=b["C"], info=b["info"], work=b["work"])
+            self.h.diag_batched(b["H"], tol=self.tol, max_sweeps=self.max_sweeps, W=b["W"], Cm=b["C"], info=b["info"], work=b["work"],
+                                rows=self.rows[kind])
             rec("diag_" + tag, 1)
             rec("onshell_" + tag, 0)
             self.h.onshell_T(self.N, kind, self.geo["e0"], self.geo["Eedge"], b["H"], b["W"], b["C"], self.Ecm,

@@ -50,7 +50,7 @@ _lib.wpcd_onshell_workspace_bytes.argtypes = [_vp, _i, _i, _i, _i]; _lib.wpcd_on
 _lib.wpcd_build_channels.argtypes = [_vp, C.POINTER(Grid), C.POINTER(Potential), C.POINTER(Channel), _i, _vp, _i, _i,
                                      _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
 _lib.wpcd_build_channels.restype = _i
-_lib.wpcd_diag_batched.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _d, _i, _vp, _sz, _vp]
+_lib.wpcd_diag_batched.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _d, _i, C.POINTER(_i), _i, _vp, _sz, _vp]
 _lib.wpcd_diag_batched.restype = _i
 _lib.wpcd_onshell_T.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp, _vp, _vp, _sz, _vp]
 _lib.wpcd_onshell_T.restype = _i
@@ -58,6 +58,8 @@ _lib.wpcd_phase_shifts.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp
 _lib.wpcd_phase_shifts.restype = _i
 _lib.wpcd_interp_phases.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _i, _vp, _vp]
 _lib.wpcd_interp_phases.restype = _i
+_lib.wpcd_onshell_rows.argtypes = [C.POINTER(Grid), _i, C.POINTER(_d), _i, C.POINTER(_i), C.POINTER(_i)]
+_lib.wpcd_onshell_rows.restype = _i
 
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
@@ -150,8 +152,9 @@ class Handle:
     def diag_workspace_bytes(self, n, batch):
         return _lib.wpcd_diag_workspace_bytes(self._h, n, batch)
 
-    def diag_batched(self, A, tol=0.0, max_sweeps=30, stream=None, W=None, Cm=None, info=None, work=None):
-        """A: device tensor [batch][n][n] (read only).  Returns (W [batch][n] ascending, C [batch][n][n], info)."""
+    def diag_batched(self, A, tol=0.0, max_sweeps=30, stream=None, W=None, Cm=None, info=None, work=None, rows=None):
+        """A: device tensor [batch][n][n] (read only).  Returns (W [batch][n] ascending, C [batch][n][n], info).
+        rows: optional list of up to 4 (lo, hi) row ranges of C that are needed (the other rows come back as zeros)."""
         batch, n = A.shape[0], A.shape[-1]
         dev = A.device
         W = torch.empty((batch, n), dtype=torch.float64, device=dev) if W is None else W
@@ -160,8 +163,10 @@ class Handle:
         wb = _lib.wpcd_diag_workspace_bytes(self._h, n, batch)
         if work is None or work.numel() < wb:
             work = self._work(wb)
+        nr = 0 if rows is None else len(rows)
+        h_rows = (_i * (2 * nr))(*[int(x) for r in rows for x in r]) if nr else None
         rc = _lib.wpcd_diag_batched(self._h, n, batch, _ptr(A), _ptr(W), _ptr(Cm), _ptr(info), float(tol), int(max_sweeps),
-                                    _ptr(work), work.numel(), _stream(stream))
+                                    h_rows, nr, _ptr(work), work.numel(), _stream(stream))
         self._check(rc, "wpcd_diag_batched")
         return W, Cm, info
 
@@ -179,6 +184,17 @@ class Handle:
                                  _ptr(Ecm), nE, int(mode), _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream))
         self._check(rc, "wpcd_onshell_T")
         return T, bins
+
+    # ------------------------------------------------------------------ wpcd_onshell_rows
+    def onshell_rows(self, edges, coupled, Ecm, hbarc=197.327, mu=469.46):
+        """Row ranges of C that onshell_T will read for the (host) energies Ecm; None = all rows."""
+        import numpy as np
+        e = np.ascontiguousarray(edges, dtype=np.float64); E = np.ascontiguousarray(Ecm, dtype=np.float64)
+        g = Grid(len(e) - 1, e.ctypes.data_as(C.POINTER(_d)), hbarc, mu, 8)
+        rows = (_i * 8)(); nr = _i(0)
+        self._check(_lib.wpcd_onshell_rows(C.byref(g), int(coupled), E.ctypes.data_as(C.POINTER(_d)), len(E), rows, C.byref(nr)),
+                    "wpcd_onshell_rows")
+        return [(rows[2 * r], rows[2 * r + 1]) for r in range(nr.value)] or None
 
     # ------------------------------------------------------------------ wpcd_interp_phases
     def interp_phases(self, coupled, pedge, delta_mid, q, stream=None, out=None):

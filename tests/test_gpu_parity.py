@@ -224,11 +224,11 @@ def test_abi_argument_errors(ctx):
     wp = ctx["wpcd"]
     lib = wp._lib
     h = ctx["h"]._h
-    assert lib.wpcd_diag_batched(h, 1, 1, None, None, None, None, 0.0, 10, None, 0, None) == -1      # NULL pointers
+    assert lib.wpcd_diag_batched(h, 1, 1, None, None, None, None, 0.0, 10, None, 0, None, 0, None) == -1      # NULL pointers
     t = ctx["torch"].zeros(16, dtype=ctx["torch"].float64, device=ctx["dev"])
     ti = ctx["torch"].zeros(4, dtype=ctx["torch"].int32, device=ctx["dev"])
-    assert lib.wpcd_diag_batched(h, 1, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None) == -2
-    assert lib.wpcd_diag_batched(h, 200, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None) == -3
+    assert lib.wpcd_diag_batched(h, 1, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None, 0, None) == -2
+    assert lib.wpcd_diag_batched(h, 200, 1, t.data_ptr(), t.data_ptr(), t.data_ptr(), ti.data_ptr(), 0.0, 10, None, 0, None, 0, None) == -3
     edges = (C.c_double * 3)(0.0, 2.0, 1.0)     # not increasing
     g = wp.Grid(2, edges, 197.327, 469.46, 8)
     assert lib.wpcd_build_channels(h, C.byref(g), None, None, 1, None, 1, 0, None, None, None, None, None, None, 0, None) == -1
@@ -340,3 +340,43 @@ def test_production_variant_averaged_T_then_interpolation(ctx, N, kind, lJ):
     dm = np.stack([wrapped, (0.5 * smooth + 90.0) % 180.0 - 90.0, rng.uniform(-5, 5, N)], axis=1) if kind else wrapped
     g2 = h.interp_phases(kind, _to_dev(ctx, p), _to_dev(ctx, dm[None]), _to_dev(ctx, q)).cpu().numpy()[0]
     assert np.allclose(g2, o.interp_phases(p, dm, q), atol=1e-10, rtol=0, equal_nan=True)
+
+
+def test_diag_row_ranges_and_pipeline_rows(ctx):
+    """wpcd_diag_batched with h_rows: same eigenvalues, the wanted rows of C bit-identical to the full run, the other
+    rows zero; and the pipeline (which asks wpcd_onshell_rows for the rows) gives the same phases either way."""
+    from paper_2106_00454_b200.pipeline import Pipeline
+    h, torch = ctx["h"], ctx["torch"]
+    N = 60
+    out = h.build_channels(inp.grid_edges(N), [(1, 1)], S=3, scales=_to_dev(ctx, inp.sample_scales(3, seed=5)), V0=inp.MT_V0,
+                           mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    Hb = out["H_cpl"].reshape(-1, 2 * N, 2 * N)
+    W0, C0, i0 = h.diag_batched(Hb)
+    rows = [(5, 41), (N + 5, N + 41)]
+    W1, C1, i1 = h.diag_batched(Hb, rows=rows)
+    torch.cuda.synchronize()
+    assert torch.equal(W0, W1) and torch.equal(i0, i1)
+    keep = np.zeros(2 * N, dtype=bool)
+    for lo, hi in rows:
+        keep[(lo // 8) * 8:min(-(-hi // 8) * 8, 2 * N)] = True
+    C0n, C1n = C0.cpu().numpy(), C1.cpu().numpy()
+    assert np.array_equal(C1n[:, keep, :], C0n[:, keep, :]) and not C1n[:, ~keep, :].any() and (~keep).any()
+    # argument errors
+    with pytest.raises(Exception):
+        h.diag_batched(Hb, rows=[(10, 5)])
+    with pytest.raises(Exception):
+        h.diag_batched(Hb, rows=[(0, 2 * N + 1)])
+    # library-chosen rows: inside the grid for n <= 200, all rows beyond
+    tl, Ecm = inp.energies(60)
+    r = h.onshell_rows(inp.grid_edges(100), 1, Ecm)
+    assert r is not None and len(r) == 2 and r[0][0] <= 6 and r[0][1] >= 72 and r[1] == (100 + r[0][0], 100 + r[0][1])
+    assert h.onshell_rows(inp.grid_edges(150), 1, Ecm) is None and h.onshell_rows(inp.grid_edges(150), 0, Ecm) is not None
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    sc = inp.sample_scales(4, seed=2)
+    res = []
+    for flag in (True, False):
+        pipe = Pipeline(inp.grid_edges(64), [(0, 0), (1, 1)], Ecm, 4, pot, device=0, onshell_rows_only=flag)
+        d, info = pipe.solve_host(sc)
+        res.append({k: v.clone() for k, v in d.items()})
+    for k in res[0]:
+        assert torch.equal(res[0][k], res[1][k])
