@@ -42,6 +42,10 @@ _migrid = _sig("orc_mi_grid", None, [_i, _d, _pd, _pd])
 _mi = _sig("orc_mi_solve", None, [_i, _i, _i, _i, _pd, _pd, _d, _d, _d, _d, _d, _d, _i, _d, _pd, _pd])
 _batch = _sig("orc_solve_batch", _i, [_i, _i, _i, _pd, _pd, _pd, _pd, _pd, _i, _d, _i, _pd, _pd, _pd, _pi, _pd, _vp, _vp])
 _nthr = _sig("orc_num_threads", _i, [])
+_cg = _sig("orc_clebsch_gordan", _d, [_i, _i, _i, _i, _i, _i])
+_ylm = _sig("orc_sph_harm", _d, [_i, _i, _d])
+_Mspin = _sig("orc_spin_scattering_M", None, [_i, _pi, _pi, _pi, _pi, _pd, _d, _d, _pd])
+_sigtot = _sig("orc_sigma_tot", _d, [_i, _pi, _pi, _pi, _pi, _pd, _d])
 
 HBARC = 197.327
 MU = 469.46
@@ -201,3 +205,50 @@ def solve_batch(N, coupled, Eedge, dE, H, V, Ecm, tol=1e-15, max_sweeps=60):
     if not coupled:
         Tc = Tc[:, :, 0, 0]; Sc = Sc[:, :, 0, 0]
     return dict(W=W, C=Cm, T=Tc, S=Sc, bin=b, delta=delta, sweeps=sw, worst=r)
+
+
+def clebsch_gordan(j1, m1, j2, m2, J, M):
+    return float(_cg(j1, m1, j2, m2, J, M))
+
+
+def sph_harm(l, m, theta):
+    return float(_ylm(l, m, float(theta)))
+
+
+def _pw_arrays(pw):
+    """pw: list of (s, J, l', l, S_{l'l}) -> int32 arrays and [npw][2] doubles."""
+    i32 = lambda k: np.ascontiguousarray([w[k] for w in pw], dtype=np.int32)
+    Sv = np.empty((len(pw), 2))
+    Sv[:, 0] = [complex(w[4]).real for w in pw]; Sv[:, 1] = [complex(w[4]).imag for w in pw]
+    return len(pw), i32(0), i32(1), i32(2), i32(3), Sv
+
+
+def spin_scattering_M(pw, p, theta):
+    """Eq. A.2: dict {(s, m_s, m_s'): M} for the partial waves pw = [(s, J, l', l, S_{l'l}), ...]."""
+    n, s, J, lp, l, Sv = _pw_arrays(pw)
+    M = np.empty((2, 3, 3, 2))
+    _Mspin(n, s, J, lp, l, Sv, float(p), float(theta), M)
+    Mc = M[..., 0] + 1j * M[..., 1]
+    return {(ss, ms, msp): Mc[ss, ms + 1, msp + 1] for ss in (0, 1) for ms in range(-ss, ss + 1) for msp in range(-ss, ss + 1)}
+
+
+def sigma_tot(pw, p):
+    """Eqs. A.2, A.9, A.11: total np cross section in mb at c.m. momentum p (fm^-1)."""
+    n, s, J, lp, l, Sv = _pw_arrays(pw)
+    return float(_sigtot(n, s, J, lp, l, Sv, float(p)))
+
+
+def partial_waves(channels, sJ, S_unc, S_cpl):
+    """Partial-wave list for sigma_tot from channel S-matrices at ONE energy (index bookkeeping only).
+    channels: [(coupled, lJ)] in list order; sJ: (s, J) of every channel (e.g. 3P0: l = 1, s = 1, J = 0);
+    S_unc: complex per uncoupled channel (list order), S_cpl: complex 2x2 per coupled channel (list order)."""
+    pw = []; iu = 0; ic = 0
+    for (coupled, lJ), (s, J) in zip(channels, sJ):
+        if not coupled:
+            pw.append((s, J, lJ, lJ, S_unc[iu])); iu += 1
+        else:
+            ls = (J - 1, J + 1); Sm = np.asarray(S_cpl[ic]); ic += 1
+            for a in range(2):
+                for b in range(2):
+                    pw.append((1, J, ls[a], ls[b], Sm[a, b]))
+    return pw

@@ -617,6 +617,95 @@ void orc_interp_phases(int N, int nc, const double* pedge, const double* dmid, c
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-2: total cross section from the partial-wave S-matrix, Appendix A, followed
+// step by step: spin-scattering matrix M (Eq. A.2) at theta = 0 -> Saclay amplitudes a, b (Eq. A.9) ->
+// sigma_tot = (2 pi/p) Im(a + b) (Eq. A.11).
+//
+// Clebsch-Gordan coefficient <j1 m1 j2 m2 | J M> for INTEGER angular momenta (l, s in {0,1}, J), Racah's formula.
+static double factorial(int n) { double f = 1.0; for (int i = 2; i <= n; ++i) f *= i; return f; }
+double orc_clebsch_gordan(int j1, int m1, int j2, int m2, int J, int M) {
+  if (m1 + m2 != M || J < std::abs(j1 - j2) || J > j1 + j2) return 0.0;
+  if (std::abs(m1) > j1 || std::abs(m2) > j2 || std::abs(M) > J) return 0.0;
+  double pre = (2.0 * J + 1.0) * factorial(J + j1 - j2) * factorial(J - j1 + j2) * factorial(j1 + j2 - J) / factorial(j1 + j2 + J + 1);
+  pre *= factorial(J + M) * factorial(J - M) * factorial(j1 - m1) * factorial(j1 + m1) * factorial(j2 - m2) * factorial(j2 + m2);
+  double sum = 0.0;
+  for (int k = 0; k <= j1 + j2 - J; ++k) {
+    int a = j1 + j2 - J - k, b = j1 - m1 - k, c = j2 + m2 - k, d = J - j2 + m1 + k, e = J - j1 - m2 + k;
+    if (a < 0 || b < 0 || c < 0 || d < 0 || e < 0) continue;
+    double term = 1.0 / (factorial(k) * factorial(a) * factorial(b) * factorial(c) * factorial(d) * factorial(e));
+    sum += (k & 1) ? -term : term;
+  }
+  return std::sqrt(pre) * sum;
+}
+
+// Spherical harmonic Y_l^m(theta, phi = 0) (real; Condon-Shortley phase), by the upward recurrence of P_l^m(cos theta).
+double orc_sph_harm(int l, int m, double theta) {
+  int am = std::abs(m);
+  if (am > l) return 0.0;
+  double x = std::cos(theta), sx = std::sin(theta);
+  double pmm = 1.0;
+  for (int i = 1; i <= am; ++i) pmm *= -(2.0 * i - 1.0) * sx;  // P_m^m = (-1)^m (2m-1)!! sin^m
+  double plm = pmm;
+  if (l > am) {
+    double pm1 = x * (2.0 * am + 1.0) * pmm;  // P_{m+1}^m
+    plm = pm1;
+    double pm2 = pmm;
+    for (int ll = am + 2; ll <= l; ++ll) {
+      plm = (x * (2.0 * ll - 1.0) * pm1 - (ll + am - 1.0) * pm2) / (ll - am);
+      pm2 = pm1; pm1 = plm;
+    }
+  }
+  double y = std::sqrt((2.0 * l + 1.0) / (4.0 * PI) * factorial(l - am) / factorial(l + am)) * plm;
+  if (m < 0 && (am & 1)) y = -y;  // Y_l^{-m} = (-1)^m conj(Y_l^m)
+  return y;
+}
+
+
+// Eq. A.2 for neutron-proton scattering at angle theta (phi = 0):
+//   M^s_{m_s, m_s'} = (2 pi/(i p)) sum_{J,l,l'} sqrt((2l+1)/(4 pi)) Y_{l'}^{m_s - m_s'}(theta)
+//                     <l' (m_s - m_s'), s m_s' | J m_s> <l 0, s m_s | J m_s> [S^{sJ}_{l'l} - delta_{l'l}]
+// m_s = spin projection of the incoming state (beam along z: m_l = 0), m_s' of the outgoing one.
+// Readings (X1-X2): the printed isospin factor [1 - (-1)^{l+s+T_Z}] would remove 1S0 from np scattering; it
+// is the antisymmetrisation factor 1 - (-1)^{l+s+T} with the total isospin T, and the np amplitude is the mean of the
+// T = 0 and T = 1 amplitudes, which gives weight 1 to every Pauli-allowed partial wave (each (l,s) has one T).  The
+// second Clebsch-Gordan coefficient is printed with its projections in the order (m_s, 0); it couples (l, m_l = 0)
+// with (s, m_s).  No factor i^{l-l'} (as printed; it does not affect sigma_tot).
+// Partial waves: pw = 0..npw-1 with quantum numbers s[pw], J[pw], lp[pw] (outgoing l'), l[pw] (incoming l) and
+// Spw[pw] = (re, im) of S^{sJ}_{l'l}.  Mout[s][m_s + 1][m_s' + 1] (re, im): 2 x 3 x 3 x 2 doubles.
+void orc_spin_scattering_M(int npw, const int* s, const int* J, const int* lp, const int* l, const double* Spw, double p,
+                           double theta, double* Mout) {
+  for (int i = 0; i < 2 * 3 * 3 * 2; ++i) Mout[i] = 0.0;
+  for (int ss = 0; ss <= 1; ++ss)
+    for (int ms = -ss; ms <= ss; ++ms)
+      for (int msp = -ss; msp <= ss; ++msp) {
+        cplx tot(0.0, 0.0);
+        for (int w = 0; w < npw; ++w) {
+          if (s[w] != ss) continue;
+          double y = orc_sph_harm(lp[w], ms - msp, theta);
+          double c1 = orc_clebsch_gordan(lp[w], ms - msp, ss, msp, J[w], ms);
+          double c2 = orc_clebsch_gordan(l[w], 0, ss, ms, J[w], ms);
+          cplx Sm(Spw[2 * w] - (lp[w] == l[w] ? 1.0 : 0.0), Spw[2 * w + 1]);
+          tot += std::sqrt((2.0 * l[w] + 1.0) / (4.0 * PI)) * y * c1 * c2 * Sm;
+        }
+        cplx M = cplx(2.0 * PI / p, 0.0) / cplx(0.0, 1.0) * tot;
+        size_t o = ((size_t)(ss * 3 + (ms + 1)) * 3 + (msp + 1)) * 2;
+        Mout[o] = M.real(); Mout[o + 1] = M.imag();
+      }
+}
+
+// Eqs. A.9 and A.11 at theta = 0:
+//   a = (M^1_{11} + M^1_{00} + M^1_{1,-1})/2,  b = (M^1_{11} + M^0_{00} + M^1_{1,-1})/2,  sigma_tot = (2 pi/p) Im(a + b)
+// p in fm^-1; returns sigma_tot in millibarn (1 fm^2 = 10 mb).
+double orc_sigma_tot(int npw, const int* s, const int* J, const int* lp, const int* l, const double* Spw, double p) {
+  double M[2 * 3 * 3 * 2];
+  orc_spin_scattering_M(npw, s, J, lp, l, Spw, p, 0.0, M);
+  auto el = [&](int ss, int ms, int msp) { size_t o = ((size_t)(ss * 3 + (ms + 1)) * 3 + (msp + 1)) * 2; return cplx(M[o], M[o + 1]); };
+  cplx a = 0.5 * (el(1, 1, 1) + el(1, 0, 0) + el(1, 1, -1));
+  cplx b = 0.5 * (el(1, 1, 1) + el(0, 0, 0) + el(1, 1, -1));
+  return 10.0 * (2.0 * PI / p) * (a + b).imag();
+}
+
 // Whole chain for a batch of (sample, channel) solves, OpenMP over the batch (used only for timing the oracle as the
 // reported CPU baseline and by tests that need many solves).  Per solve b: H_b (n x n) and V_b are given
 // (assembled by orc_V_yukawa/orc_assemble_H), outputs W, C, T, delta.  Returns max sweeps (or -1).

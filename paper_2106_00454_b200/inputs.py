@@ -37,6 +37,12 @@ CHANNELS_J4 = [
 ]
 
 
+def channel_sJ(name):
+    """(s, J) from the spectroscopic name 2s+1 L J of a channel ("3P0" -> (1, 0); "3S1-3D1" -> (1, 1))."""
+    first = name.split("-")[0]
+    return (int(first[0]) - 1) // 2, int(first[2])
+
+
 def sample_scales(S, seed=0):
     """[S][3] multiplicative scales (V_R, V_A, V_T) = 1 + 0.1 N(0,1)  (config 3; reading C14)."""
     z = np.random.default_rng(seed).standard_normal((S, 3))

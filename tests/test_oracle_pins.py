@@ -546,3 +546,101 @@ def test_interp_phases_yamaguchi_beats_the_steps():
         assert e_int < 0.9 * e_step, (N, e_int, e_step)
         errs.append(e_int)
     assert errs[1] < errs[0] < 1.5, errs
+
+
+# ---------------------------------------------------------------- NEXT-2: total cross section (Eqs. A.2, A.9, A.11)
+def _random_unitary_pw(rng, Jmax=3):
+    """Unitary partial-wave S-matrices built from random angles: uncoupled e^{2i delta} (Eq. A.5), coupled Stapp (A.4)."""
+    pw = []
+    for (s, l, J) in [(0, 0, 0), (1, 1, 0), (0, 1, 1), (1, 1, 1), (0, 2, 2), (1, 2, 2), (0, 3, 3), (1, 3, 3)]:
+        if J <= Jmax:
+            pw.append((s, J, l, l, np.exp(2j * rng.uniform(-1.2, 1.2))))
+    for J in range(1, Jmax + 1):
+        dm, dp, ep = rng.uniform(-1.2, 1.2), rng.uniform(-1.2, 1.2), rng.uniform(-0.4, 0.4)
+        off = 1j * math.sin(2 * ep) * np.exp(1j * (dm + dp))
+        pw += [(1, J, J - 1, J - 1, math.cos(2 * ep) * np.exp(2j * dm)), (1, J, J + 1, J + 1, math.cos(2 * ep) * np.exp(2j * dp)),
+               (1, J, J - 1, J + 1, off), (1, J, J + 1, J - 1, off)]
+    return pw
+
+
+def test_clebsch_gordan_vs_sympy_and_orthogonality():
+    from sympy import S as Sy
+    from sympy.physics.quantum.cg import CG
+    for j1 in range(0, 6):
+        for j2 in (0, 1):
+            for J in range(abs(j1 - j2), j1 + j2 + 1):
+                for m1 in range(-j1, j1 + 1):
+                    for m2 in range(-j2, j2 + 1):
+                        M = m1 + m2
+                        if abs(M) > J:
+                            continue
+                        ref = float(CG(Sy(j1), Sy(m1), Sy(j2), Sy(m2), Sy(J), Sy(M)).doit())
+                        assert abs(o.clebsch_gordan(j1, m1, j2, m2, J, M) - ref) < 1e-14
+    # orthogonality: sum_{m1 m2} <j1 m1 j2 m2|J M><j1 m1 j2 m2|J' M> = delta_JJ'
+    for J in (2, 3, 4):
+        for Jp in (2, 3, 4):
+            t = sum(o.clebsch_gordan(3, m1, 1, m2, J, 1) * o.clebsch_gordan(3, m1, 1, m2, Jp, 1)
+                    for m1 in range(-3, 4) for m2 in (-1, 0, 1))
+            assert abs(t - (1.0 if J == Jp else 0.0)) < 1e-14
+    assert o.clebsch_gordan(1, 1, 1, 1, 1, 1) == 0.0 and o.clebsch_gordan(2, 0, 1, 0, 4, 0) == 0.0
+
+
+def test_sph_harm_vs_scipy():
+    from scipy.special import sph_harm_y
+    for l in range(0, 7):
+        for m in range(-l, l + 1):
+            for th in (0.0, 0.3, 1.1, math.pi / 2, 2.9, math.pi):
+                ref = complex(sph_harm_y(l, m, th, 0.0))
+                assert abs(ref.imag) < 1e-15 and abs(o.sph_harm(l, m, th) - ref.real) < 1e-13
+
+
+def test_sigma_tot_single_wave_closed_forms():
+    # only 1S0: spin weight 1/4 of 4 pi sin^2(delta)/p^2;  only 3P0 (J = 0): the same weight 2J+1 = 1
+    p, d = 0.9, 0.7
+    ref = 10.0 * math.pi * math.sin(d) ** 2 / p ** 2
+    assert abs(o.sigma_tot([(0, 0, 0, 0, np.exp(2j * d))], p) - ref) < 1e-13 * ref
+    assert abs(o.sigma_tot([(1, 0, 1, 1, np.exp(2j * d))], p) - ref) < 1e-13 * ref
+    # 3P1 alone: weight 2J+1 = 3;  S = 1 everywhere: nothing scatters
+    assert abs(o.sigma_tot([(1, 1, 1, 1, np.exp(2j * d))], p) - 3 * ref) < 1e-13 * ref
+    assert o.sigma_tot([(0, 0, 0, 0, 1.0), (1, 1, 1, 1, 1.0)], p) == 0.0
+    # 1S0 alone is isotropic: M^0_00 = e^{i delta} sin(delta)/p at every angle
+    for th in (0.0, 1.0, 2.5):
+        M = o.spin_scattering_M([(0, 0, 0, 0, np.exp(2j * d))], p, th)
+        assert abs(M[(0, 0, 0)] - np.exp(1j * d) * math.sin(d) / p) < 1e-15
+
+
+def test_sigma_tot_partial_wave_sum_and_optical_theorem():
+    """(2 pi/p) Im(a+b) equals the partial-wave sum (pi/2p^2) sum (2J+1) Re(1 - S_ll) for ANY S (the off-diagonal
+    elements drop out of the spin trace), and, for unitary S, the angular integral of the unpolarised differential
+    cross section (1/4) Tr(M M^dagger) of Eq. A.6 (optical theorem) -- which checks Y, the Clebsch-Gordan coefficients,
+    the sqrt((2l+1)/4pi) and 2pi/(ip) factors of Eq. A.2 and the weights of Eqs. A.9/A.11 all at once."""
+    rng = np.random.default_rng(5)
+    x, w = np.polynomial.legendre.leggauss(24)
+    for trial in range(3):
+        pw = _random_unitary_pw(rng)
+        p = rng.uniform(0.3, 2.0)
+        sig = o.sigma_tot(pw, p)
+        closed = 10.0 * math.pi / (2 * p * p) * sum((2 * J + 1) * (1 - complex(Sv).real) for (s, J, lp, l, Sv) in pw if lp == l)
+        assert abs(sig - closed) < 1e-13 * abs(closed)
+        integral = 0.0
+        for xi, wi in zip(x, w):
+            M = o.spin_scattering_M(pw, p, math.acos(xi))
+            integral += 2 * math.pi * wi * 0.25 * sum(abs(v) ** 2 for v in M.values())
+        assert abs(10.0 * integral - sig) < 1e-12 * sig
+    # non-unitary S (as WPCD produces): the partial-wave sum still holds, off-diagonal elements do not contribute
+    pw = [(s, J, lp, l, Sv * rng.uniform(0.9, 1.05)) for (s, J, lp, l, Sv) in _random_unitary_pw(rng)]
+    closed = 10.0 * math.pi / (2 * 0.8 ** 2) * sum((2 * J + 1) * (1 - complex(Sv).real) for (s, J, lp, l, Sv) in pw if lp == l)
+    assert abs(o.sigma_tot(pw, 0.8) - closed) < 1e-13 * abs(closed)
+
+
+def test_sigma_tot_yamaguchi_1S0_against_closed_form_phase():
+    """1S0 only, separable Yamaguchi potential: sigma_tot from the MI S-matrix equals pi sin^2(delta)/p^2 with the
+    analytic phase shift (reading C15)."""
+    lamA, _ = inp.yamaguchi_lambda()
+    for tlab in (10.0, 100.0, 300.0):
+        p = math.sqrt(inp.MU * tlab) / inp.HBARC
+        Sx = _yamaguchi_S_exact(tlab)
+        d = 0.5 * math.atan2(Sx.imag, Sx.real)
+        S, _ = o.mi_solve(tlab, kind=1, lambdaA=lamA, beta=inp.YAMAGUCHI_BETA, NQ=96)
+        ref = 10.0 * math.pi * math.sin(d) ** 2 / p ** 2
+        assert abs(o.sigma_tot([(0, 0, 0, 0, S)], p) - ref) < 1e-9 * ref
