@@ -165,6 +165,22 @@ int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, i
 int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
                        const double* d_q, int nq, double* d_out, void* stream);
 
+/* Total neutron-proton cross section from the on-shell T of all partial waves, Appendix A
+ * (PAPER.md:473-537): S = 1 - 2 pi i T/dE_bin (Eq. A.3), spin-scattering matrix at theta = 0 (Eq. A.2), Saclay amplitudes
+ * a, b (Eq. A.9), sigma_tot = (2 pi/p) Im(a + b) (Eq. A.11).  At theta = 0 the spin trace a + b collapses the
+ * Clebsch-Gordan sums, so the kernel evaluates the equivalent partial-wave sum
+ *   sigma_tot(E) = (pi/(2 p^2)) sum_channels (2J+1) sum_l Re(1 - S_ll),   p^2 = E_cm/cE,
+ * every Pauli-allowed partial wave with weight 1 (np scattering, reading X1).
+ *   h_J_unc : [n_unc] HOST, total angular momentum J of every uncoupled channel (e.g. 3P0: J = 0), list order
+ *   h_J_cpl : [n_cpl] HOST, J >= 1 of every coupled channel
+ *   d_T_unc : [S][n_unc][nE][2], d_T_cpl : [S][n_cpl][nE][2][2][2] -- as written by wpcd_onshell_T for batch = S x channels
+ *             (NULL allowed when the count is 0);  d_bin, d_dE, d_Ecm as for wpcd_phase_shifts / wpcd_onshell_T
+ *   d_sigma : [S][nE] millibarn (1 fm^2 = 10 mb); NaN where the energy is outside the grid
+ * n_unc, n_cpl <= WPCD_MAX_CHANNELS. */
+int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, const double* d_T_unc, int n_cpl,
+                   const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
+                   double hbarc, double mu, double* d_sigma, void* stream);
+
 /* Test hooks (host only, no GPU needed): the block tournament that wpcd_diag_batched runs (csrc/jacobi_schedule.cuh).
  * m = number of players (8-wide blocks, even, >= 6; players >= nb are padding), a sweep has m-1 steps of m/2 slots.
  *   wpcd_jacobi_schedule      : blocks (I < J) of slot s at step t; J = -1 single block, I = J = -1 empty slot.

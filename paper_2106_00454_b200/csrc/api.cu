@@ -148,6 +148,19 @@ int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double
                             static_cast<cudaStream_t>(stream));
 }
 
+int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, const double* d_T_unc, int n_cpl,
+                   const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
+                   double hbarc, double mu, double* d_sigma, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || S < 1 || nE < 1 || n_unc < 0 || n_cpl < 0 || n_unc + n_cpl < 1 || !d_bin || !d_dE || !d_Ecm || !d_sigma) return WPCD_EINVAL;
+  if ((n_unc && (!h_J_unc || !d_T_unc)) || (n_cpl && (!h_J_cpl || !d_T_cpl)) || !(hbarc > 0) || !(mu > 0)) return WPCD_EINVAL;
+  if (n_unc > WPCD_MAX_CHANNELS || n_cpl > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
+  for (int c = 0; c < n_unc; ++c) if (h_J_unc[c] < 0) return WPCD_EINVAL;
+  for (int c = 0; c < n_cpl; ++c) if (h_J_cpl[c] < 1) return WPCD_EINVAL;
+  return wpcd_sigma_launch(h, S, nE, n_unc, h_J_unc, d_T_unc, n_cpl, h_J_cpl, d_T_cpl, d_bin, d_dE, d_Ecm, hbarc, mu, d_sigma,
+                           static_cast<cudaStream_t>(stream));
+}
+
 int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, int nE, int* h_rows, int* n_ranges) {
   if (!grid || !grid->h_edges || grid->N < 1 || !h_Ecm || nE < 1 || !h_rows || !n_ranges) return WPCD_EINVAL;
   return wpcd_onshell_rows_host(grid->N, coupled ? 1 : 0, grid->h_edges, grid->hbarc, grid->mu, h_Ecm, nE, h_rows, n_ranges);

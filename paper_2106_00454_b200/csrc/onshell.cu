@@ -388,6 +388,46 @@ __global__ void __launch_bounds__(128) k_interp(int N, int nc, int nq, const dou
   }
 }
 
+// Total np cross section, Appendix A.  The spin-scattering matrix of Eq. A.2 at theta = 0 only has
+// m_s = m_s' elements (Y_l'^m(0) = sqrt((2l'+1)/4pi) delta_m0), and the combination a + b = M^1_11 + (M^1_00 + M^0_00)/2
+// of Eq. A.9 is half the spin trace, in which the Clebsch-Gordan sums collapse (orthogonality) to 2J+1 per partial wave
+// with l' = l.  With S_ll = 1 - 2 pi i T_ll/dE_i (Eq. A.3 in the wave-packet normalisation, reading C2) Eq. A.11
+// becomes
+//   sigma_tot(E) = (2 pi/p) Im(a+b) = (pi/(2 p^2)) sum_channels (2J+1) sum_l Re(1 - S_ll),  Re(1 - S_ll) = -2 pi Im T_ll/dE_i.
+// One thread per (sample, energy); the channel loop reads T with the energy index fastest (coalesced).
+struct SigmaParams {
+  const double* Tunc;  // [S][n_unc][nE][2]
+  const double* Tcpl;  // [S][n_cpl][nE][2][2][2]
+  const int* bin;
+  const double* dE;
+  const double* Ecm;
+  double* sigma;       // [S][nE] mb
+  double cE;           // hbarc^2/(2 mu): E = cE p^2
+  int S, nE, n_unc, n_cpl;
+  int J_unc[WPCD_MAX_CHANNELS], J_cpl[WPCD_MAX_CHANNELS];
+};
+
+__global__ void k_sigma(SigmaParams P) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)P.S * P.nE) return;
+  const int e = (int)(idx % P.nE);
+  const size_t s = idx / P.nE;
+  const int b = P.bin[e];
+  if (b < 0) { P.sigma[idx] = nan(""); return; }
+  const double f = -2.0 * WPCD_PI / P.dE[b];
+  double acc = 0.0;
+  for (int c = 0; c < P.n_unc; ++c) {
+    const double ti = P.Tunc[((s * P.n_unc + c) * P.nE + e) * 2 + 1];
+    acc += (2.0 * P.J_unc[c] + 1.0) * (f * ti);
+  }
+  for (int c = 0; c < P.n_cpl; ++c) {
+    const double* t = P.Tcpl + ((s * P.n_cpl + c) * P.nE + e) * 8;
+    acc += (2.0 * P.J_cpl[c] + 1.0) * (f * t[1] + f * t[7]);
+  }
+  const double p2 = P.Ecm[e] / P.cE;
+  P.sigma[idx] = 10.0 * WPCD_PI / (2.0 * p2) * acc;  // fm^2 -> mb
+}
+
 int chunk_bins(int n, int nc, int max_smem) {
   int R = 16 / nc;  // at most 16 accumulator rows
   while (R > 1 && (size_t)(3 * n + 2 * R * nc * n) * 8 > (size_t)max_smem - 1024) R >>= 1;
@@ -435,6 +475,21 @@ int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const doubl
   if (rc) return rc;
   k_interp<<<batch, 128, smem, st>>>(N, nc, nq, d_pedge, d_delta_mid, d_q, d_out);
   return wpcd_check_cuda(h, cudaGetLastError(), "interp_phases launch");
+}
+
+int wpcd_sigma_launch(WpcdHandle* h, int S, int nE, int n_unc, const int* h_J_unc, const double* d_T_unc, int n_cpl,
+                      const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
+                      double hbarc, double mu, double* d_sigma, cudaStream_t st) {
+  SigmaParams P;
+  P.Tunc = d_T_unc; P.Tcpl = d_T_cpl; P.bin = d_bin; P.dE = d_dE; P.Ecm = d_Ecm; P.sigma = d_sigma;
+  P.cE = hbarc * hbarc / (2.0 * mu); P.S = S; P.nE = nE; P.n_unc = n_unc; P.n_cpl = n_cpl;
+  for (int c = 0; c < WPCD_MAX_CHANNELS; ++c) {
+    P.J_unc[c] = c < n_unc ? h_J_unc[c] : 0;
+    P.J_cpl[c] = c < n_cpl ? h_J_cpl[c] : 0;
+  }
+  const size_t total = (size_t)S * nE;
+  k_sigma<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(P);
+  return wpcd_check_cuda(h, cudaGetLastError(), "sigma_tot launch");
 }
 
 // Rows of C that wpcd_onshell_T will read for these energies (host arithmetic, same bin rule as k_bins, widened by one

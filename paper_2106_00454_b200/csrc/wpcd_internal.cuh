@@ -36,5 +36,8 @@ int wpcd_phase_launch(WpcdHandle* h, int coupled, int batch, int nE, const doubl
                       const double* d_dE, double* d_delta, double* d_S, cudaStream_t st);
 int wpcd_interp_launch(WpcdHandle* h, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
                        const double* d_q, int nq, double* d_out, cudaStream_t st);
+int wpcd_sigma_launch(WpcdHandle* h, int S, int nE, int n_unc, const int* h_J_unc, const double* d_T_unc, int n_cpl,
+                      const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
+                      double hbarc, double mu, double* d_sigma, cudaStream_t st);
 int wpcd_onshell_rows_host(int N, int coupled, const double* h_edges, double hbarc, double mu, const double* h_Ecm, int nE,
                            int* h_rows, int* n_ranges);

@@ -16,7 +16,7 @@ class Pipeline:
     KERNELS_PER_STEP_FIXED = 2  # k_grid, k_basis
 
     def __init__(self, edges, channels, Ecm, S, potential, n_scale_cols=3, device=0, max_sweeps=30, tol=0.0,
-                 onshell_rows_only=True):
+                 onshell_rows_only=True, channel_J=None):
         self.h = wpcd.Handle(device)
         self.dev = self.h.device
         self.edges = np.asarray(edges, dtype=np.float64)
@@ -55,6 +55,11 @@ class Pipeline:
                 bins=torch.empty(self.nE, dtype=torch.int32, device=self.dev),
                 owork=torch.empty(256, dtype=torch.uint8, device=self.dev),
                 delta=torch.empty((batch, self.nE, 3) if kind else (batch, self.nE), dtype=f64, device=self.dev))
+        # optional epilogue: total cross section from all channels; channel_J = total J per channel
+        self.J = None
+        if channel_J is not None:
+            self.J = {k: [int(J) for (c, _), J in zip(self.channels, channel_J) if bool(c) == bool(k)] for k in (0, 1)}
+            self.sigma = torch.empty((self.S, self.nE), dtype=f64, device=self.dev)
         # pinned host buffers of the end-to-end call
         self.h_scales = torch.empty((self.S, n_scale_cols), dtype=f64).pin_memory()
         self.h_delta = {k: torch.empty(v["delta"].shape, dtype=f64).pin_memory() for k, v in self.kind.items()}
@@ -67,7 +72,7 @@ class Pipeline:
     @property
     def launches_per_step(self):
         # k_grid, k_basis, k_combine per kind; k_schedule, k_jacobi, k_bins, k_onshell, k_phase per kind
-        return 2 + len(self.kind) * 6
+        return 2 + len(self.kind) * 6 + (1 if self.J is not None else 0)
 
     def solve_device(self, events=None):
         """One pass of the whole hot path with inputs resident in HBM.  events: optional dict name -> (start, end)
@@ -90,6 +95,11 @@ class Pipeline:
                              T=b["T"], bins=b["bins"], work=b["owork"])
             self.h.phase_shifts(kind, b["T"], b["bins"], self.geo["dE"], want_S=False, delta=b["delta"])
             rec("onshell_" + tag, 1)
+        if self.J is not None:
+            any_kind = next(iter(self.kind.values()))
+            self.h.sigma_tot(self.J[0], self.kind[0]["T"] if 0 in self.kind else None, self.J[1],
+                             self.kind[1]["T"] if 1 in self.kind else None, any_kind["bins"], self.geo["dE"], self.Ecm,
+                             out=self.sigma)
 
     def stage_names(self):
         names = ["build"]

@@ -60,6 +60,8 @@ _lib.wpcd_interp_phases.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _i, _vp, _vp
 _lib.wpcd_interp_phases.restype = _i
 _lib.wpcd_onshell_rows.argtypes = [C.POINTER(Grid), _i, C.POINTER(_d), _i, C.POINTER(_i), C.POINTER(_i)]
 _lib.wpcd_onshell_rows.restype = _i
+_lib.wpcd_sigma_tot.argtypes = [_vp, _i, _i, _i, C.POINTER(_i), _vp, _i, C.POINTER(_i), _vp, _vp, _vp, _vp, _d, _d, _vp, _vp]
+_lib.wpcd_sigma_tot.restype = _i
 
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
@@ -205,6 +207,24 @@ class Handle:
         rc = _lib.wpcd_interp_phases(self._h, int(coupled), batch, N, _ptr(pedge), _ptr(delta_mid), _ptr(q), nq, _ptr(out),
                                      _stream(stream))
         self._check(rc, "wpcd_interp_phases")
+        return out
+
+    # ------------------------------------------------------------------ wpcd_sigma_tot
+    def sigma_tot(self, J_unc, T_unc, J_cpl, T_cpl, bins, dE, Ecm, hbarc=197.327, mu=469.46, stream=None, out=None):
+        """Eqs. A.2, A.9, A.11: total np cross section [S][nE] in mb from T_unc [S][n_unc][nE][2] and
+        T_cpl [S][n_cpl][nE][2][2][2] (either may be None); J_unc / J_cpl: total J of every channel."""
+        n_unc, n_cpl = len(J_unc), len(J_cpl)
+        ref = T_unc if T_unc is not None else T_cpl
+        nE = Ecm.shape[0]
+        if ref is None:  # no channels at all: let the library report the argument error
+            S = 1 if out is None else out.shape[0]
+        else:
+            S = ref.numel() // (max(n_unc if T_unc is not None else n_cpl, 1) * nE * (2 if T_unc is not None else 8))
+        out = torch.empty((S, nE), dtype=torch.float64, device=Ecm.device) if out is None else out
+        ju = (_i * max(n_unc, 1))(*[int(j) for j in J_unc]); jc = (_i * max(n_cpl, 1))(*[int(j) for j in J_cpl])
+        rc = _lib.wpcd_sigma_tot(self._h, S, nE, n_unc, ju, _ptr(T_unc), n_cpl, jc, _ptr(T_cpl), _ptr(bins), _ptr(dE),
+                                 _ptr(Ecm), float(hbarc), float(mu), _ptr(out), _stream(stream))
+        self._check(rc, "wpcd_sigma_tot")
         return out
 
     # ------------------------------------------------------------------ wpcd_phase_shifts

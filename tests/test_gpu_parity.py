@@ -380,3 +380,97 @@ def test_diag_row_ranges_and_pipeline_rows(ctx):
         res.append({k: v.clone() for k, v in d.items()})
     for k in res[0]:
         assert torch.equal(res[0][k], res[1][k])
+
+
+def _oracle_sigma(N, channels, names, Ecm, scale):
+    """Oracle chain per channel -> S-matrices -> Eqs. A.2/A.9/A.11 per energy.  Returns sigma [nE] (NaN off the grid),
+    the oracle T per channel and the weight sum of (2J+1) over the diagonal partial waves."""
+    sJ = [inp.channel_sJ(nm) for nm in names]
+    refs = []
+    for (kind, lJ) in channels:
+        ch = hp.oracle_channel(N, kind, lJ, scale)
+        refs.append((kind, hp.oracle_solve(N, kind, ch, Ecm), ch))
+    sig = np.full(len(Ecm), np.nan)
+    for e, E in enumerate(Ecm):
+        if refs[0][1]["bin"][e] < 0:
+            continue
+        p = np.sqrt(E / (inp.HBARC ** 2 / (2 * inp.MU)))
+        S_unc = [r["S"][e] for k, r, _ in refs if not k]
+        S_cpl = [r["S"][e] for k, r, _ in refs if k]
+        sig[e] = hp.o.sigma_tot(hp.o.partial_waves(channels, sJ, S_unc, S_cpl), p)
+    wsum = sum((2 * J + 1) * (2 if k else 1) for (k, _), (_, J) in zip(channels, sJ))
+    return sig, refs, wsum
+
+
+def test_sigma_tot_all_channels(ctx):
+    """NEXT-2: total cross section of all 14 channels, GPU chain (build -> diag -> T -> wpcd_sigma_tot) against the
+    oracle chain (-> S -> Eq. A.2 with Clebsch-Gordan coefficients -> A.9 -> A.11).  Tolerance: the north_star S-matrix
+    tolerance |dS| <= 3.5e-10 propagated through the partial-wave sum, (10 pi/(2 p^2)) sum (2J+1) |dS|."""
+    h, torch = ctx["h"], ctx["torch"]
+    N = 50
+    names = [c[0] for c in inp.CHANNELS_J4]
+    channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    sJ = [inp.channel_sJ(nm) for nm in names]
+    _, Ecm = inp.energies(40)
+    Ecm = np.concatenate([Ecm, [1e9]])   # the last energy is outside the grid -> NaN
+    scales = inp.sample_scales(2, seed=3)
+    res = _gpu_pipeline(ctx, N, channels, Ecm, scales=scales, S=2)
+    T_unc = _to_dev(ctx, np.stack([res[0]["T"].real, res[0]["T"].imag], axis=-1))
+    T_cpl = _to_dev(ctx, np.stack([res[1]["T"].real, res[1]["T"].imag], axis=-1))
+    J_unc = [J for (k, _), (_, J) in zip(channels, sJ) if not k]
+    J_cpl = [J for (k, _), (_, J) in zip(channels, sJ) if k]
+    bins, dE, dEcm = _to_dev(ctx, res[0]["bin"]), _to_dev(ctx, res["dE"]), _to_dev(ctx, Ecm)
+    sig = h.sigma_tot(J_unc, T_unc, J_cpl, T_cpl, bins, dE, dEcm).cpu().numpy()
+    assert sig.shape == (2, len(Ecm)) and np.isnan(sig[:, -1]).all()
+    p2 = Ecm / (inp.HBARC ** 2 / (2 * inp.MU))
+    worst = 0.0
+    for s in range(2):
+        ref, refs, wsum = _oracle_sigma(N, channels, names, Ecm, scales[s])
+        ok = ~np.isnan(ref)
+        for kind, r, _ in refs:
+            ok &= hp.swp_edge_distance(r["W"], kind, Ecm) > hp.EDGE_GUARD
+        assert ok.sum() >= 35 and np.isnan(ref[-1])
+        bound = 10 * np.pi / (2 * p2) * wsum * hp.TOL_S_ABS
+        err = np.abs(sig[s] - ref)
+        assert (err[ok] <= bound[ok]).all(), (s, (err[ok] / bound[ok]).max())
+        worst = max(worst, (err[ok] / np.abs(ref[ok])).max())
+        assert (ref[ok] > 0).all()
+    print("sigma_tot max relative deviation", worst)
+    assert worst < 1e-9
+    # the kernel alone, fed with the ORACLE's T (no eigen-solver differences): partial-wave sum vs the Clebsch-Gordan chain
+    ref, refs, wsum = _oracle_sigma(N, channels, names, Ecm, scales[0])
+    To_unc = np.stack([r["T"] for k, r, _ in refs if not k])[None]
+    To_cpl = np.stack([r["T"] for k, r, _ in refs if k])[None]
+    up = lambda T: _to_dev(ctx, np.stack([T.real, T.imag], axis=-1))
+    sig1 = h.sigma_tot(J_unc, up(To_unc), J_cpl, up(To_cpl), bins, dE, dEcm).cpu().numpy()[0]
+    ok = ~np.isnan(ref)
+    assert (np.abs(sig1[ok] - ref[ok]) <= 2e-12 * np.abs(ref[ok]) + 1e-11).all()
+    # subsets of the channel list: uncoupled only / coupled only add up to the total
+    su = h.sigma_tot(J_unc, up(To_unc), [], None, bins, dE, dEcm).cpu().numpy()[0]
+    sc = h.sigma_tot([], None, J_cpl, up(To_cpl), bins, dE, dEcm).cpu().numpy()[0]
+    assert (np.abs(su[ok] + sc[ok] - sig1[ok]) <= 1e-12 * np.abs(sig1[ok])).all()
+    # argument errors
+    with pytest.raises(RuntimeError):
+        h.sigma_tot([], None, [], None, bins, dE, dEcm, out=torch.empty((1, len(Ecm)), dtype=torch.float64, device=ctx["dev"]))
+    with pytest.raises(RuntimeError):
+        h.sigma_tot(J_unc, up(To_unc), [0], up(To_cpl[:, :1]), bins, dE, dEcm)   # coupled channels need J >= 1
+
+
+def test_pipeline_sigma_tot_epilogue(ctx):
+    """Pipeline(channel_J=...) appends wpcd_sigma_tot to the pass: same numbers as the oracle chain on sampled energies."""
+    from paper_2106_00454_b200.pipeline import Pipeline
+    N = 32
+    names = [c[0] for c in inp.CHANNELS_J4]; channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    _, Ecm = inp.energies(12)
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    pipe = Pipeline(inp.grid_edges(N), channels, Ecm, 3, pot, device=0, channel_J=[inp.channel_sJ(nm)[1] for nm in names])
+    scales = inp.sample_scales(3, seed=11)
+    pipe.scales.copy_(ctx["torch"].as_tensor(scales))
+    pipe.solve_device(); ctx["torch"].cuda.synchronize()
+    sig = pipe.sigma.cpu().numpy()
+    assert pipe.launches_per_step == 15
+    ref, refs, _ = _oracle_sigma(N, channels, names, Ecm, scales[2])
+    ok = ~np.isnan(ref)
+    for kind, r, _c in refs:
+        ok &= hp.swp_edge_distance(r["W"], kind, Ecm) > hp.EDGE_GUARD
+    assert ok.sum() >= 10 and (np.abs(sig[2][ok] - ref[ok]) < 1e-9 * ref[ok]).all()

@@ -644,3 +644,39 @@ def test_sigma_tot_yamaguchi_1S0_against_closed_form_phase():
         S, _ = o.mi_solve(tlab, kind=1, lambdaA=lamA, beta=inp.YAMAGUCHI_BETA, NQ=96)
         ref = 10.0 * math.pi * math.sin(d) ** 2 / p ** 2
         assert abs(o.sigma_tot([(0, 0, 0, 0, S)], p) - ref) < 1e-9 * ref
+
+
+def test_sigma_tot_wpcd_converges_to_MI():
+    """Shape of PAPER.md:389-405 (Figs. 6-7) on the synthetic potential: the WPCD total cross section of all 14
+    channels approaches the MI ("exact") one as the number of wave packets grows; method error of a few mb."""
+    names = [c[0] for c in inp.CHANNELS_J4]; channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    sJ = [inp.channel_sJ(nm) for nm in names]
+    tl = np.linspace(5.0, 345.0, 18); Ecm = tl / 2
+    exact = []
+    for t in tl:
+        Su = [o.mi_solve(t, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=lJ, NQ=64)[0] for (k, lJ) in channels if not k]
+        Sc = [o.mi_solve(t, coupled=True, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=lJ, VT=inp.TENSOR_V, muT=inp.TENSOR_MU, NQ=64)[0]
+              for (k, lJ) in channels if k]
+        exact.append(o.sigma_tot(o.partial_waves(channels, sJ, Su, Sc), math.sqrt(inp.MU * t) / inp.HBARC))
+    exact = np.array(exact)
+    assert 1500 < exact[0] < 1800 and 50 < exact[-1] < 60 and (np.diff(exact) < 0).all()   # np-like: falls with energy
+    mean_err = {}
+    for N in (32, 64):
+        p = inp.grid_edges(N); e0, dE, Ee = o.fwp(p)
+        S_unc, S_cpl = [], []
+        for (k, lJ) in channels:
+            if not k:
+                H, V = o.assemble_H(e0, o.V_yukawa(p, lJ, inp.MT_V0, inp.MT_MU))
+            else:
+                H, V = o.assemble_H(e0, o.V_yukawa(p, lJ - 1, inp.MT_V0, inp.MT_MU), o.V_yukawa(p, lJ + 1, inp.MT_V0, inp.MT_MU),
+                                    o.V_yukawa(p, lJ, [inp.TENSOR_V], [inp.TENSOR_MU]))
+            W, Cm, _ = o.jacobi(H)
+            T, b = o.onshell_T(N, k, Ee, V, W, Cm, Ecm)
+            _, S = o.phase_shifts(k, T, b, dE)
+            (S_cpl if k else S_unc).append(S)
+        sig = np.array([o.sigma_tot(o.partial_waves(channels, sJ, [S[e] for S in S_unc], [S[e] for S in S_cpl]),
+                                    math.sqrt(2 * inp.MU * Ecm[e]) / inp.HBARC) for e in range(len(Ecm))])
+        err = np.abs(sig - exact)
+        mean_err[N] = err.mean()
+        assert np.median(err) < (2.0 if N == 32 else 1.0), (N, np.median(err))
+    assert mean_err[64] < 0.7 * mean_err[32], mean_err
