@@ -25,6 +25,7 @@ def _sig(name, res, args):
 _gl = _sig("orc_gl_rule", None, [_i, _pd, _pd])
 _Q = _sig("orc_legendre_Q", _d, [_i, _d])
 _grid = _sig("orc_grid_tan", None, [_i, _d, _pd])
+_gridc = _sig("orc_grid_chebyshev", None, [_i, _d, _d, _pd])
 _fwp = _sig("orc_fwp", None, [_i, _pd, _d, _d, _pd, _pd, _pd])
 _Vyuk = _sig("orc_V_yukawa", None, [_i, _pd, _i, _i, _pd, _pd, _i, _pd])
 _Vyam = _sig("orc_V_yamaguchi", None, [_i, _pd, _d, _d, _i, _i, _pd, _pd])
@@ -72,6 +73,13 @@ def legendre_Q(l, z):
 def grid_tan(N, alpha=1.0):
     p = np.empty(N + 1)
     _grid(N, alpha, p)
+    return p
+
+
+def grid_chebyshev(N, t=2.0, alpha=100.0 / HBARC):
+    """Eq. 31: y_0 = 0, y_j = alpha tan^t((2j-1) pi/(4N)); defaults are the paper's (t = 2, alpha = 100 MeV)."""
+    p = np.empty(N + 1)
+    _gridc(N, t, alpha, p)
     return p
 
 

@@ -118,6 +118,14 @@ void orc_grid_tan(int N, double alpha, double* p) {
   for (int i = 0; i <= N; ++i) p[i] = alpha * std::tan(PI * i / (2.0 * N + 1.0));
 }
 
+// The paper's own bin distribution, Eq. 31: y_0 = 0, y_j = alpha tan^t((2j-1) pi/(4 N)), j = 1..N
+// ("sparseness degree" t, scale alpha; the paper uses momentum bins with t = 2 and alpha = 100 MeV, i.e.
+// alpha = 100/hbarc fm^-1).  SURVEY 8(f)-3.
+void orc_grid_chebyshev(int N, double t, double alpha, double* p) {
+  p[0] = 0.0;
+  for (int j = 1; j <= N; ++j) p[j] = alpha * std::pow(std::tan((2.0 * j - 1.0) * PI / (4.0 * N)), t);
+}
+
 // Free wave-packet (f(k)=1, N_i = Delta k_i, Eq. 17) kinetic energies and bin energy widths.
 // Reading C4: exact matrix element <x_i|h0|x_i> = cE (p_i^2 + p_i p_{i+1} + p_{i+1}^2)/3, not Eq. 18's midpoint.
 // Eedge_i = cE p_i^2 (E = p^2/m_N, m_N = 2 mu), dE_i = Eedge_{i+1} - Eedge_i.

@@ -23,6 +23,13 @@ def grid_edges(N, alpha=1.0):
     return alpha * np.tan(np.pi * i / (2.0 * N + 1.0))
 
 
+def grid_chebyshev(N, t=2.0, alpha=100.0 / HBARC):
+    """The paper's own bin edges, Eq. 31 (PAPER.md:240-245): y_0 = 0, y_j = alpha tan^t((2j-1) pi/(4N)), j = 1..N, fm^-1;
+    defaults t = 2, alpha = 100 MeV (an input of the C ABI like grid_edges)."""
+    j = np.arange(1, N + 1, dtype=np.float64)
+    return np.concatenate([[0.0], alpha * np.tan((2.0 * j - 1.0) * np.pi / (4.0 * N)) ** t])
+
+
 def energies(nE):
     """nE lab energies uniform on 1..350 MeV; returns (T_lab, E_cm = T_lab/2)."""
     tlab = np.linspace(1.0, 350.0, nE)

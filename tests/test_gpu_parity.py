@@ -24,15 +24,15 @@ def _to_dev(ctx, a, dtype=None):
     return t if dtype is None else t.to(dtype)
 
 
-def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0.0):
+def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0.0, edges=None, n_gl=8, mode=0):
     """Full hot path on the GPU for a channel list; returns per-kind dicts of numpy arrays."""
     h, torch = ctx["h"], ctx["torch"]
-    p = inp.grid_edges(N)
+    p = inp.grid_edges(N) if edges is None else edges
     d_scales = None if scales is None else _to_dev(ctx, scales)
     kw = dict(yamaguchi=yamaguchi) if yamaguchi is not None else dict(
         V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1] if scales is not None else None, VT=inp.TENSOR_V,
         muT=inp.TENSOR_MU, VT_scale_idx=2 if scales is not None else -1)
-    out = h.build_channels(p, channels, scales=d_scales, S=S, **kw)
+    out = h.build_channels(p, channels, scales=d_scales, S=S, n_gl=n_gl, **kw)
     d_E = _to_dev(ctx, Ecm)
     res = {}
     for kind, key in ((0, "H_unc"), (1, "H_cpl")):
@@ -42,7 +42,7 @@ def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0
         n = H.shape[-1]
         Hb = H.reshape(-1, n, n)
         W, C, info = h.diag_batched(Hb, tol=tol)
-        T, bins = h.onshell_T(N, kind, out["e0"], out["Eedge"], Hb, W, C, d_E)
+        T, bins = h.onshell_T(N, kind, out["e0"], out["Eedge"], Hb, W, C, d_E, mode=mode)
         delta, Sm = h.phase_shifts(kind, T, bins, out["dE"])
         torch.cuda.synchronize()
         nch = H.shape[1]
@@ -55,9 +55,10 @@ def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0
     return res
 
 
-def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguchi=None, label=""):
-    ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi)
-    ref = hp.oracle_solve(N, kind, ch, Ecm)
+def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguchi=None, label="", edges=None, ngl=8,
+                     averaged=False):
+    ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi, edges=edges, ngl=ngl)
+    ref = hp.oracle_solve(N, kind, ch, Ecm, averaged=averaged)
     g = res[kind]
     n = ch["H"].shape[0]
     normH = np.abs(ch["H"]).max()
@@ -474,3 +475,21 @@ def test_pipeline_sigma_tot_epilogue(ctx):
     for kind, r, _c in refs:
         ok &= hp.swp_edge_distance(r["W"], kind, Ecm) > hp.EDGE_GUARD
     assert ok.sum() >= 10 and (np.abs(sig[2][ok] - ref[ok]) < 1e-9 * ref[ok]).all()
+
+
+
+@pytest.mark.parametrize("N", [16, 24, 32, 64, 96])
+def test_paper_discretisation_chebyshev_midpoint(ctx, N):
+    """NEXT-3: the paper's own set-up -- Chebyshev momentum bins of Eq. 31 (t = 2, alpha = 100 MeV), the
+    mid-point potential of Eq. 30 (= the n_gl = 1 rule) and the 8-point bin average of Eq. 29, N_WP = 16..96 (the regime
+    of PAPER.md:437-447, several matrices per SM), point-wise and energy-averaged T, uncoupled and coupled."""
+    edges = inp.grid_chebyshev(N)
+    tl, Ecm = inp.energies(60)
+    scales = inp.sample_scales(3, seed=N)
+    channels = [(0, 0), (0, 2), (1, 1)]
+    for n_gl, mode in ((1, 1), (8, 0), (1, 0)):
+        res = _gpu_pipeline(ctx, N, channels, Ecm, scales=scales, S=3, edges=edges, n_gl=n_gl, mode=mode)
+        for s, c, kind, lJ in ((0, 0, 0, 0), (2, 1, 0, 2), (1, 0, 1, 1)):
+            r = _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=scales[s], label=f"cheb N={N} ngl={n_gl} mode={mode} kind={kind}",
+                                 edges=edges, ngl=n_gl, averaged=bool(mode))
+            print(f"cheb N={N} ngl={n_gl} mode={mode} kind={kind} lJ={lJ}: H {r[0]:.1e} eig {r[1]:.1e} phase {r[2]:.1e} S {r[3]:.1e}")

@@ -680,3 +680,58 @@ def test_sigma_tot_wpcd_converges_to_MI():
         mean_err[N] = err.mean()
         assert np.median(err) < (2.0 if N == 32 else 1.0), (N, np.median(err))
     assert mean_err[64] < 0.7 * mean_err[32], mean_err
+
+
+# ---------------------------------------------------------------- NEXT-3: the paper's own discretisation (Eqs. 30-31)
+def test_chebyshev_grid_eq31():
+    N = 32
+    p = o.grid_chebyshev(N)                       # t = 2, alpha = 100 MeV
+    assert p[0] == 0.0 and (np.diff(p) > 0).all()
+    assert np.abs(p - inp.grid_chebyshev(N)).max() < 1e-13 * p[-1]
+    a = 100.0 / inp.HBARC
+    # hand values: j = 1 and the middle point j = (N+1)/2 -> tan(pi/4 + pi/(4N)...) ; t = 1 reduces to a plain tan grid
+    assert abs(p[1] - a * math.tan(math.pi / 128) ** 2) < 1e-16
+    assert abs(p[N] - a / math.tan(math.pi / 128) ** 2) < 1e-9 * p[N]      # tan(pi/2 - x) = 1/tan(x)
+    # symmetry of Eq. 31 about alpha: y_j y_{N+1-j} = alpha^2 for t-th powers of tan(x) tan(pi/2 - x) = 1
+    assert np.allclose(p[1:] * p[1:][::-1], a * a, rtol=1e-12)
+    p1 = o.grid_chebyshev(8, t=1.0, alpha=2.5)
+    assert np.allclose(p1[1:], 2.5 * np.tan((2 * np.arange(1, 9) - 1) * np.pi / 32), rtol=1e-14)
+
+
+def test_midpoint_potential_eq30_is_the_one_point_rule():
+    """Eq. 30: <x_i|v|x_j> ~ kbar_i kbar_j sqrt(Dk_i Dk_j) <kbar_i|v|kbar_j> with the convention-B
+    element <k'|v_l|k> = (1/pi) sum_t V0_t Q_l(z_t)/(k'k).  The n_gl = 1 Gauss-Legendre rule of Eq. 29 is exactly that."""
+    p = o.grid_chebyshev(12)
+    for l in (0, 2):
+        V = o.V_yukawa(p, l, inp.MT_V0, inp.MT_MU, ngl=1)
+        kb = 0.5 * (p[:-1] + p[1:]); dk = np.diff(p)
+        ref = np.empty_like(V)
+        for i in range(12):
+            for j in range(12):
+                el = sum(V0 * float(mp.legenq(l, 0, (kb[i] ** 2 + kb[j] ** 2 + m ** 2) / (2 * kb[i] * kb[j]), type=3).real)
+                         for V0, m in zip(inp.MT_V0, inp.MT_MU)) / (math.pi * kb[i] * kb[j])
+                ref[i, j] = kb[i] * kb[j] * math.sqrt(dk[i] * dk[j]) * el
+        assert np.abs(V - ref).max() < 1e-11 * np.abs(ref).max()
+    # and it approaches the 8-point bin average where the potential varies mildly over a bin (PAPER.md:227-229)
+    pf = inp.grid_edges(60)
+    V1, V8 = o.V_yukawa(pf, 0, inp.MT_V0, inp.MT_MU, ngl=1), o.V_yukawa(pf, 0, inp.MT_V0, inp.MT_MU, ngl=8)
+    assert np.abs(V1 - V8)[:30, :30].max() < 2e-3 * np.abs(V8)[:30, :30].max()
+
+
+def test_chebyshev_grid_chain_converges_to_MI():
+    """The paper's set-up (Chebyshev momentum bins, t = 2, alpha = 100 MeV) on the synthetic 1S0 potential: phase shifts
+    approach MI as N_WP grows over the paper's range 16..96, with Eq. 29 and with Eq. 30."""
+    tl = np.linspace(10.0, 340.0, 12); Ecm = tl / 2
+    exact = np.array([0.5 * math.degrees(math.atan2(S.imag, S.real)) for S in
+                      (o.mi_solve(t, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=0, NQ=96)[0] for t in tl)])
+    for ngl in (8, 1):
+        med = {}
+        for N in (16, 32, 96):
+            p = o.grid_chebyshev(N); e0, dE, Ee = o.fwp(p)
+            H, V = o.assemble_H(e0, o.V_yukawa(p, 0, inp.MT_V0, inp.MT_MU, ngl=ngl))
+            W, Cm, _ = o.jacobi(H)
+            T, b = o.onshell_T(N, 0, Ee, V, W, Cm, Ecm, averaged=True)
+            d, _ = o.phase_shifts(0, T, b, dE)
+            err = np.abs((d - exact + 90.0) % 180.0 - 90.0)
+            med[N] = np.median(err)
+        assert med[96] < med[32] < med[16] and med[96] < 2.0, (ngl, med)
