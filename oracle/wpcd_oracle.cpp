@@ -15,7 +15,9 @@
 //                      against numerical quadrature of the point-wise resolvent and the Yamaguchi closed form
 //   phases           : closed forms of Eqs. A.3-A.5 (unit-modulus S built from known angles)
 //   MI solver        : Yamaguchi analytic phase shifts; unitarity
-//   whole WPCD chain : converges to MI as N grows
+//   whole WPCD chain : converges to MI as N grows, also on the paper's Chebyshev grid (Eq. 31)
+//   sigma_tot        : Clebsch-Gordan vs sympy, Y_lm vs scipy, single-wave closed forms, partial-wave sum, optical
+//                      theorem (angular integral of Eq. A.6), Yamaguchi closed form, WPCD -> MI convergence
 //   The paper prints no matrix, eigenvalue or phase shift for a reproducible input (its potential, NNLO_opt, is
 //   not available), so no value of the chain is pinned to a PAPER-PRINTED number: "parity unpinned by the paper
 //   itself"; the pins above are closed forms / independent evaluations instead.
