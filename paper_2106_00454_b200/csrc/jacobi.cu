@@ -22,6 +22,7 @@
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
 #include <math.h>
+#include <type_traits>
 #include "jacobi_schedule.cuh"
 #include "wpcd_internal.cuh"
 
@@ -217,50 +218,64 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
   }
   bool doit = rotation(app, aqq, apq, tol2, c, s, t);
   bool any = false;
-  const int nrounds = need ? (full ? 15 : 8) : 0;
+  // The round loop, compiled twice: in the cross tournament the even positions never move, so the pivot's a_pp, the
+  // first Q column of a pair and the exceptions of positions 0 and 15 need no shuffle and no select.
+  auto rounds = [&](auto full_c) {
+    constexpr bool kFull = decltype(full_c)::value;
+    constexpr int nrounds = kFull ? 15 : 8;
+    const bool f0 = kFull && fix0, f7 = kFull && fix7;
 #pragma unroll 1
-  for (int r = 0; r < nrounds; ++r) {
-    const double2 a0 = *reinterpret_cast<const double2*>(ldA);
-    const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDS_);
-    const double2 b0 = *reinterpret_cast<const double2*>(ldB);
-    const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDS_);
-    __syncwarp();  // every lane has read its inputs before anybody stores
-    any |= doit;
-    const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
-    const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
-    const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
-    // block (k0, j)
-    const double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
-    const double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
-    const double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
-    const double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
-    // block (k0 + 4, j)
-    const double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
-    const double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
-    const double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
-    const double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
-    // next round's pivot by shuffle
-    const double zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
-    double appn = __shfl_sync(0xffffffffu, fix0 ? dbot : dtop, src_pp);
-    double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
-    const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
-    if (fix0) appn = dtop;
-    if (fix7) aqqn = dtop;
-    // this round's stores, at the positions of the next round
-    stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
-    stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
-    // Q <- Q R, then the columns move like the positions
+    for (int r = 0; r < nrounds; ++r) {
+      const double2 a0 = *reinterpret_cast<const double2*>(ldA);
+      const double2 a1 = *reinterpret_cast<const double2*>(ldA + LDS_);
+      const double2 b0 = *reinterpret_cast<const double2*>(ldB);
+      const double2 b1 = *reinterpret_cast<const double2*>(ldB + LDS_);
+      __syncwarp();  // every lane has read its inputs before anybody stores
+      any |= doit;
+      const double ca = __shfl_sync(0xffffffffu, c, k0), sa = __shfl_sync(0xffffffffu, s, k0);
+      const double cb = __shfl_sync(0xffffffffu, c, k0 + 4), sb = __shfl_sync(0xffffffffu, s, k0 + 4);
+      const double dtop = app - t * apq, dbot = aqq + t * apq;  // rotated diagonal of pair j (t = 0: unchanged)
+      // block (k0, j)
+      const double xa00 = c * a0.x - s * a0.y, xa01 = s * a0.x + c * a0.y;
+      const double xa10 = c * a1.x - s * a1.y, xa11 = s * a1.x + c * a1.y;
+      const double ya00 = ca * xa00 - sa * xa10, ya10 = sa * xa00 + ca * xa10;
+      const double ya01 = ca * xa01 - sa * xa11, ya11 = sa * xa01 + ca * xa11;
+      // block (k0 + 4, j)
+      const double xb00 = c * b0.x - s * b0.y, xb01 = s * b0.x + c * b0.y;
+      const double xb10 = c * b1.x - s * b1.y, xb11 = s * b1.x + c * b1.y;
+      const double yb00 = cb * xb00 - sb * xb10, yb10 = sb * xb00 + cb * xb10;
+      const double yb01 = cb * xb01 - sb * xb11, yb11 = sb * xb01 + cb * xb11;
+      // next round's pivot by shuffle
+      double zsel;
+      if (kFull) zsel = own_sel == 0 ? ya01 : (own_sel == 1 ? ya11 : (own_sel == 2 ? yb01 : yb00));
+      else zsel = own_sel == 0 ? ya01 : yb01;
+      double appn = dtop;
+      if (kFull) appn = __shfl_sync(0xffffffffu, f0 ? dbot : dtop, src_pp);
+      double aqqn = __shfl_sync(0xffffffffu, dbot, src_qq);
+      const double apqn = __shfl_sync(0xffffffffu, zsel, own_src);
+      if (f0) appn = dtop;
+      if (f7) aqqn = dtop;
+      // this round's stores, at the positions of the next round
+      stA0[cp] = ya00; stA0[cq] = ya01; stA1[cp] = ya10; stA1[cq] = ya11;
+      stB0[cp] = yb00; stB0[cq] = yb01; stB1[cp] = yb10; stB1[cq] = yb11;
+      // Q <- Q R, then the columns move like the positions
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const double nt = c * qt[u] - s * qb[u], nb = s * qt[u] + c * qb[u];
-      const double mt = __shfl_sync(0xffffffffu, fix0 ? nb : nt, grp | src_pp);
-      const double mb = __shfl_sync(0xffffffffu, nb, grp | src_qq);
-      qt[u] = fix0 ? nt : mt;
-      qb[u] = fix7 ? nt : mb;
+      for (int u = 0; u < 4; ++u) {
+        const double nt = c * qt[u] - s * qb[u], nb = s * qt[u] + c * qb[u];
+        double mt = nt;
+        if (kFull) mt = __shfl_sync(0xffffffffu, f0 ? nb : nt, grp | src_pp);
+        const double mb = __shfl_sync(0xffffffffu, nb, grp | src_qq);
+        qt[u] = f0 ? nt : mt;
+        qb[u] = f7 ? nt : mb;
+      }
+      app = appn; aqq = aqqn; apq = apqn;
+      doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
+      __syncwarp();
     }
-    app = appn; aqq = aqqn; apq = apqn;
-    doit = rotation(app, aqq, apq, tol2, c, s, t);  // independent of the stores above: overlaps them
-    __syncwarp();
+  };
+  if (need) {
+    if (full) rounds(std::true_type{});
+    else rounds(std::false_type{});
   }
   const bool anyw = __any_sync(0xffffffffu, any);
   if (anyw) {
