@@ -375,93 +375,49 @@ __device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* 
   else apply_tile_n<kHalf, 1, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
 }
 
-// V[rows of row-blocks rb0..rb1-1][P] <- V[..][P] Q
-// V[rows of row-blocks rbA, rbB][P] <- V[..][P] Q for exactly two row blocks: all four 16-byte loads are in flight
-// before the first product (V lives in global memory in every mode: L2 latency).
+// V[rows of the given row blocks][P] <- V[..][P] Q (V lives in global memory in every mode: L2 latency, so all loads of
+// a pair of row blocks are in flight before the first product).
+// One V item: row blocks rb[0..nrb-1] of V times the same Q, two row blocks at a time; the Q fragments are loaded once.
+// Items of 4 row blocks where A sits in shared memory (half the queue traffic and Q loads: n=200 6 % faster), 2 where A
+// goes through L2 as well (measured: 4 is 5 % slower at n=400).
+
 template <int nbk>
-__device__ __forceinline__ void apply_V_2(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                          int rbA, int rbB, int lane) {
+__device__ __forceinline__ void apply_V_item(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
+                                             const int* __restrict__ rb, int nrb, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int cb[2] = {I, J};
-  double* v0 = V + (size_t)(8 * rbA + g) * ld + 2 * t;
-  double* v1 = V + (size_t)(8 * rbB + g) * ld + 2 * t;
-  double2 f0[2], f1[2];
-#pragma unroll
-  for (int c = 0; c < nbk; ++c) {
-    f0[c] = *reinterpret_cast<const double2*>(v0 + 8 * cb[c]);
-    f1[c] = *reinterpret_cast<const double2*>(v1 + 8 * cb[c]);
-  }
   double2 bq[2][2];
 #pragma unroll
   for (int c = 0; c < nbk; ++c)
 #pragma unroll
     for (int r = 0; r < 2; ++r) bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
-  double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll 1
+  for (int k = 0; k < nrb; k += 2) {
+    const bool two = k + 1 < nrb;
+    double* v0 = V + (size_t)(8 * rb[k] + g) * ld + 2 * t;
+    double* v1 = V + (size_t)(8 * rb[two ? k + 1 : k] + g) * ld + 2 * t;
+    double2 f0[2], f1[2];
 #pragma unroll
-  for (int c = 0; c < nbk; ++c)
+    for (int c = 0; c < nbk; ++c) {
+      f0[c] = *reinterpret_cast<const double2*>(v0 + 8 * cb[c]);
+      f1[c] = *reinterpret_cast<const double2*>(v1 + 8 * cb[c]);
+    }
+    double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
-    for (int r = 0; r < 2; ++r)
+    for (int c = 0; c < nbk; ++c)
 #pragma unroll
-      for (int ni = 0; ni < nbk; ++ni) {
-        const double q = ni ? bq[c][r].y : bq[c][r].x;
-        dmma(o0[ni], r ? f0[c].y : f0[c].x, q);
-        dmma(o1[ni], r ? f1[c].y : f1[c].x, q);
-      }
+      for (int r = 0; r < 2; ++r)
 #pragma unroll
-  for (int ni = 0; ni < nbk; ++ni) {
-    *reinterpret_cast<double2*>(v0 + 8 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
-    *reinterpret_cast<double2*>(v1 + 8 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
-  }
-}
-
-template <int nbk>
-__device__ __forceinline__ void apply_V_n(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                          int rb0, int rb1, int lane) {
-  const int g = lane >> 2, t = lane & 3;
-  const int cb[2] = {I, J};
-  double2 bq[2][2];
+        for (int ni = 0; ni < nbk; ++ni) {
+          const double q = ni ? bq[c][r].y : bq[c][r].x;
+          dmma(o0[ni], r ? f0[c].y : f0[c].x, q);
+          dmma(o1[ni], r ? f1[c].y : f1[c].x, q);
+        }
 #pragma unroll
-  for (int c = 0; c < 2; ++c)
-#pragma unroll
-    for (int r = 0; r < 2; ++r)
-      if (c < nbk) bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
-  for (int rb = rb0; rb < rb1; ++rb) {
-    const int row = 8 * rb + g;
-    double2 vf[2];
-#pragma unroll
-    for (int c = 0; c < 2; ++c)
-      if (c < nbk) {
-        int col = 8 * cb[c] + 2 * t;
-        vf[c] = *reinterpret_cast<const double2*>(V + (size_t)row * ld + col);
-      }
-    double out[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
-#pragma unroll
-    for (int c = 0; c < 2; ++c)
-      if (c < nbk) {
-#pragma unroll
-        for (int r = 0; r < 2; ++r)
-#pragma unroll
-          for (int ni = 0; ni < 2; ++ni)
-            if (ni < nbk) dmma(out[ni], r ? vf[c].y : vf[c].x, ni ? bq[c][r].y : bq[c][r].x);
-      }
-#pragma unroll
-    for (int ni = 0; ni < 2; ++ni)
-      if (ni < nbk) {
-        int col = 8 * cb[ni] + 2 * t;
-        *reinterpret_cast<double2*>(V + (size_t)row * ld + col) = make_double2(out[ni][0], out[ni][1]);
-      }
-  }
-}
-
-// rbB < 0: a single row block
-__device__ __forceinline__ void apply_V(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
-                                        int rbA, int rbB, int lane) {
-  if (rbB >= 0) {
-    if (J >= 0) apply_V_2<2>(V, ld, Q, I, J, rbA, rbB, lane);
-    else apply_V_2<1>(V, ld, Q, I, J, rbA, rbB, lane);
-  } else {
-    if (J >= 0) apply_V_n<2>(V, ld, Q, I, J, rbA, rbA + 1, lane);
-    else apply_V_n<1>(V, ld, Q, I, J, rbA, rbA + 1, lane);
+    for (int ni = 0; ni < nbk; ++ni) {
+      *reinterpret_cast<double2*>(v0 + 8 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
+      if (two) *reinterpret_cast<double2*>(v1 + 8 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+    }
   }
 }
 
@@ -480,7 +436,6 @@ struct JacobiParams {
   double tol;
 };
 
-constexpr int kVRowBlocksPerItem = 2;
 
 // Schedule tables (one copy per launch, read through the L1): the tournament needs integer divisions that would
 // otherwise be redone for every work item.
@@ -621,6 +576,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   const int nact = sm.ctr[0];
   __syncthreads();
   const int ntiles = nslots * (nslots - 1) / 2;
+  constexpr int kVRowBlocksPerItem = (kMode == 1) ? 4 : 2;
   const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
   const int nitems = ntiles + nslots * nvgrp;
   const float rnvgrp = 1.0f / (float)nvgrp;
@@ -695,8 +651,10 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
             if (!rot[s]) continue;
             int I, J;
             decode_slot(tab_slot[s], I, J);
-            const int rbA = sm.act[2 * grp], rbB = 2 * grp + 1 < nact ? sm.act[2 * grp + 1] : -1;
-            apply_V(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, rbA, rbB, lane);
+            const int r0 = kVRowBlocksPerItem * grp;
+            const int nrb = nact - r0 < kVRowBlocksPerItem ? nact - r0 : kVRowBlocksPerItem;
+            if (J >= 0) apply_V_item<2>(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
+            else apply_V_item<1>(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
           }
         }
 #ifdef WPCD_PROFILE
