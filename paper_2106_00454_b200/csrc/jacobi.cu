@@ -166,19 +166,41 @@ template <bool kHalf>
 __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __restrict__ S, int I, int J, double tol,
                                             bool full, int lane) {
   constexpr int LDS_ = 16;  // S is the slot's 16 x LDQ array: a row = all 32 banks
-  for (int e = lane; e < 256; e += 32) {
-    const int a = e >> 4, b = e & 15;
-    const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c = 8 * ((b & 1) ? J : I) + (b >> 1);
-    S[a * LDS_ + b] = A.get(r, c);
-  }
-  __syncwarp();
   const int j = lane & 7, k0 = lane >> 3;
   const double tol2 = tol * tol;
   bool need = false;  // early exit: no pair of this sweep passes the rotation test (the usual case in the last sweeps)
-  for (int e = lane; e < 256; e += 32) {
-    const int a = e >> 4, b = e & 15;
-    const double x = S[a * LDS_ + b];
-    need |= (a < b) && (full || ((a ^ b) & 1)) && (x * x > tol2 * fabs(S[a * LDS_ + a] * S[b * LDS_ + b]));
+  // Lane (h = lane >> 4, gam = lane & 15) moves column gam of the rows 2k + h of S: always the same block of A.
+  const int h = lane >> 4, gam = lane & 15, bet = gam & 1;
+  if (kHalf) {
+    const int b = gam >> 1;
+    const double* src;
+    int stride = 8;
+    if (h == 0) src = A.p + A.blk(I, bet ? J : I) + b;                 // (I,I) or (I,J): element [k][b]
+    else if (bet) src = A.p + A.blk(J, J) + b;                          // (J,J)
+    else { src = A.p + A.blk(I, J) + 8 * b; stride = 1; }               // (J,I) = transpose of (I,J): element [b][k]
+#pragma unroll 4
+    for (int k = 0; k < 8; ++k) S[(2 * k + h) * LDS_ + gam] = src[k * stride];
+    __syncwarp();
+    const double dg = S[gam * (LDS_ + 1)];
+    const bool par = full || (h != bet);
+#pragma unroll 4
+    for (int k = 0; k < 8; ++k) {
+      const int rho = 2 * k + h;
+      const double x = S[rho * LDS_ + gam];
+      need |= par && (rho < gam) && (x * x > tol2 * fabs(S[rho * (LDS_ + 1)] * dg));
+    }
+  } else {
+    for (int e = lane; e < 256; e += 32) {
+      const int a = e >> 4, b = e & 15;
+      const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c = 8 * ((b & 1) ? J : I) + (b >> 1);
+      S[a * LDS_ + b] = A.get(r, c);
+    }
+    __syncwarp();
+    for (int e = lane; e < 256; e += 32) {
+      const int a = e >> 4, b = e & 15;
+      const double x = S[a * LDS_ + b];
+      need |= (a < b) && (full || ((a ^ b) & 1)) && (x * x > tol2 * fabs(S[a * LDS_ + a] * S[b * LDS_ + b]));
+    }
   }
   need = __any_sync(0xffffffffu, need);
   // static addresses: loads at (row pair, column pair), stores at the permuted positions
@@ -279,7 +301,9 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
   }
   const bool anyw = __any_sync(0xffffffffu, any);
   if (anyw) {
-    for (int e = lane; e < 256; e += 32) {  // symmetric write-back (upper triangle is the master copy)
+    // symmetric write-back (upper triangle of S is the master copy); a per-block variant like the load above was
+    // measured slower at n=200
+    for (int e = lane; e < 256; e += 32) {
       const int a = e >> 4, b = e & 15;
       const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c2 = 8 * ((b & 1) ? J : I) + (b >> 1);
       A.put(r, c2, a <= b ? S[a * LDS_ + b] : S[b * LDS_ + a]);
