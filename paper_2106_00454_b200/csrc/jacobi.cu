@@ -57,8 +57,14 @@ __device__ __forceinline__ int qrow(int k) { return (k & 8) | ((k & 1) << 2) | (
 
 // View of the symmetric working matrix A.
 //   kHalf = false: full np x ld array, XOR-swizzled, both triangles kept up to date (mirror stores).
-//   kHalf = true : only the blocks (rb <= cb) are stored, 64 contiguous doubles each (row-major 8x8); a block below the
-//                  diagonal is read/written through its transpose.  Halves the footprint: n = 200 fits shared memory.
+//   kHalf = true : only the blocks (rb <= cb) are stored, 64 contiguous doubles each; a block below the diagonal is
+//                  read/written through its transpose.  Halves the footprint: n = 200 fits shared memory.
+//                  Inside a block row r sits in row slot prow(r) = 0,4,1,5,2,6,3,7: a row is 8 doubles = half the
+//                  banks, and with this order the transposed fragment access (rows 2t resp. 2t+1, t = 0..3, column g)
+//                  spreads over both halves -- 2 wavefronts instead of 4-6 -- while the direct access stays
+//                  conflict free.
+__device__ __forceinline__ int prow(int r) { return ((r & 1) << 2) | (r >> 1); }
+
 template <bool kHalf>
 struct AView {
   double* p;
@@ -67,13 +73,13 @@ struct AView {
   __device__ __forceinline__ double get(int r, int c) const {
     if (!kHalf) return p[(size_t)r * ld + swz(r, c)];
     const int rb = r >> 3, cb = c >> 3;
-    return rb <= cb ? p[blk(rb, cb) + ((r & 7) << 3) + (c & 7)] : p[blk(cb, rb) + ((c & 7) << 3) + (r & 7)];
+    return rb <= cb ? p[blk(rb, cb) + (prow(r & 7) << 3) + (c & 7)] : p[blk(cb, rb) + (prow(c & 7) << 3) + (r & 7)];
   }
   // element (r,c) of a symmetric update where the caller visits BOTH (r,c) and (c,r)
   __device__ __forceinline__ void put(int r, int c, double v) const {
     if (!kHalf) { p[(size_t)r * ld + swz(r, c)] = v; return; }
     const int rb = r >> 3, cb = c >> 3;
-    if (rb <= cb) p[blk(rb, cb) + ((r & 7) << 3) + (c & 7)] = v;
+    if (rb <= cb) p[blk(rb, cb) + (prow(r & 7) << 3) + (c & 7)] = v;
   }
   // fragment of the off-diagonal block (rb != cb): rows 8rb+g, columns 8cb+2t, 8cb+2t+1
   __device__ __forceinline__ double2 load_frag(int rb, int cb, int g, int t) const {
@@ -81,9 +87,9 @@ struct AView {
       const int r = 8 * rb + g, c = 8 * cb + 2 * t;
       return *reinterpret_cast<const double2*>(p + (size_t)r * ld + swz(r, c));
     }
-    if (rb < cb) return *reinterpret_cast<const double2*>(p + blk(rb, cb) + (g << 3) + 2 * t);
-    const double* q = p + blk(cb, rb) + (t << 4) + g;
-    return make_double2(q[0], q[8]);
+    if (rb < cb) return *reinterpret_cast<const double2*>(p + blk(rb, cb) + (prow(g) << 3) + 2 * t);
+    const double* q = p + blk(cb, rb) + (t << 3) + g;  // rows 2t, 2t+1 of the stored block: slots t, 4+t
+    return make_double2(q[0], q[32]);
   }
   __device__ __forceinline__ void store_frag(int rb, int cb, int g, int t, double v0, double v1) const {
     if (!kHalf) {
@@ -93,9 +99,9 @@ struct AView {
       p[(size_t)(c + 1) * ld + swz(c + 1, r)] = v1;
       return;
     }
-    if (rb < cb) { *reinterpret_cast<double2*>(p + blk(rb, cb) + (g << 3) + 2 * t) = make_double2(v0, v1); return; }
-    double* q = p + blk(cb, rb) + (t << 4) + g;
-    q[0] = v0; q[8] = v1;
+    if (rb < cb) { *reinterpret_cast<double2*>(p + blk(rb, cb) + (prow(g) << 3) + 2 * t) = make_double2(v0, v1); return; }
+    double* q = p + blk(cb, rb) + (t << 3) + g;
+    q[0] = v0; q[32] = v1;
   }
 };
 
@@ -177,9 +183,9 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
     int stride = 8;
     if (h == 0) src = A.p + A.blk(I, bet ? J : I) + b;                 // (I,I) or (I,J): element [k][b]
     else if (bet) src = A.p + A.blk(J, J) + b;                          // (J,J)
-    else { src = A.p + A.blk(I, J) + 8 * b; stride = 1; }               // (J,I) = transpose of (I,J): element [b][k]
+    else { src = A.p + A.blk(I, J) + 8 * prow(b); stride = 1; }         // (J,I) = transpose of (I,J): element [b][k]
 #pragma unroll 4
-    for (int k = 0; k < 8; ++k) S[(2 * k + h) * LDS_ + gam] = src[k * stride];
+    for (int k = 0; k < 8; ++k) S[(2 * k + h) * LDS_ + gam] = src[(stride == 8 ? prow(k) : k) * stride];
     __syncwarp();
     const double dg = S[gam * (LDS_ + 1)];
     const bool par = full || (h != bet);
@@ -301,8 +307,6 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
   }
   const bool anyw = __any_sync(0xffffffffu, any);
   if (anyw) {
-    // symmetric write-back (upper triangle of S is the master copy); a per-block variant like the load above was
-    // measured slower at n=200
     for (int e = lane; e < 256; e += 32) {
       const int a = e >> 4, b = e & 15;
       const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c2 = 8 * ((b & 1) ? J : I) + (b >> 1);
