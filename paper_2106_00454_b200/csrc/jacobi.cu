@@ -795,8 +795,11 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.max_sweeps = max_sweeps;
   P.nranges = n_ranges;
   for (int r = 0; r < 4; ++r) { P.row_lo[r] = r < n_ranges ? h_rows[2 * r] : 0; P.row_hi[r] = r < n_ranges ? h_rows[2 * r + 1] : 0; }
-  // about four full pivot sweeps per sweep of the tournament (measured: fewer cost extra sweeps, more cost pivot time)
-  P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
+  // full pivot sweeps per sweep of the tournament (measured: fewer cost extra sweeps, more cost pivot time): about three
+  // on the shared-memory path (n = 75 .. 300: periods 5, 5, 7, 9, 13 are the measured optima), about four where A goes
+  // through L2 (n = 400: 13 beats 17)
+  if (g.mode == 1) P.full_every = (g.m - 1 + 2) / 3 > 5 ? (g.m - 1 + 2) / 3 : 5;
+  else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   const int grid = global_grid(h, g, batch);
   if (work_bytes < g.tab_bytes + (size_t)grid * g.gstride * 8) return WPCD_EWORK;
