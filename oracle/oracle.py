@@ -26,6 +26,9 @@ _gl = _sig("orc_gl_rule", None, [_i, _pd, _pd])
 _Q = _sig("orc_legendre_Q", _d, [_i, _d])
 _grid = _sig("orc_grid_tan", None, [_i, _d, _pd])
 _gridc = _sig("orc_grid_chebyshev", None, [_i, _d, _d, _pd])
+_fwpE = _sig("orc_fwp_energy", None, [_i, _pd, _d, _d, _pd, _pd, _pd])
+_VyukE = _sig("orc_V_yukawa_energy", None, [_i, _pd, _i, _i, _pd, _pd, _i, _d, _d, _pd])
+_VyamE = _sig("orc_V_yamaguchi_energy", None, [_i, _pd, _d, _d, _i, _d, _d, _pd, _pd])
 _fwp = _sig("orc_fwp", None, [_i, _pd, _d, _d, _pd, _pd, _pd])
 _Vyuk = _sig("orc_V_yukawa", None, [_i, _pd, _i, _i, _pd, _pd, _i, _pd])
 _Vyam = _sig("orc_V_yamaguchi", None, [_i, _pd, _d, _d, _i, _i, _pd, _pd])
@@ -83,19 +86,30 @@ def grid_chebyshev(N, t=2.0, alpha=100.0 / HBARC):
     return p
 
 
-def fwp(p, hbarc=HBARC, mu=MU):
+def fwp(p, hbarc=HBARC, mu=MU, energy_packets=False):
+    """FWP kinetic energies, bin energy widths and energy edges; energy_packets: f = sqrt(k/mu), N_i = dE_i (Eq. 18)."""
     p = _f(p); N = len(p) - 1
     e0 = np.empty(N); dE = np.empty(N); Ee = np.empty(N + 1)
-    _fwp(N, p, hbarc, mu, e0, dE, Ee)
+    (_fwpE if energy_packets else _fwp)(N, p, hbarc, mu, e0, dE, Ee)
     return e0, dE, Ee
 
 
-def V_yukawa(p, l, V0, mu, ngl=8):
+def V_yukawa(p, l, V0, mu, ngl=8, energy_packets=False, hbarc=HBARC, mured=MU):
     p = _f(p); N = len(p) - 1
     V0 = _f(np.atleast_1d(V0)); mu = _f(np.atleast_1d(mu))
     V = np.empty((N, N))
-    _Vyuk(N, p, int(l), len(V0), V0, mu, ngl, V)
+    if energy_packets:
+        _VyukE(N, p, int(l), len(V0), V0, mu, ngl, hbarc, mured, V)
+    else:
+        _Vyuk(N, p, int(l), len(V0), V0, mu, ngl, V)
     return V
+
+
+def V_yamaguchi_energy(p, lambdaB, beta, ngl=8, hbarc=HBARC, mured=MU):
+    p = _f(p); N = len(p) - 1
+    V = np.empty((N, N)); G = np.empty(N)
+    _VyamE(N, p, lambdaB, beta, ngl, hbarc, mured, V, G)
+    return V, G
 
 
 def V_yamaguchi(p, lambdaB, beta, ngl=8, closed_form=True):

@@ -198,6 +198,69 @@ void orc_V_yamaguchi(int N, const double* p, double lambdaB, double beta, int ng
     for (int j = 0; j < N; ++j) V[i * N + j] = -lambdaB * G[i] * G[j];
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-4: ENERGY wave packets, Eq. 17 with the weighting function f(k) = hbarc sqrt(k/mu) (PAPER.md:143:
+// "sqrt(k/mu)", hbar restored so that k dk f^2 = k dE) and N_i = Delta E_i.
+//   <x_i|h0|x_i> = (1/dE_i) int_{D_i} E dE = E_i + dE_i/2                       -- Eq. 18, exact for these packets
+//   <x_i|v|x_j>  = (1/sqrt(dE_i dE_j)) int int k'k dk'dk f(k')f(k) <k'|v|k>      -- Eq. 29
+//               = (hbarc^2/(pi mu sqrt(dE_i dE_j))) sum_ab w_ia w_jb sqrt(k_ia k_jb) sum_t V0_t Q_l(z_t)   (Yukawa)
+// The S-matrix relation S = 1 - 2 pi i T_ii/dE_i (reading C2) holds for them at every q of the bin: Eq. 20 gives
+// <E|T|E> = (mu q/hbarc^2) f(q)^2/(N_i q^2) T_ii = T_ii/dE_i.  Steps (ii)-(v) are unchanged.
+void orc_fwp_energy(int N, const double* p, double hbarc, double mu, double* e0, double* dE, double* Eedge) {
+  double cE = hbarc * hbarc / (2.0 * mu);
+  for (int i = 0; i <= N; ++i) Eedge[i] = cE * p[i] * p[i];
+  for (int i = 0; i < N; ++i) {
+    dE[i] = Eedge[i + 1] - Eedge[i];
+    e0[i] = Eedge[i] + 0.5 * dE[i];
+  }
+}
+
+void orc_V_yukawa_energy(int N, const double* p, int l, int nterms, const double* V0, const double* mu, int ngl,
+                         double hbarc, double mured, double* V) {
+  std::vector<double> x(ngl), w(ngl);
+  orc_gl_rule(ngl, x.data(), w.data());
+  double cE = hbarc * hbarc / (2.0 * mured);
+  for (int i = 0; i < N; ++i)
+    for (int j = i; j < N; ++j) {
+      double dki = p[i + 1] - p[i], dkj = p[j + 1] - p[j];
+      double acc = 0.0;
+      for (int a = 0; a < ngl; ++a)
+        for (int b = 0; b < ngl; ++b) {
+          double kp = 0.5 * (p[i] + p[i + 1]) + 0.5 * dki * x[a], kk = 0.5 * (p[j] + p[j + 1]) + 0.5 * dkj * x[b];
+          double s = 0.0;
+          for (int t = 0; t < nterms; ++t) {
+            double z, zm1;
+            yukawa_z(kp, kk, mu[t], &z, &zm1);
+            s += V0[t] * orc_legendre_Qz(l, z, zm1);
+          }
+          // k'k dk'dk f(k')f(k) <k'|v|k> = (hbarc^2/mu) sqrt(k'k) (1/pi) s dk'dk
+          acc += (0.5 * dki * w[a]) * (0.5 * dkj * w[b]) * std::sqrt(kp * kk) * s;
+        }
+      double dEi = cE * (p[i + 1] * p[i + 1] - p[i] * p[i]), dEj = cE * (p[j + 1] * p[j + 1] - p[j] * p[j]);
+      double v = hbarc * hbarc / mured * acc / (PI * std::sqrt(dEi * dEj));
+      V[i * N + j] = v;
+      V[j * N + i] = v;
+    }
+}
+
+// Yamaguchi with energy packets: V_ij = -lambdaB G_i G_j, G_i = dE_i^{-1/2} int_{D_i} k f(k) g(k) dk by n_gl-point GL.
+void orc_V_yamaguchi_energy(int N, const double* p, double lambdaB, double beta, int ngl, double hbarc, double mured,
+                            double* V, double* G) {
+  std::vector<double> x(ngl), w(ngl);
+  orc_gl_rule(ngl, x.data(), w.data());
+  double cE = hbarc * hbarc / (2.0 * mured);
+  for (int i = 0; i < N; ++i) {
+    double dk = p[i + 1] - p[i], acc = 0.0;
+    for (int a = 0; a < ngl; ++a) {
+      double k = 0.5 * (p[i] + p[i + 1]) + 0.5 * dk * x[a];
+      acc += 0.5 * dk * w[a] * k * (hbarc * std::sqrt(k / mured)) / (k * k + beta * beta);
+    }
+    G[i] = acc / std::sqrt(cE * (p[i + 1] * p[i + 1] - p[i] * p[i]));
+  }
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) V[i * N + j] = -lambdaB * G[i] * G[j];
+}
+
 // H = H0 + V.  Uncoupled: n = N, H = diag(e0) + Vmm.  Coupled (degenerate FWP bases,
 // the same H0 in both blocks): n = 2N, H = [[H0 + Vmm, Vmp],[Vmp^T, H0 + Vpp]].  Also returns V (same layout).
 void orc_assemble_H(int N, int coupled, const double* e0, const double* Vmm, const double* Vpp, const double* Vmp,

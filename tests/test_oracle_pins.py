@@ -735,3 +735,64 @@ def test_chebyshev_grid_chain_converges_to_MI():
             err = np.abs((d - exact + 90.0) % 180.0 - 90.0)
             med[N] = np.median(err)
         assert med[96] < med[32] < med[16] and med[96] < 2.0, (ngl, med)
+
+
+# ---------------------------------------------------------------- NEXT-4: energy wave packets (Eqs. 17-18)
+def test_energy_packets_h0_and_potential_vs_adaptive_integrals():
+    p = np.array([0.4, 0.9, 1.5, 2.4])
+    cE = inp.HBARC ** 2 / (2 * inp.MU)
+    e0, dE, Ee = o.fwp(p, energy_packets=True)
+    f = lambda k: inp.HBARC * math.sqrt(k / inp.MU)          # weighting function of the energy packets
+    for i in range(3):
+        # normalisation N_i = dE_i:  int k dk f(k) int k' dk' f(k') delta(k-k')/(k k') = int f^2 dk
+        nrm, _ = integrate.quad(lambda k: f(k) ** 2, p[i], p[i + 1])
+        assert abs(nrm - dE[i]) < 1e-12 * dE[i]
+        # Eq. 18: <x_i|h0|x_i> = (1/N_i) int f^2 cE k^2 dk = E_i + dE_i/2
+        val, _ = integrate.quad(lambda k: f(k) ** 2 * cE * k * k, p[i], p[i + 1])
+        assert abs(e0[i] - val / dE[i]) < 1e-12 * e0[i] and abs(e0[i] - (Ee[i] + 0.5 * dE[i])) < 1e-13 * e0[i]
+    for l in (0, 2):
+        V = o.V_yukawa(p, l, energy_packets=True, **MT)
+        assert np.array_equal(V, V.T)
+        for i, j in [(0, 0), (0, 2), (1, 2)]:
+            def integrand(k, kp):     # k'k f(k')f(k) <k'|v_l|k>_B
+                s = sum(V0 * float(mp.legenq(l, 0, (kp * kp + k * k + mu * mu) / (2 * kp * k), type=3).real)
+                        for V0, mu in zip(inp.MT_V0, inp.MT_MU))
+                return f(kp) * f(k) * s / math.pi
+            val, _ = integrate.dblquad(integrand, p[i], p[i + 1], p[j], p[j + 1], epsabs=1e-10, epsrel=1e-10)
+            ref = val / math.sqrt(dE[i] * dE[j])
+            assert abs(V[i, j] - ref) < 2e-6 * abs(ref), (l, i, j, V[i, j], ref)
+    # Yamaguchi form factor G_i = dE_i^{-1/2} int k f(k) g(k) dk
+    lamA, lamB = inp.yamaguchi_lambda()
+    V, G = o.V_yamaguchi_energy(p, lamB, inp.YAMAGUCHI_BETA)
+    for i in range(3):
+        val, _ = integrate.quad(lambda k: k * f(k) / (k * k + inp.YAMAGUCHI_BETA ** 2), p[i], p[i + 1])
+        assert abs(G[i] - val / math.sqrt(dE[i])) < 1e-10 * abs(G[i])
+    assert np.allclose(V, -lamB * np.outer(G, G), rtol=1e-15)
+
+
+def test_energy_packets_chain_agrees_with_momentum_packets_and_MI():
+    """"we have implemented energy as well as momentum wave-packets, and have found no significant
+    difference": the two bases give the same narrow-bin matrix elements, phase shifts that differ by less than the
+    method error, and both approach MI / the Yamaguchi closed form as N grows."""
+    p = inp.grid_edges(60)
+    Vk = o.V_yukawa(p, 0, **MT); Ve = o.V_yukawa(p, 0, energy_packets=True, **MT)
+    assert np.abs(Vk - Ve)[8:30, 8:30].max() < 5e-4 * np.abs(Vk)[8:30, 8:30].max()
+    tl = np.linspace(10.0, 340.0, 12); Ecm = tl / 2
+    lamA, lamB = inp.yamaguchi_lambda()
+    exact = np.array([0.5 * math.degrees(math.atan2(S.imag, S.real)) for S in map(_yamaguchi_S_exact, tl)])
+    med = {}
+    for N in (50, 200):
+        p = inp.grid_edges(N)
+        d = {}
+        for ep in (False, True):
+            e0, dE, Ee = o.fwp(p, energy_packets=ep)
+            V = o.V_yamaguchi_energy(p, lamB, inp.YAMAGUCHI_BETA)[0] if ep else o.V_yamaguchi(p, lamB, inp.YAMAGUCHI_BETA)[0]
+            H, Vf = o.assemble_H(e0, V)
+            W, Cm, _ = o.jacobi(H)
+            T, b = o.onshell_T(N, 0, Ee, Vf, W, Cm, Ecm, averaged=True)
+            d[ep], _ = o.phase_shifts(0, T, b, dE)
+        err = {ep: np.abs((d[ep] - exact + 90.0) % 180.0 - 90.0) for ep in d}
+        med[N] = np.median(err[True])
+        # no significant difference: the two bases differ by less than either differs from the exact result
+        assert np.abs((d[True] - d[False] + 90.0) % 180.0 - 90.0).max() < max(err[True].max(), err[False].max())
+    assert med[200] < 0.5 * med[50] and med[200] < 0.3, med
