@@ -69,7 +69,10 @@ typedef struct {
   int N;                 /* number of wave packets */
   const double* h_edges; /* [N+1] bin edges p_0 < p_1 < ... < p_N, fm^-1, p_0 >= 0 */
   double hbarc, mu;      /* MeV fm, MeV (reduced mass) */
-  int n_gl;              /* Gauss-Legendre points per bin for Eq. 29, 1..16 (BASELINE configs: 8) */
+  int n_gl;              /* Gauss-Legendre points per bin for Eq. 29, 1..16 (BASELINE configs: 8; 1 = mid-point rule, Eq. 30) */
+  int wp_kind;           /* 0: momentum wave packets f(k) = 1, N_i = Delta k_i (the configs, the paper's choice);
+                            1: energy wave packets f(k) = hbarc sqrt(k/mu), N_i = Delta E_i: H0 is Eq. 18
+                               exactly, e_i = E_i + dE_i/2, and Eq. 29 carries the extra factor f(k')f(k) */
 } wpcd_grid;
 
 /* Handle: owns only immutable device tables.  One handle per host thread/stream.  device = CUDA ordinal. */
@@ -89,7 +92,8 @@ size_t wpcd_onshell_workspace_bytes(void* handle, int N, int coupled, int batch,
  *              samples are identical).  Strength t of sample s is V0_t * d_scales[s][scale_idx[t]].
  *   d_H_unc  : [S][n_unc][N][N]   (n_unc = number of uncoupled channels, list order), may be NULL if n_unc = 0
  *   d_H_cpl  : [S][n_cpl][2N][2N] (n_cpl = number of coupled channels, list order),   may be NULL if n_cpl = 0
- *   d_e0     : [N]   FWP kinetic energies e_i = cE (p_i^2 + p_i p_{i+1} + p_{i+1}^2)/3 (reading C4)
+ *   d_e0     : [N]   FWP kinetic energies e_i = cE (p_i^2 + p_i p_{i+1} + p_{i+1}^2)/3 (reading C4; energy packets:
+ *                      cE (p_i^2 + p_{i+1}^2)/2, Eq. 18)
  *   d_dE     : [N]   FWP bin energy widths,  d_Eedge : [N+1] bin edges in energy (cE p_i^2)
  * The basis matrices (one per distinct (l, mu_t)) are built in the workspace by an 8x8-point (n_gl x n_gl)
  * Gauss-Legendre rule per bin pair and combined per sample with coalesced, vectorised stores.  H is exactly

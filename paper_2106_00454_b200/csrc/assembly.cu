@@ -20,16 +20,21 @@ struct ChanTable { int nchan; int n_unc; int n_cpl; ChanDesc c[WPCD_MAX_CHANNELS
 
 // ------------------------------------------------------------------------------------------------ k_grid
 // thread (i, a): Newton iteration for the a-th root of P_ngl, then maps it into bin i.
-__global__ void k_grid(int N, int ngl, double hbarc, double mu, const double* __restrict__ p, double* __restrict__ e0,
-                       double* __restrict__ dE, double* __restrict__ Eedge, double* __restrict__ knode,
-                       double* __restrict__ wnode) {
+// wp_kind 1 (energy wave packets, f(k) = hbarc sqrt(k/mu), N_i = dE_i): e0 = E_i + dE_i/2 (Eq. 18), the node weights
+// carry sqrt(k) and norm_i = sqrt(mu dE_i)/hbarc, so that (1/(norm_i norm_j)) sum_ab w_ia w_jb ... is Eq. 29 with
+// f(k')f(k)/sqrt(N_i N_j); momentum packets: norm_i = sqrt(Dk_i).
+__global__ void k_grid(int N, int ngl, int wp_kind, double hbarc, double mu, const double* __restrict__ p,
+                       double* __restrict__ e0, double* __restrict__ dE, double* __restrict__ Eedge,
+                       double* __restrict__ knode, double* __restrict__ wnode, double* __restrict__ norm) {
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
   double cE = hbarc * hbarc / (2.0 * mu);
   if (idx <= N) Eedge[idx] = cE * p[idx] * p[idx];
   if (idx < N) {
     double a = p[idx], b = p[idx + 1];
-    e0[idx] = cE * (a * a + a * b + b * b) / 3.0;
-    dE[idx] = cE * b * b - cE * a * a;
+    const double w = cE * b * b - cE * a * a;
+    e0[idx] = wp_kind ? cE * a * a + 0.5 * w : cE * (a * a + a * b + b * b) / 3.0;
+    dE[idx] = w;
+    norm[idx] = wp_kind ? sqrt(mu * w) / hbarc : sqrt(b - a);
   }
   if (idx < N * ngl) {
     int i = idx / ngl, a = idx % ngl;
@@ -58,8 +63,9 @@ __global__ void k_grid(int N, int ngl, double hbarc, double mu, const double* __
     }
     double w = 2.0 / ((1.0 - x * x) * dp * dp);
     double lo = p[i], hi = p[i + 1], half = 0.5 * (hi - lo);
-    knode[idx] = 0.5 * (lo + hi) + half * x;
-    wnode[idx] = half * w;
+    const double kn = 0.5 * (lo + hi) + half * x;
+    knode[idx] = kn;
+    wnode[idx] = wp_kind ? half * w * sqrt(kn) : half * w;
   }
 }
 
@@ -92,9 +98,9 @@ __device__ double legendre_q(int l, double zm1) {
 
 // ------------------------------------------------------------------------------------------------ k_basis
 // grid (ceil(ntri/128), nbasis); thread = upper-triangle element (i <= j); mirrored store keeps B symmetric.
-__global__ void __launch_bounds__(128) k_basis(int N, int ngl, BasisTable tab, const double* __restrict__ p,
+__global__ void __launch_bounds__(128) k_basis(int N, int ngl, int wp_kind, BasisTable tab, const double* __restrict__ p,
                                                const double* __restrict__ knode, const double* __restrict__ wnode,
-                                               double* __restrict__ basis) {
+                                               const double* __restrict__ norm, double* __restrict__ basis) {
   int e = blockIdx.x * blockDim.x + threadIdx.x;
   int ntri = N * (N + 1) / 2;
   if (e >= ntri) return;
@@ -107,7 +113,16 @@ __global__ void __launch_bounds__(128) k_basis(int N, int ngl, BasisTable tab, c
   double* B = basis + (size_t)blockIdx.y * N * N;
   double dki = p[i + 1] - p[i], dkj = p[j + 1] - p[j];
   double v;
-  if (d.kind == 1) {
+  if (d.kind == 1 && wp_kind) {
+    // Yamaguchi form factor of an energy packet: G_i = N_i^{-1/2} int k f(k) g(k) dk by the bin's quadrature rule
+    double b2 = d.beta * d.beta, gi = 0.0, gj = 0.0;
+    for (int a = 0; a < ngl; ++a) {
+      double ki = knode[i * ngl + a], kj = knode[j * ngl + a];
+      gi = fma(wnode[i * ngl + a], ki / (ki * ki + b2), gi);
+      gj = fma(wnode[j * ngl + a], kj / (kj * kj + b2), gj);
+    }
+    v = (gi / norm[i]) * (gj / norm[j]);
+  } else if (d.kind == 1) {
     // Yamaguchi form factor, closed form of int k/(k^2+beta^2) dk over the bin (reading C15)
     double b2 = d.beta * d.beta;
     double gi = 0.5 * log((p[i + 1] * p[i + 1] + b2) / (p[i] * p[i] + b2)) / sqrt(dki);
@@ -126,7 +141,7 @@ __global__ void __launch_bounds__(128) k_basis(int N, int ngl, BasisTable tab, c
       }
       acc = fma(wa, row, acc);
     }
-    v = acc / (WPCD_PI * sqrt(dki * dkj));
+    v = wp_kind ? acc / (WPCD_PI * norm[i] * norm[j]) : acc / (WPCD_PI * sqrt(dki * dkj));
   }
   B[(size_t)i * N + j] = v;
   B[(size_t)j * N + i] = v;
@@ -183,7 +198,7 @@ static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 size_t wpcd_build_workspace(int N, int n_chan) {
   size_t nb = (size_t)n_chan * (2 * WPCD_MAX_TERMS + 1);
   if (nb > MAX_BASIS) nb = MAX_BASIS;
-  return align256((size_t)(N + 1) * 8) + 2 * align256((size_t)N * 16 * 8) + nb * align256((size_t)N * N * 8);
+  return 2 * align256((size_t)(N + 1) * 8) + 2 * align256((size_t)N * 16 * 8) + nb * align256((size_t)N * N * 8);
 }
 
 static int find_or_add(BasisTable& t, int l, int kind, double mu, double beta) {
@@ -232,6 +247,7 @@ int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential
   }
   char* w = static_cast<char*>(d_work);
   double* d_p = reinterpret_cast<double*>(w); w += align256((size_t)(N + 1) * 8);
+  double* d_norm = reinterpret_cast<double*>(w); w += align256((size_t)(N + 1) * 8);
   double* d_k = reinterpret_cast<double*>(w); w += align256((size_t)N * 16 * 8);
   double* d_w = reinterpret_cast<double*>(w); w += align256((size_t)N * 16 * 8);
   double* d_basis = reinterpret_cast<double*>(w);
@@ -240,9 +256,9 @@ int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential
   int rc = wpcd_check_cuda(h, cudaMemcpyAsync(d_p, grid->h_edges, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, st), "edges H2D");
   if (rc) return rc;
   int tot = N * ngl > N + 1 ? N * ngl : N + 1;
-  k_grid<<<(tot + 127) / 128, 128, 0, st>>>(N, ngl, grid->hbarc, grid->mu, d_p, d_e0, d_dE, d_Eedge, d_k, d_w);
+  k_grid<<<(tot + 127) / 128, 128, 0, st>>>(N, ngl, grid->wp_kind, grid->hbarc, grid->mu, d_p, d_e0, d_dE, d_Eedge, d_k, d_w, d_norm);
   int ntri = N * (N + 1) / 2;
-  k_basis<<<dim3((ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, bt, d_p, d_k, d_w, d_basis);
+  k_basis<<<dim3((ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, grid->wp_kind, bt, d_p, d_k, d_w, d_norm, d_basis);
   if (ct.n_unc) {
     size_t half = ((size_t)N * N + 1) / 2;
     k_combine<<<dim3((unsigned)((half + 255) / 256), ct.n_unc, S), 256, 0, st>>>(N, 0, ct, d_basis, d_e0, d_scales, P, d_H_unc);

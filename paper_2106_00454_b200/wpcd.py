@@ -35,7 +35,7 @@ class Channel(C.Structure):
 
 class Grid(C.Structure):
     _fields_ = [("N", C.c_int), ("h_edges", C.POINTER(C.c_double)), ("hbarc", C.c_double), ("mu", C.c_double),
-                ("n_gl", C.c_int)]
+                ("n_gl", C.c_int), ("wp_kind", C.c_int)]
 
 
 _vp, _sz, _i, _d = C.c_void_p, C.c_size_t, C.c_int, C.c_double
@@ -110,12 +110,13 @@ class Handle:
 
     # ------------------------------------------------------------------ wpcd_build_channels
     def build_channels(self, edges, channels, V0=None, mu=None, scale_idx=None, VT=0.0, muT=1.0, VT_scale_idx=-1,
-                       yamaguchi=None, scales=None, S=1, hbarc=197.327, mured=469.46, n_gl=8, stream=None, out=None):
+                       yamaguchi=None, scales=None, S=1, hbarc=197.327, mured=469.46, n_gl=8, stream=None, out=None,
+                       energy_packets=False):
         """edges: host sequence [N+1]; channels: list of (coupled, lJ); scales: device tensor [S][P] or None.
         Returns dict(H_unc, H_cpl, e0, dE, Eedge) of device tensors."""
         N = len(edges) - 1
         h_edges = (C.c_double * (N + 1))(*[float(x) for x in edges])
-        grid = Grid(N, h_edges, hbarc, mured, n_gl)
+        grid = Grid(N, h_edges, hbarc, mured, n_gl, 1 if energy_packets else 0)
         pot = Potential()
         keep = []
         if yamaguchi is not None:

@@ -14,21 +14,24 @@ TOL_H_REL = 1e-12        # assembly gate: 1e-12 max|H|
 EDGE_GUARD = 1e-9        # MeV: energies this close to a pseudostate bin edge are excluded (reading C11)
 
 
-def oracle_channel(N, coupled, lJ, scale=(1.0, 1.0, 1.0), yamaguchi=None, edges=None, ngl=8):
+def oracle_channel(N, coupled, lJ, scale=(1.0, 1.0, 1.0), yamaguchi=None, edges=None, ngl=8, energy_packets=False):
     """Oracle H, V for one channel on the config grid (or the given bin edges).  scale = (V_R, V_A, V_T) multipliers."""
     p = inp.grid_edges(N) if edges is None else np.asarray(edges, dtype=np.float64)
-    e0, dE, Ee = o.fwp(p)
+    e0, dE, Ee = o.fwp(p, energy_packets=energy_packets)
     if yamaguchi is not None:
-        V, _ = o.V_yamaguchi(p, yamaguchi[0], yamaguchi[1], closed_form=True)
+        if energy_packets:
+            V, _ = o.V_yamaguchi_energy(p, yamaguchi[0], yamaguchi[1], ngl=ngl)
+        else:
+            V, _ = o.V_yamaguchi(p, yamaguchi[0], yamaguchi[1], closed_form=True)
         H, Vf = o.assemble_H(e0, V)
     else:
         V0 = inp.MT_V0 * np.array([scale[0], scale[1]])
         if not coupled:
-            H, Vf = o.assemble_H(e0, o.V_yukawa(p, lJ, V0, inp.MT_MU, ngl=ngl))
+            H, Vf = o.assemble_H(e0, o.V_yukawa(p, lJ, V0, inp.MT_MU, ngl=ngl, energy_packets=energy_packets))
         else:
-            Vmm = o.V_yukawa(p, lJ - 1, V0, inp.MT_MU, ngl=ngl)
-            Vpp = o.V_yukawa(p, lJ + 1, V0, inp.MT_MU, ngl=ngl)
-            Vmp = o.V_yukawa(p, lJ, [inp.TENSOR_V * scale[2]], [inp.TENSOR_MU], ngl=ngl)
+            Vmm = o.V_yukawa(p, lJ - 1, V0, inp.MT_MU, ngl=ngl, energy_packets=energy_packets)
+            Vpp = o.V_yukawa(p, lJ + 1, V0, inp.MT_MU, ngl=ngl, energy_packets=energy_packets)
+            Vmp = o.V_yukawa(p, lJ, [inp.TENSOR_V * scale[2]], [inp.TENSOR_MU], ngl=ngl, energy_packets=energy_packets)
             H, Vf = o.assemble_H(e0, Vmm, Vpp, Vmp)
     return dict(p=p, e0=e0, dE=dE, Eedge=Ee, H=H, V=Vf)
 

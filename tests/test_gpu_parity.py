@@ -24,7 +24,8 @@ def _to_dev(ctx, a, dtype=None):
     return t if dtype is None else t.to(dtype)
 
 
-def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0.0, edges=None, n_gl=8, mode=0):
+def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0.0, edges=None, n_gl=8, mode=0,
+                  energy_packets=False):
     """Full hot path on the GPU for a channel list; returns per-kind dicts of numpy arrays."""
     h, torch = ctx["h"], ctx["torch"]
     p = inp.grid_edges(N) if edges is None else edges
@@ -32,7 +33,7 @@ def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0
     kw = dict(yamaguchi=yamaguchi) if yamaguchi is not None else dict(
         V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1] if scales is not None else None, VT=inp.TENSOR_V,
         muT=inp.TENSOR_MU, VT_scale_idx=2 if scales is not None else -1)
-    out = h.build_channels(p, channels, scales=d_scales, S=S, n_gl=n_gl, **kw)
+    out = h.build_channels(p, channels, scales=d_scales, S=S, n_gl=n_gl, energy_packets=energy_packets, **kw)
     d_E = _to_dev(ctx, Ecm)
     res = {}
     for kind, key in ((0, "H_unc"), (1, "H_cpl")):
@@ -56,8 +57,8 @@ def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0
 
 
 def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguchi=None, label="", edges=None, ngl=8,
-                     averaged=False):
-    ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi, edges=edges, ngl=ngl)
+                     averaged=False, energy_packets=False):
+    ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi, edges=edges, ngl=ngl, energy_packets=energy_packets)
     ref = hp.oracle_solve(N, kind, ch, Ecm, averaged=averaged)
     g = res[kind]
     n = ch["H"].shape[0]
@@ -81,6 +82,19 @@ def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguc
     assert np.array_equal(g["bin"], ref["bin"]), (label, "bins")
     dphi, dS, nok = hp.check_phases(kind, g["delta"][s, c], g["S"][s, c], ref, Ecm)
     assert nok > 0.9 * len(Ecm)
+    if dphi > hp.TOL_PHASE_DEG or dS > hp.TOL_S_ABS:
+        # DESIGN.md section 3 "arbitration": the fp64 oracle stops on a NORM-wise criterion (off(A) <= 1e-15 ||A||_F), so on
+        # grids where ||H|| is 1e9 MeV (the paper's Chebyshev bins at N = 100) its small eigenpairs carry a relative error
+        # that the log-singular resolvent amplifies near a bin edge.  The same chain with the eigenpairs of the oracle's
+        # 80-bit Jacobi run (T and phases still fp64) decides.
+        from oracle import oracle as o
+        W_ld, C_ld, _ = o.jacobi_ld(ch["H"])
+        T_ld, b_ld = o.onshell_T(N, kind, ch["Eedge"], ch["V"], W_ld, C_ld, Ecm, averaged=averaged)
+        d_ld, S_ld = o.phase_shifts(kind, T_ld, b_ld, ch["dE"])
+        ref_ld = dict(ref, W=W_ld, delta=d_ld, S=S_ld, bin=b_ld)
+        dphi_o, dS_o, _ = hp.check_phases(kind, ref["delta"], ref["S"], ref_ld, Ecm)
+        dphi, dS, nok = hp.check_phases(kind, g["delta"][s, c], g["S"][s, c], ref_ld, Ecm)
+        print(label, "phase arbitration vs long-double eigenpairs: gpu", dphi, dS, "fp64 oracle", dphi_o, dS_o)
     assert dphi <= hp.TOL_PHASE_DEG, (label, "phase", dphi)
     assert dS <= hp.TOL_S_ABS, (label, "S", dS)
     return errH, errW, dphi, dS
@@ -493,3 +507,27 @@ def test_paper_discretisation_chebyshev_midpoint(ctx, N):
             r = _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=scales[s], label=f"cheb N={N} ngl={n_gl} mode={mode} kind={kind}",
                                  edges=edges, ngl=n_gl, averaged=bool(mode))
             print(f"cheb N={N} ngl={n_gl} mode={mode} kind={kind} lJ={lJ}: H {r[0]:.1e} eig {r[1]:.1e} phase {r[2]:.1e} S {r[3]:.1e}")
+
+
+
+@pytest.mark.parametrize("N", [50, 100])
+def test_energy_wave_packets(ctx, N):
+    """NEXT-4: energy wave packets (wpcd_grid.wp_kind = 1; f = hbarc sqrt(k/mu), N_i = dE_i, Eq. 18 H0):
+    same gates as the momentum packets of the configs -- H 1e-12, eigenvalues 1e-11, phases 1e-8 deg -- on the config
+    grid and the Chebyshev grid, uncoupled and coupled, plus the Yamaguchi matrix (form factors by quadrature)."""
+    tl, Ecm = inp.energies(50)
+    scales = inp.sample_scales(2, seed=7)
+    channels = [(0, 0), (0, 3), (1, 1), (1, 2)]
+    for edges in (None, inp.grid_chebyshev(N)):
+        res = _gpu_pipeline(ctx, N, channels, Ecm, scales=scales, S=2, edges=edges, energy_packets=True)
+        for s, c, kind, lJ in ((0, 0, 0, 0), (1, 1, 0, 3), (1, 0, 1, 1), (0, 1, 1, 2)):
+            r = _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=scales[s], label=f"E-packets N={N} kind={kind} lJ={lJ}",
+                                 edges=edges, energy_packets=True)
+            print(f"E-packets N={N} cheb={edges is not None} kind={kind} lJ={lJ}: H {r[0]:.1e} eig {r[1]:.1e} phase {r[2]:.1e} S {r[3]:.1e}")
+    lamA, lamB = inp.yamaguchi_lambda()
+    res = _gpu_pipeline(ctx, N, [(0, 0)], Ecm, yamaguchi=(lamB, inp.YAMAGUCHI_BETA), energy_packets=True)
+    _compare_channel(res, 0, 0, 0, N, 0, Ecm, yamaguchi=(lamB, inp.YAMAGUCHI_BETA), label="E-packets Yamaguchi", energy_packets=True)
+    # the two kinds of packets really differ (e0 and V), so the test above is not vacuous
+    res_k = _gpu_pipeline(ctx, N, [(0, 0)], Ecm)
+    res_e = _gpu_pipeline(ctx, N, [(0, 0)], Ecm, energy_packets=True)
+    assert np.abs(res_k["e0"] - res_e["e0"]).max() > 1e-3 and np.abs(res_k[0]["H"] - res_e[0]["H"]).max() > 1e-3
