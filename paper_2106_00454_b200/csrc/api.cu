@@ -68,6 +68,7 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
   if (!h || !grid || !pot || !chan || !d_e0 || !d_dE || !d_Eedge) return WPCD_EINVAL;
   if (grid->N < 1 || !grid->h_edges || grid->n_gl < 1 || grid->n_gl > 16 || !(grid->hbarc > 0) || !(grid->mu > 0)) return WPCD_EINVAL;
   if (grid->wp_kind != 0 && grid->wp_kind != 1) return WPCD_EINVAL;
+  if (grid->N > 4096) return WPCD_ESIZE;  // 32-bit element indices in the assembly kernels (n = 2N <= 8192)
   if (n_chan < 1 || S < 1 || P < 0 || (P > 0 && !d_scales)) return WPCD_EINVAL;
   if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
   if (!(grid->h_edges[0] >= 0)) return WPCD_EINVAL;

@@ -163,12 +163,14 @@ __device__ __forceinline__ double combine_elem(const ChanDesc& c, int N, int i, 
   return v + acc;
 }
 
-// grid: (ceil(n*n/2/256), nchan_of_kind, S).  Each thread writes two adjacent elements (double2) when n is even.
+// grid: (ceil(n*n/4/256), nchan_of_kind, S).  N % 4 == 0 (the configs): each thread writes four adjacent elements of a
+// row -- same block of the channel, same terms, 32-byte aligned loads of the basis rows and stores of H, 32-bit index
+// arithmetic.  Other N: two elements per thread through combine_elem.
 __global__ void __launch_bounds__(256) k_combine(int N, int coupled, ChanTable tab, const double* __restrict__ basis,
                                                  const double* __restrict__ e0, const double* __restrict__ scales, int P,
                                                  double* __restrict__ Hout) {
-  int n = coupled ? 2 * N : N;
-  int nkind = coupled ? tab.n_cpl : tab.n_unc;
+  const unsigned n = coupled ? 2 * N : N;
+  const int nkind = coupled ? tab.n_cpl : tab.n_unc;
   // find the channel with this slot
   int ci = 0;
   for (int c = 0; c < tab.nchan; ++c)
@@ -176,20 +178,33 @@ __global__ void __launch_bounds__(256) k_combine(int N, int coupled, ChanTable t
   const ChanDesc& cd = tab.c[ci];
   const double* scale = scales ? scales + (size_t)blockIdx.z * P : nullptr;
   double* H = Hout + ((size_t)blockIdx.z * nkind + blockIdx.y) * (size_t)n * n;
-  size_t total = (size_t)n * n;
-  size_t e = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2;
-  if (e >= total) return;
-  if ((total & 1) == 0) {
-    int i = (int)(e / n), j = (int)(e % n);
-    double2 out;
-    out.x = combine_elem(cd, N, i, j, basis, e0, scale, P);
-    size_t e1 = e + 1;
-    int i1 = (int)(e1 / n), j1 = (int)(e1 % n);
-    out.y = combine_elem(cd, N, i1, j1, basis, e0, scale, P);
-    *reinterpret_cast<double2*>(H + e) = out;
-  } else {
-    for (size_t k = e; k < e + 2 && k < total; ++k) H[k] = combine_elem(cd, N, (int)(k / n), (int)(k % n), basis, e0, scale, P);
+  const unsigned total = n * n;  // n <= 8192
+  if ((N & 3) == 0) {
+    const unsigned e = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
+    if (e >= total) return;
+    const unsigned i = e / n, j = e - i * n;
+    const unsigned bi = coupled && i >= (unsigned)N, bj = coupled && j >= (unsigned)N;
+    const unsigned ii = i - bi * N, jj = j - bj * N;
+    const BlockTerms& bt = (bi == bj) ? (bi ? cd.pp : cd.mm) : cd.mp;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int t = 0; t < bt.nterms; ++t) {
+      double coef = bt.V0[t];
+      if (bt.sidx[t] >= 0) coef *= scale[bt.sidx[t]];
+      const double2* b = reinterpret_cast<const double2*>(basis + (size_t)bt.basis[t] * N * N + (size_t)ii * N + jj);
+      const double2 x0 = b[0], x1 = b[1];
+      acc[0] = fma(coef, x0.x, acc[0]); acc[1] = fma(coef, x0.y, acc[1]);
+      acc[2] = fma(coef, x1.x, acc[2]); acc[3] = fma(coef, x1.y, acc[3]);
+    }
+    const double d = e0[ii];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc[k] = ((j + k == i) ? d : 0.0) + acc[k];
+    double2* out = reinterpret_cast<double2*>(H + e);
+    out[0] = make_double2(acc[0], acc[1]);
+    out[1] = make_double2(acc[2], acc[3]);
+    return;
   }
+  const unsigned e = (blockIdx.x * blockDim.x + threadIdx.x) * 4u;
+  for (unsigned k = e; k < e + 4 && k < total; ++k) H[k] = combine_elem(cd, N, (int)(k / n), (int)(k % n), basis, e0, scale, P);
 }
 
 // ------------------------------------------------------------------------------------------------ host side
@@ -260,12 +275,12 @@ int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential
   int ntri = N * (N + 1) / 2;
   k_basis<<<dim3((ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, grid->wp_kind, bt, d_p, d_k, d_w, d_norm, d_basis);
   if (ct.n_unc) {
-    size_t half = ((size_t)N * N + 1) / 2;
-    k_combine<<<dim3((unsigned)((half + 255) / 256), ct.n_unc, S), 256, 0, st>>>(N, 0, ct, d_basis, d_e0, d_scales, P, d_H_unc);
+    size_t quarter = ((size_t)N * N + 3) / 4;
+    k_combine<<<dim3((unsigned)((quarter + 255) / 256), ct.n_unc, S), 256, 0, st>>>(N, 0, ct, d_basis, d_e0, d_scales, P, d_H_unc);
   }
   if (ct.n_cpl) {
-    size_t half = ((size_t)4 * N * N + 1) / 2;
-    k_combine<<<dim3((unsigned)((half + 255) / 256), ct.n_cpl, S), 256, 0, st>>>(N, 1, ct, d_basis, d_e0, d_scales, P, d_H_cpl);
+    size_t quarter = ((size_t)4 * N * N + 3) / 4;
+    k_combine<<<dim3((unsigned)((quarter + 255) / 256), ct.n_cpl, S), 256, 0, st>>>(N, 1, ct, d_basis, d_e0, d_scales, P, d_H_cpl);
   }
   return wpcd_check_cuda(h, cudaGetLastError(), "build_channels launch");
 }
