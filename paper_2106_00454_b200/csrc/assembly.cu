@@ -2,7 +2,7 @@
 // and potential sample.  Three kernels:
 //   k_grid    : bin quantities (e0, dE, Eedge) and the n_gl-point Gauss-Legendre nodes/weights of every bin
 //   k_basis   : one "basis matrix" per distinct (l, mu):  B[i][j] = (1/(pi sqrt(Dk_i Dk_j))) sum_ab w_ia w_jb Q_l(z)
-//               (n_gl x n_gl rule per bin pair; FP64/SFU bound, done once per grid)
+//               (n_gl x n_gl rule per bin pair, 8 threads per element; FP64/SFU bound, done once per grid)
 //   k_combine : H[s][c] = diag(e0) + sum_t V0_t scale[s][t] B_t   -- HBM-write bound: 8 B written per element,
 //               double2 stores, the basis matrices stay L2-resident.
 // Strengths enter linearly, so the per-sample work is the combine only.
@@ -97,13 +97,17 @@ __device__ double legendre_q(int l, double zm1) {
 }
 
 // ------------------------------------------------------------------------------------------------ k_basis
-// grid (ceil(ntri/128), nbasis); thread = upper-triangle element (i <= j); mirrored store keeps B symmetric.
+// grid (ceil(8 ntri/128), nbasis); 8 threads per upper-triangle element (i <= j), each taking the quadrature rows
+// a = sub, sub + 8, ... of the bin pair, summed over the 8 lanes by shuffles; mirrored store keeps B symmetric.
 __global__ void __launch_bounds__(128) k_basis(int N, int ngl, int wp_kind, BasisTable tab, const double* __restrict__ p,
                                                const double* __restrict__ knode, const double* __restrict__ wnode,
                                                const double* __restrict__ norm, double* __restrict__ basis) {
-  int e = blockIdx.x * blockDim.x + threadIdx.x;
-  int ntri = N * (N + 1) / 2;
-  if (e >= ntri) return;
+  const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+  const int sub = gt & 7;
+  int e = gt >> 3;
+  const int ntri = N * (N + 1) / 2;
+  const bool live = e < ntri;
+  if (!live) e = ntri - 1;  // keeps the whole warp in the shuffles below
   // row i of the upper triangle: first element index i*N - i(i-1)/2
   int i = (int)((2.0 * N + 1.0 - sqrt((2.0 * N + 1.0) * (2.0 * N + 1.0) - 8.0 * e)) * 0.5);
   while (i * N - i * (i - 1) / 2 > e) --i;
@@ -130,7 +134,7 @@ __global__ void __launch_bounds__(128) k_basis(int N, int ngl, int wp_kind, Basi
     v = gi * gj;
   } else {
     double mu2 = d.mu * d.mu, acc = 0.0;
-    for (int a = 0; a < ngl; ++a) {
+    for (int a = sub; a < ngl; a += 8) {
       double kp = knode[i * ngl + a], wa = wnode[i * ngl + a];
       double row = 0.0;
       for (int b = 0; b < ngl; ++b) {
@@ -141,10 +145,15 @@ __global__ void __launch_bounds__(128) k_basis(int N, int ngl, int wp_kind, Basi
       }
       acc = fma(wa, row, acc);
     }
+    acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+    acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+    acc += __shfl_xor_sync(0xffffffffu, acc, 4);
     v = wp_kind ? acc / (WPCD_PI * norm[i] * norm[j]) : acc / (WPCD_PI * sqrt(dki * dkj));
   }
-  B[(size_t)i * N + j] = v;
-  B[(size_t)j * N + i] = v;
+  if (live && sub == 0) {
+    B[(size_t)i * N + j] = v;
+    B[(size_t)j * N + i] = v;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ k_combine
@@ -273,7 +282,7 @@ int wpcd_build_launch(WpcdHandle* h, const wpcd_grid* grid, const wpcd_potential
   int tot = N * ngl > N + 1 ? N * ngl : N + 1;
   k_grid<<<(tot + 127) / 128, 128, 0, st>>>(N, ngl, grid->wp_kind, grid->hbarc, grid->mu, d_p, d_e0, d_dE, d_Eedge, d_k, d_w, d_norm);
   int ntri = N * (N + 1) / 2;
-  k_basis<<<dim3((ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, grid->wp_kind, bt, d_p, d_k, d_w, d_norm, d_basis);
+  k_basis<<<dim3((8 * ntri + 127) / 128, bt.nbasis), 128, 0, st>>>(N, ngl, grid->wp_kind, bt, d_p, d_k, d_w, d_norm, d_basis);
   if (ct.n_unc) {
     size_t quarter = ((size_t)N * N + 3) / 4;
     k_combine<<<dim3((unsigned)((quarter + 255) / 256), ct.n_unc, S), 256, 0, st>>>(N, 0, ct, d_basis, d_e0, d_scales, P, d_H_unc);
