@@ -458,6 +458,7 @@ struct JacobiParams {
   double* gwork;   // per-CTA global workspace: [A np*ld] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
   size_t gstride;  // doubles per CTA
   const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
+  int* next;       // global counter of the next matrix to hand out (behind the tables; k_schedule sets it to the grid size)
   int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
   int nranges, row_lo[4], row_hi[4];  // rows of C that are wanted (nranges = 0: all); the others are returned as zeros
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
@@ -470,8 +471,9 @@ struct JacobiParams {
 //   slot[t][s]  = I | J << 16                 blocks of slot s at step t (0xFFFF = none)
 //   feed[t][s]  = s1 | s2 << 16               slots (s1 < s2) of the PREVIOUS step whose tile feeds the pivot of slot s
 //   tile[t][k]  = s1 | s2 << 12 | crit << 24  k-th tile of step t (s1 < s2); crit: it feeds a pivot of the next step
-__global__ void k_schedule(int m, int nb, int* __restrict__ tab) {
+__global__ void k_schedule(int m, int nb, int* __restrict__ tab, int* __restrict__ next, int first) {
   const int nslots = m / 2, ntiles = nslots * (nslots - 1) / 2, t = blockIdx.x;
+  if (t == 0 && threadIdx.x == 0) *next = first;
   const int tp = (t + m - 2) % (m - 1), tn = (t + 1) % (m - 1);
   int* slot = tab + t * nslots;
   int* feed = tab + (m - 1) * nslots + t * nslots;
@@ -609,7 +611,10 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   const int nitems = ntiles + nslots * nvgrp;
   const float rnvgrp = 1.0f / (float)nvgrp;
 
-  for (int mat = blockIdx.x; mat < P.batch; mat += gridDim.x) {
+  // matrices are handed out dynamically (they need 6-8 sweeps each): the first one is the CTA's own index, the next ones
+  // come from a global counter that k_schedule set to gridDim.x
+  __shared__ int s_next;
+  for (int mat = blockIdx.x; mat < P.batch;) {
     const double* H = P.H + (size_t)mat * n * n;
     __syncthreads();
     for (int e = tid; e < np * np; e += kThreads) {
@@ -720,7 +725,12 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
       int c = sm.src[k];
       Co[e] = sm.act[nb + (i >> 3)] ? sm.V[(size_t)i * ldv + c] : 0.0;
     }
-    if (tid == 0) P.info[mat] = converged ? sweeps : -1;
+    if (tid == 0) {
+      P.info[mat] = converged ? sweeps : -1;
+      s_next = atomicAdd(P.next, 1);
+    }
+    __syncthreads();
+    mat = s_next;
   }
 }
 
@@ -743,7 +753,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
-  g.tab_bytes = (((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255;
+  g.tab_bytes = ((((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255) + 256;  // + counter
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
@@ -803,7 +813,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   const int grid = global_grid(h, g, batch);
   if (work_bytes < g.tab_bytes + (size_t)grid * g.gstride * 8) return WPCD_EWORK;
-  k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work));
+  P.next = reinterpret_cast<int*>(static_cast<char*>(d_work) + g.tab_bytes - 256);
+  k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work), P.next, grid);
   int rc;
   switch (g.mode) {
     case 1:
