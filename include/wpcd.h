@@ -104,7 +104,7 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
 
 /* Step (ii), Eq. 21.  Batched real-symmetric eigendecomposition by two-sided block-Jacobi, one CTA per matrix: 8-wide
  * blocks paired in a round-robin tournament; each 16x16 pivot sub-problem gets one parallel-ordered (Brent-Luk) Jacobi
- * sweep inside one warp -- all 120 pairs every 4th step, the 64 pairs between the two blocks otherwise; the
+ * sweep inside one warp -- all 120 pairs at about three steps per sweep, the 64 pairs between the two blocks otherwise; the
  * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products; the pivots of the next step
  * are solved while the current step's updates run.  n <= 200: the matrix (upper 8x8 blocks) in shared memory, the
  * eigenvectors in an L2-resident workspace, 1-4 matrices in flight per SM; larger n: both through the workspace.

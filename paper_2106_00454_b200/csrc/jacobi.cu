@@ -5,8 +5,8 @@
 //     per launch by k_schedule) pairs the blocks; each pair (I,J) is a "slot" with a 16x16 symmetric pivot
 //     sub-problem S = A[IJ,IJ].
 //   * Pivot solve (one warp per slot): one Brent-Luk sweep of S -- all 120 pairs (15 rounds of 8 disjoint rotations)
-//     every 4th step, the 64 pairs between the two blocks (8 rounds) otherwise -- with the classical rotation angle,
-//     division-free, accumulating the 16x16 orthogonal Q in registers.  A serial chain of rounds: latency/issue bound.
+//     at about three steps per tournament sweep, the 64 pairs between the two blocks (8 rounds) otherwise -- with the
+//     classical rotation angle, division-free, accumulating the 16x16 orthogonal Q in registers.  A serial chain of rounds: latency/issue bound.
 //   * Apply (all warps, dynamic work queue): A <- Q^T A Q tile by tile (one tile per slot pair) and V <- V Q, as fp64
 //     tensor-core products (mma.sync m8n8k4 = DMMA, same flop rate as DFMA on B200 but operands distributed over the
 //     warp).  The accumulator fragment of the first product is re-used directly as the B fragment of the second one
@@ -16,6 +16,7 @@
 //     g+1 (into the other Q buffer), then joins the queue of the other tiles and the V updates of step g; one
 //     __syncthreads per step.
 //   * A sweep = m-1 steps.  Converged when a whole sweep rotates nothing (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
+//   * Matrices are handed out to the CTAs dynamically (global counter): they need 6-8 sweeps each.
 // n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
 // n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
 //
@@ -588,8 +589,8 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
     }
   }
   __syncthreads();
-  // Pivot solves are latency bound and suffer when DMMAs of the update queue the same FP64 pipe: they run on the
-  // warps of SM sub-partitions 0 and 1 (warp & 3 < 2), the update queue on those of sub-partitions 2 and 3.
+  // (Keeping the pivot solves on the warps of two SM sub-partitions and the update queue on the other two was measured
+  // slower: the pivots then contend with each other for issue slots and the fp64 pipe.)
   const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
   const AView<kHalf> Av{sm.A, ld, nb};
   if (tid == 0) {  // row blocks of V that hold wanted rows of C (all of them unless row ranges were given)
