@@ -264,6 +264,40 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_table1(args):
+    """Context only (not the bench metric): the regime of the paper's Table 1 -- all 14 channels J <= 4,
+    Chebyshev momentum bins (Eq. 31), mid-point potential (Eq. 30), energy-averaged T (Eq. 28) at 350 energies, phase
+    shifts and total cross section -- as wall time per potential sample for N_WP = 16, 24, 32, 96; one sample (latency)
+    and 1024 samples (throughput).  The paper: 0.5 / 2.5 / 6 / 35 ms on a V100 for one sample with a pre-computed V."""
+    import torch
+    from paper_2106_00454_b200.pipeline import Pipeline
+    names = [c[0] for c in inp.CHANNELS_J4]
+    channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    _, Ecm = inp.energies(350)
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    out = {}
+    for N in (16, 24, 32, 96):
+        for S in (1, 1024):
+            pipe = Pipeline(inp.grid_chebyshev(N), channels, Ecm, S, pot, device=0, mode=1, n_gl=1,
+                            channel_J=[inp.channel_sJ(nm)[1] for nm in names])
+            pipe.scales.copy_(torch.as_tensor(inp.sample_scales(S, seed=0)))
+            for _ in range(3):
+                pipe.solve_device()
+            torch.cuda.synchronize()
+            reps = 20 if S == 1 else 5
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                pipe.solve_device()
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            assert all(int((b["info"] < 1).sum()) == 0 for b in pipe.kind.values())
+            out[f"N_WP={N},S={S}"] = {"ms_per_pass": ms, "ms_per_sample": ms / S, "sigma_tot_mb_at_175MeV": float(pipe.sigma[0, 174])}
+    print(json.dumps({"workload": "paper_table1 (context, not the bench metric)", "channels": 14, "energies": 350,
+                      "variant": "Chebyshev bins, mid-point V, energy-averaged T, phases, sigma_tot", "results": out,
+                      "paper": {"hardware": "Tesla V100, one sample, pre-computed V", "ms": {"16": 0.5, "24": 2.5, "32": 6, "96": 35}}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -274,7 +308,10 @@ def main():
     ap.add_argument("--N", type=int, default=100)
     ap.add_argument("--nE", type=int, default=350)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="bench", choices=["bench", "paper_table1"])
     args = ap.parse_args()
+    if args.workload == "paper_table1":
+        return run_table1(args)
     if args.impl == "reference":
         run_reference(args)
     else:

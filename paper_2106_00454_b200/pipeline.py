@@ -16,7 +16,7 @@ class Pipeline:
     KERNELS_PER_STEP_FIXED = 2  # k_grid, k_basis
 
     def __init__(self, edges, channels, Ecm, S, potential, n_scale_cols=3, device=0, max_sweeps=30, tol=0.0,
-                 onshell_rows_only=True, channel_J=None):
+                 onshell_rows_only=True, channel_J=None, mode=0, n_gl=8, energy_packets=False):
         self.h = wpcd.Handle(device)
         self.dev = self.h.device
         self.edges = np.asarray(edges, dtype=np.float64)
@@ -25,6 +25,8 @@ class Pipeline:
         self.S = int(S)
         self.potential = dict(potential)
         self.max_sweeps, self.tol = max_sweeps, tol
+        # mode 1: energy-averaged resolvent (the paper's production variant); n_gl = 1: mid-point potential (Eq. 30)
+        self.mode, self.n_gl, self.energy_packets = int(mode), int(n_gl), bool(energy_packets)
         self.n_unc = sum(1 for c, _ in self.channels if not c)
         self.n_cpl = len(self.channels) - self.n_unc
         N, f64 = self.N, torch.float64
@@ -82,7 +84,8 @@ class Pipeline:
                 events[name][which].record()
         p = self.potential
         rec("build", 0)
-        self.h.build_channels(self.edges, self.channels, scales=self.scales, S=self.S, out=self.geo, **p)
+        self.h.build_channels(self.edges, self.channels, scales=self.scales, S=self.S, out=self.geo, n_gl=self.n_gl,
+                              energy_packets=self.energy_packets, **p)
         rec("build", 1)
         for kind, b in self.kind.items():
             tag = "cpl" if kind else "unc"
@@ -92,7 +95,7 @@ class Pipeline:
             rec("diag_" + tag, 1)
             rec("onshell_" + tag, 0)
             self.h.onshell_T(self.N, kind, self.geo["e0"], self.geo["Eedge"], b["H"], b["W"], b["C"], self.Ecm,
-                             T=b["T"], bins=b["bins"], work=b["owork"])
+                             T=b["T"], bins=b["bins"], work=b["owork"], mode=self.mode)
             self.h.phase_shifts(kind, b["T"], b["bins"], self.geo["dE"], want_S=False, delta=b["delta"])
             rec("onshell_" + tag, 1)
         if self.J is not None:
