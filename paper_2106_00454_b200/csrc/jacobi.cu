@@ -17,6 +17,8 @@
 //     __syncthreads per step.
 //   * A sweep = m-1 steps.  Converged when a whole sweep rotates nothing (pivot test |a_pq| > tol sqrt(|a_pp a_qq|)).
 //   * Matrices are handed out to the CTAs dynamically (global counter): they need 6-8 sweeps each.
+//   * Rows/columns are relabelled in the order of descending diagonal entries (de Rijk): on the graded WPCD Hamiltonians
+//     the sweeps converge faster than in the natural ascending order (n=200: 7.0 -> 6.3 sweeps).
 // n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
 // n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
 //
@@ -115,6 +117,7 @@ struct Smem {
   int* src;      // [np]
   int* ctr;      // [0..1] work queues (step parity), [2..3] rotations per sweep (sweep parity)
   int* act;      // [nb] active row blocks of V (those that hold wanted rows of C)
+  int* perm;     // [np] internal row/column i holds original index perm[i] & 0xFFFF; bit 16: row i of C is wanted
   const int* tab; // slot and feed tables [2][m-1][nslots]: shared-memory copy (modes 0, 1) or k_schedule's global ones
 };
 
@@ -581,6 +584,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
     sm.src = ip; ip += np;
     sm.ctr = ip; ip += 4;
     sm.act = ip; ip += 2 * nb;  // list of active row blocks, then a flag per row block
+    sm.perm = ip; ip += np;
     if (kMode == 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
       for (int e = tid; e < 2 * (m - 1) * nslots; e += kThreads) ip[e] = P.tab[e];
       sm.tab = ip;
@@ -593,24 +597,8 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   // slower: the pivots then contend with each other for issue slots and the fp64 pipe.)
   const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
   const AView<kHalf> Av{sm.A, ld, nb};
-  if (tid == 0) {  // row blocks of V that hold wanted rows of C (all of them unless row ranges were given)
-    int na = 0;
-    for (int rb = 0; rb < nb; ++rb) {
-      bool want = P.nranges == 0;
-      for (int r = 0; r < P.nranges; ++r) want |= (8 * rb < P.row_hi[r]) && (8 * rb + 8 > P.row_lo[r]);
-      if (want) sm.act[na++] = rb;
-      sm.act[nb + rb] = want ? 1 : 0;
-    }
-    sm.ctr[0] = na;
-  }
-  __syncthreads();
-  const int nact = sm.ctr[0];
-  __syncthreads();
   const int ntiles = nslots * (nslots - 1) / 2;
   constexpr int kVRowBlocksPerItem = (kMode == 1) ? 4 : 2;
-  const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
-  const int nitems = ntiles + nslots * nvgrp;
-  const float rnvgrp = 1.0f / (float)nvgrp;
 
   // matrices are handed out dynamically (they need 6-8 sweeps each): the first one is the CTA's own index, the next ones
   // come from a global counter that k_schedule set to gridDim.x
@@ -618,9 +606,48 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   for (int mat = blockIdx.x; mat < P.batch;) {
     const double* H = P.H + (size_t)mat * n * n;
     __syncthreads();
+    // Ordering (de Rijk): the rows/columns are taken in the order of DESCENDING diagonal entries.  On these graded
+    // Hamiltonians (kinetic energies from 1e-3 to 1e5 MeV along the diagonal) the cyclic sweeps then converge in one to
+    // two sweeps fewer than in the natural ascending order (oracle: 7 -> 5-6 sweeps at N = 100).  Pure relabelling:
+    // internal index i <-> original index perm[i]; eigenvalues are sorted at the end anyway, rows of C are written back
+    // to their original places.
+    for (int k = tid; k < n; k += kThreads) sm.wsort[k] = H[(size_t)k * n + k];
+    __syncthreads();
+    for (int k = tid; k < np; k += kThreads) {
+      if (k < n) {
+        const double dk = sm.wsort[k];
+        int rank = 0;
+        for (int j = 0; j < n; ++j) {
+          const double dj = sm.wsort[j];
+          rank += (dj > dk) || (dj == dk && j < k);
+        }
+        bool want = P.nranges == 0;
+        for (int r = 0; r < P.nranges; ++r) want |= (k >= P.row_lo[r]) && (k < P.row_hi[r]);
+        sm.perm[rank] = k | (want ? 0x10000 : 0);
+      } else {
+        sm.perm[k] = k;  // padding stays behind the matrix, never wanted
+      }
+    }
+    __syncthreads();
+    if (tid == 0) {  // row blocks of V that hold wanted rows of C (all of them unless row ranges were given)
+      int na = 0;
+      for (int rb = 0; rb < nb; ++rb) {
+        int want = 0;
+        for (int i = 0; i < 8; ++i) want |= sm.perm[8 * rb + i] >> 16;
+        if (want) sm.act[na++] = rb;
+        sm.act[nb + rb] = want;
+      }
+      sm.ctr[0] = na;
+    }
+    __syncthreads();
+    const int nact = sm.ctr[0];
+    const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
+    const int nitems = ntiles + nslots * nvgrp;
+    const float rnvgrp = 1.0f / (float)(nvgrp > 0 ? nvgrp : 1);
+    __syncthreads();
     for (int e = tid; e < np * np; e += kThreads) {
       int r = e / np, c = e - r * np;
-      double a = (r < n && c < n) ? H[(size_t)r * n + c] : 0.0;
+      double a = (r < n && c < n) ? H[(size_t)(sm.perm[r] & 0xFFFF) * n + (sm.perm[c] & 0xFFFF)] : 0.0;
       Av.put(r, c, a);
       sm.V[(size_t)r * ldv + c] = (r == c) ? 1.0 : 0.0;
     }
@@ -721,10 +748,11 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
     double* Wo = P.W + (size_t)mat * n;
     double* Co = P.C + (size_t)mat * n * n;
     for (int k = tid; k < n; k += kThreads) Wo[k] = sm.wsort[sm.src[k]];
-    for (int e = tid; e < n * n; e += kThreads) {
+    for (int e = tid; e < n * n; e += kThreads) {  // internal row i goes back to row perm[i]; unwanted rows: zeros
       int i = e / n, k = e - i * n;
       int c = sm.src[k];
-      Co[e] = sm.act[nb + (i >> 3)] ? sm.V[(size_t)i * ldv + c] : 0.0;
+      const int pi = sm.perm[i];
+      Co[(size_t)(pi & 0xFFFF) * n + k] = (pi >> 16) ? sm.V[(size_t)i * ldv + c] : 0.0;
     }
     if (tid == 0) {
       P.info[mat] = converged ? sweeps : -1;
@@ -755,7 +783,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
   g.tab_bytes = ((((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255) + 256;  // + counter
-  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + g.np + 4 + 2 * g.nb) * 4 + 64;
+  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + 2 * g.np + 4 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
