@@ -531,3 +531,38 @@ def test_energy_wave_packets(ctx, N):
     res_k = _gpu_pipeline(ctx, N, [(0, 0)], Ecm)
     res_e = _gpu_pipeline(ctx, N, [(0, 0)], Ecm, energy_packets=True)
     assert np.abs(res_k["e0"] - res_e["e0"]).max() > 1e-3 and np.abs(res_k[0]["H"] - res_e[0]["H"]).max() > 1e-3
+
+
+def test_pipeline_production_variant_options(ctx):
+    """Pipeline(mode=1, n_gl=1, energy_packets=...) runs the paper's production variant (Chebyshev bins, mid-point V,
+    energy-averaged T) end to end: phases and sigma_tot against the oracle chain with the same options."""
+    from paper_2106_00454_b200.pipeline import Pipeline
+    N = 24
+    edges = inp.grid_chebyshev(N)
+    names = [c[0] for c in inp.CHANNELS_J4]; channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    sJ = [inp.channel_sJ(nm) for nm in names]
+    _, Ecm = inp.energies(16)
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    scales = inp.sample_scales(2, seed=21)
+    for ep in (False, True):
+        pipe = Pipeline(edges, channels, Ecm, 2, pot, device=0, mode=1, n_gl=1, energy_packets=ep, channel_J=[J for _, J in sJ])
+        delta, info = pipe.solve_host(scales)
+        sig = pipe.sigma.cpu().numpy()
+        s = 1
+        S_unc, S_cpl = [], []
+        iu = ic = 0
+        for (kind, lJ) in channels:
+            ch = hp.oracle_channel(N, kind, lJ, scales[s], edges=edges, ngl=1, energy_packets=ep)
+            W, C, _ = hp.o.jacobi_ld(ch["H"])       # 80-bit eigenpairs: the arbiter on this grid (DESIGN.md section 3)
+            T, b = hp.o.onshell_T(N, kind, ch["Eedge"], ch["V"], W, C, Ecm, averaged=True)
+            d, Sm = hp.o.phase_shifts(kind, T, b, ch["dE"])
+            g = delta[kind][s * (4 if kind else 10) + (ic if kind else iu)].numpy()
+            err = hp.dist180(g, d)
+            assert (err[:, :2] if kind else err).max() <= hp.TOL_PHASE_DEG, (ep, kind, lJ)
+            (S_cpl if kind else S_unc).append(Sm)
+            if kind: ic += 1
+            else: iu += 1
+        for e, E in enumerate(Ecm):
+            p = np.sqrt(E / (inp.HBARC ** 2 / (2 * inp.MU)))
+            ref = hp.o.sigma_tot(hp.o.partial_waves(channels, sJ, [S[e] for S in S_unc], [S[e] for S in S_cpl]), p)
+            assert abs(sig[s, e] - ref) < 1e-9 * abs(ref), (ep, e, sig[s, e], ref)
