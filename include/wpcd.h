@@ -187,6 +187,23 @@ int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, c
                    const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
                    double hbarc, double mu, double* d_sigma, void* stream);
 
+/* The matrix-inversion (MI) method of Sec. 2.1 batched over (sample, channel, energy) -- the paper's
+ * comparison method as a second workload.  One CTA per Lippmann-Schwinger system:
+ * basis {k_1..k_NQ, p} with Gauss-Legendre nodes mapped k_j = cmap tan(pi(1+x_j)/4) (Eq. 4), propagator vector D derived
+ * from Eqs. 2-4 (reading C3), F = 1 - V diag(D) (Eq. 7), F T = V (Eq. 6) by complex Gauss elimination with
+ * partial pivoting in shared memory, S = 1 - 2 i f p T, f = 2 mu/hbarc^2.  The potential is the same wpcd_potential as for
+ * wpcd_build_channels, used in convention A: v_l = sum_t V0_t Q_l(z_t)/(2k'k) (Yamaguchi: lambda_A = (pi/2) lambda).
+ *   NQ      : quadrature points; the system (NQ+1, coupled 2(NQ+1), complex) must fit one CTA's shared memory:
+ *             NQ <= 114 uncoupled, NQ <= 56 coupled, else WPCD_ESIZE
+ *   d_Ecm   : [nE] c.m. energies, MeV (p = sqrt(E_cm/cE))
+ *   d_S_unc : [S][n_unc][nE][2]        S-matrix (re,im), list order of the uncoupled channels
+ *   d_S_cpl : [S][n_cpl][nE][2][2][2]  S-matrix of the coupled channels
+ *   d_work  : wpcd_mi_workspace_bytes(NQ) bytes */
+size_t wpcd_mi_workspace_bytes(void* handle, int NQ);
+int wpcd_mi_solve(void* handle, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales, int S,
+                  int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
+                  double* d_S_cpl, void* d_work, size_t work_bytes, void* stream);
+
 /* Test hooks (host only, no GPU needed): the block tournament that wpcd_diag_batched runs (csrc/jacobi_schedule.cuh).
  * m = number of players (8-wide blocks, even, >= 6; players >= nb are padding), a sweep has m-1 steps of m/2 slots.
  *   wpcd_jacobi_schedule      : blocks (I < J) of slot s at step t; J = -1 single block, I = J = -1 empty slot.

@@ -163,6 +163,38 @@ int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, c
                            static_cast<cudaStream_t>(stream));
 }
 
+size_t wpcd_mi_workspace_bytes(void* handle, int NQ) {
+  (void)handle;
+  return NQ > 0 ? wpcd_mi_workspace(NQ) : 0;
+}
+
+int wpcd_mi_solve(void* handle, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales, int S,
+                  int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
+                  double* d_S_cpl, void* d_work, size_t work_bytes, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !pot || !chan || n_chan < 1 || S < 1 || nE < 1 || !d_Ecm || NQ < 2 || !(cmap > 0) || !(hbarc > 0) || !(mu > 0)) return WPCD_EINVAL;
+  if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
+  if (pot->kind != 0 && pot->kind != 1) return WPCD_EINVAL;
+  if (pot->kind == 0 && (pot->n_terms < 1 || pot->n_terms > WPCD_MAX_TERMS || !pot->V0 || !pot->mu)) return WPCD_EINVAL;
+  if (d_scales && P < 1) return WPCD_EINVAL;
+  int n_unc = 0, n_cpl = 0;
+  for (int c = 0; c < n_chan; ++c) {
+    if (chan[c].coupled) {
+      if (chan[c].lJ < 1 || pot->kind == 1 || !(pot->muT > 0)) return WPCD_EINVAL;
+      ++n_cpl;
+    } else {
+      if (chan[c].lJ < 0) return WPCD_EINVAL;
+      ++n_unc;
+    }
+    if (chan[c].lJ > 20) return WPCD_ESIZE;
+  }
+  if ((n_unc && !d_S_unc) || (n_cpl && !d_S_cpl)) return WPCD_EINVAL;
+  if ((n_unc && !wpcd_mi_fits(h, NQ, 0)) || (n_cpl && !wpcd_mi_fits(h, NQ, 1))) return WPCD_ESIZE;
+  if (!d_work || work_bytes < wpcd_mi_workspace(NQ)) return WPCD_EWORK;
+  return wpcd_mi_launch(h, pot, chan, n_chan, d_scales, S, P, NQ, cmap, hbarc, mu, d_Ecm, nE, d_S_unc, d_S_cpl, d_work,
+                        static_cast<cudaStream_t>(stream));
+}
+
 int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, int nE, int* h_rows, int* n_ranges) {
   if (!grid || !grid->h_edges || grid->N < 1 || !h_Ecm || nE < 1 || !h_rows || !n_ranges) return WPCD_EINVAL;
   return wpcd_onshell_rows_host(grid->N, coupled ? 1 : 0, grid->h_edges, grid->hbarc, grid->mu, h_Ecm, nE, h_rows, n_ranges);

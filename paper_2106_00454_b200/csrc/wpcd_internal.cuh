@@ -41,3 +41,9 @@ int wpcd_sigma_launch(WpcdHandle* h, int S, int nE, int n_unc, const int* h_J_un
                       double hbarc, double mu, double* d_sigma, cudaStream_t st);
 int wpcd_onshell_rows_host(int N, int coupled, const double* h_edges, double hbarc, double mu, const double* h_Ecm, int nE,
                            int* h_rows, int* n_ranges);
+// mi.cu
+size_t wpcd_mi_workspace(int NQ);
+bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled);
+int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales,
+                   int S, int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
+                   double* d_S_cpl, void* d_work, cudaStream_t st);

@@ -62,6 +62,10 @@ _lib.wpcd_onshell_rows.argtypes = [C.POINTER(Grid), _i, C.POINTER(_d), _i, C.POI
 _lib.wpcd_onshell_rows.restype = _i
 _lib.wpcd_sigma_tot.argtypes = [_vp, _i, _i, _i, C.POINTER(_i), _vp, _i, C.POINTER(_i), _vp, _vp, _vp, _vp, _d, _d, _vp, _vp]
 _lib.wpcd_sigma_tot.restype = _i
+_lib.wpcd_mi_workspace_bytes.argtypes = [_vp, _i]; _lib.wpcd_mi_workspace_bytes.restype = _sz
+_lib.wpcd_mi_solve.argtypes = [_vp, C.POINTER(Potential), C.POINTER(Channel), _i, _vp, _i, _i, _i, _d, _d, _d, _vp, _i, _vp,
+                               _vp, _vp, _sz, _vp]
+_lib.wpcd_mi_solve.restype = _i
 
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
@@ -150,6 +154,37 @@ class Handle:
                                       _ptr(out["Eedge"]), _ptr(work), work.numel(), _stream(stream))
         self._check(rc, "wpcd_build_channels")
         return out
+
+    # ------------------------------------------------------------------ wpcd_mi_solve
+    def mi_solve(self, channels, Ecm, NQ=96, V0=None, mu=None, scale_idx=None, VT=0.0, muT=1.0, VT_scale_idx=-1,
+                 yamaguchi=None, scales=None, S=1, cmap=1.0, hbarc=197.327, mured=469.46, stream=None):
+        """MI method (Sec. 2.1) for every (sample, channel, energy); the potential arguments are those of build_channels
+        (yamaguchi = (lambda_B, beta)).  Returns (S_unc [S][n_unc][nE][2], S_cpl [S][n_cpl][nE][2][2][2]) device tensors."""
+        pot = Potential()
+        keep = []
+        if yamaguchi is not None:
+            pot.kind = 1; pot.n_terms = 0; pot.lambda_, pot.beta = float(yamaguchi[0]), float(yamaguchi[1])
+            pot.VT_scale_idx = -1; pot.muT = 1.0
+        else:
+            nt = len(V0)
+            a = (C.c_double * nt)(*[float(x) for x in V0]); b = (C.c_double * nt)(*[float(x) for x in mu])
+            keep += [a, b]
+            pot.kind = 0; pot.n_terms = nt; pot.V0 = a; pot.mu = b
+            if scale_idx is not None:
+                c = (C.c_int * nt)(*[int(x) for x in scale_idx]); keep.append(c); pot.scale_idx = c
+            pot.VT, pot.muT, pot.VT_scale_idx = float(VT), float(muT), int(VT_scale_idx)
+        nch = len(channels)
+        ch = (Channel * nch)(*[Channel(int(c), int(l)) for c, l in channels])
+        n_unc = sum(1 for c, _ in channels if not c); n_cpl = nch - n_unc
+        P = 0 if scales is None else scales.shape[1]
+        nE = Ecm.shape[0]; dev = self.device
+        S_unc = torch.empty((S, n_unc, nE, 2), dtype=torch.float64, device=dev) if n_unc else None
+        S_cpl = torch.empty((S, n_cpl, nE, 2, 2, 2), dtype=torch.float64, device=dev) if n_cpl else None
+        work = self._work(_lib.wpcd_mi_workspace_bytes(self._h, int(NQ)))
+        rc = _lib.wpcd_mi_solve(self._h, C.byref(pot), ch, nch, _ptr(scales), S, P, int(NQ), float(cmap), float(hbarc),
+                                float(mured), _ptr(Ecm), nE, _ptr(S_unc), _ptr(S_cpl), _ptr(work), work.numel(), _stream(stream))
+        self._check(rc, "wpcd_mi_solve")
+        return S_unc, S_cpl
 
     # ------------------------------------------------------------------ wpcd_diag_batched
     def diag_workspace_bytes(self, n, batch):

@@ -566,3 +566,51 @@ def test_pipeline_production_variant_options(ctx):
             p = np.sqrt(E / (inp.HBARC ** 2 / (2 * inp.MU)))
             ref = hp.o.sigma_tot(hp.o.partial_waves(channels, sJ, [S[e] for S in S_unc], [S[e] for S in S_cpl]), p)
             assert abs(sig[s, e] - ref) < 1e-9 * abs(ref), (ep, e, sig[s, e], ref)
+
+
+def test_mi_solver_on_gpu(ctx):
+    """NEXT-4, second half: wpcd_mi_solve (MI method of Sec. 2.1, one CTA per (sample, channel, energy)) against the
+    oracle's MI solver: all 14 channels with seeded strength scales, and the Yamaguchi potential against its closed form.
+    Tolerance: |dS| <= 1e-10 (both sides solve the same complex linear system in fp64; only the summation order differs)."""
+    h, torch = ctx["h"], ctx["torch"]
+    channels = [(c[1], c[2]) for c in inp.CHANNELS_J4]
+    tl = np.array([1.0, 10.0, 50.0, 150.0, 350.0]); Ecm = tl / 2
+    scales = inp.sample_scales(2, seed=4)
+    dE = _to_dev(ctx, Ecm)
+    for NQ in (24, 48):
+        S_unc, S_cpl = h.mi_solve(channels, dE, NQ=NQ, V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V,
+                                  muT=inp.TENSOR_MU, VT_scale_idx=2, scales=_to_dev(ctx, scales), S=2)
+        torch.cuda.synchronize()
+        Su = S_unc.cpu().numpy(); Sc = S_cpl.cpu().numpy()
+        Su = Su[..., 0] + 1j * Su[..., 1]; Sc = Sc[..., 0] + 1j * Sc[..., 1]
+        worst = 0.0
+        for s in range(2):
+            V0 = inp.MT_V0 * scales[s, :2]
+            iu = ic = 0
+            for (kind, lJ) in channels:
+                for e, t in enumerate(tl):
+                    if not kind:
+                        ref, _ = hp.o.mi_solve(t, V0=V0, mu=inp.MT_MU, l_or_J=lJ, NQ=NQ)
+                        worst = max(worst, abs(Su[s, iu, e] - ref))
+                    else:
+                        ref, _ = hp.o.mi_solve(t, coupled=True, V0=V0, mu=inp.MT_MU, l_or_J=lJ, VT=inp.TENSOR_V * scales[s, 2],
+                                               muT=inp.TENSOR_MU, NQ=NQ)
+                        worst = max(worst, np.abs(Sc[s, ic, e] - ref).max())
+                        assert np.abs(Sc[s, ic, e] @ Sc[s, ic, e].conj().T - np.eye(2)).max() < 1e-11   # unitarity (P5)
+                if kind: ic += 1
+                else: iu += 1
+        print(f"MI on the GPU, NQ={NQ}: max |dS| vs oracle {worst:.2e}")
+        assert worst < 1e-10
+        assert np.abs(np.abs(Su) - 1).max() < 1e-11
+    # Yamaguchi: closed form (reading C15)
+    lamA, lamB = inp.yamaguchi_lambda()
+    S_unc, _ = h.mi_solve([(0, 0)], dE, NQ=96, yamaguchi=(lamB, inp.YAMAGUCHI_BETA))
+    Su = S_unc.cpu().numpy(); Su = Su[0, 0, :, 0] + 1j * Su[0, 0, :, 1]
+    beta = inp.YAMAGUCHI_BETA; lp = lamA * inp.MU / inp.HBARC ** 2
+    for e, t in enumerate(tl):
+        p = np.sqrt(inp.MU * t) / inp.HBARC
+        Sx = 1 + 4j * lp * p / (p * p + beta * beta) ** 2 / (1 - lp / (beta * (beta - 1j * p) ** 2))
+        assert abs(Su[e] - Sx) < 1e-11, (t, Su[e], Sx)
+    # sizes that do not fit one CTA's shared memory are refused
+    with pytest.raises(RuntimeError):
+        h.mi_solve([(1, 1)], dE, NQ=96, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
