@@ -180,7 +180,9 @@ int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double
  *   h_J_unc : [n_unc] HOST, total angular momentum J of every uncoupled channel (e.g. 3P0: J = 0), list order
  *   h_J_cpl : [n_cpl] HOST, J >= 1 of every coupled channel
  *   d_T_unc : [S][n_unc][nE][2], d_T_cpl : [S][n_cpl][nE][2][2][2] -- as written by wpcd_onshell_T for batch = S x channels
- *             (NULL allowed when the count is 0);  d_bin, d_dE, d_Ecm as for wpcd_phase_shifts / wpcd_onshell_T
+ *             (NULL allowed when the count is 0);  d_bin, d_dE, d_Ecm as for wpcd_phase_shifts / wpcd_onshell_T.
+ *             d_bin = d_dE = NULL: the two arrays hold S-MATRICES instead (same layout, e.g. from wpcd_mi_solve) and
+ *             Re(1 - S_ll) is taken from them directly (no energy is then outside a grid)
  *   d_sigma : [S][nE] millibarn (1 fm^2 = 10 mb); NaN where the energy is outside the grid
  * n_unc, n_cpl <= WPCD_MAX_CHANNELS. */
 int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, const double* d_T_unc, int n_cpl,

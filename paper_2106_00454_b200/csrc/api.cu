@@ -154,7 +154,8 @@ int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, c
                    const int* h_J_cpl, const double* d_T_cpl, const int* d_bin, const double* d_dE, const double* d_Ecm,
                    double hbarc, double mu, double* d_sigma, void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
-  if (!h || S < 1 || nE < 1 || n_unc < 0 || n_cpl < 0 || n_unc + n_cpl < 1 || !d_bin || !d_dE || !d_Ecm || !d_sigma) return WPCD_EINVAL;
+  if (!h || S < 1 || nE < 1 || n_unc < 0 || n_cpl < 0 || n_unc + n_cpl < 1 || !d_Ecm || !d_sigma) return WPCD_EINVAL;
+  if ((d_bin == nullptr) != (d_dE == nullptr)) return WPCD_EINVAL;  // both given (inputs are T) or both NULL (inputs are S)
   if ((n_unc && (!h_J_unc || !d_T_unc)) || (n_cpl && (!h_J_cpl || !d_T_cpl)) || !(hbarc > 0) || !(mu > 0)) return WPCD_EINVAL;
   if (n_unc > WPCD_MAX_CHANNELS || n_cpl > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
   for (int c = 0; c < n_unc; ++c) if (h_J_unc[c] < 0) return WPCD_EINVAL;

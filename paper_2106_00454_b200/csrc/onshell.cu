@@ -412,17 +412,26 @@ __global__ void k_sigma(SigmaParams P) {
   if (idx >= (size_t)P.S * P.nE) return;
   const int e = (int)(idx % P.nE);
   const size_t s = idx / P.nE;
-  const int b = P.bin[e];
-  if (b < 0) { P.sigma[idx] = nan(""); return; }
-  const double f = -2.0 * WPCD_PI / P.dE[b];
   double acc = 0.0;
-  for (int c = 0; c < P.n_unc; ++c) {
-    const double ti = P.Tunc[((s * P.n_unc + c) * P.nE + e) * 2 + 1];
-    acc += (2.0 * P.J_unc[c] + 1.0) * (f * ti);
-  }
-  for (int c = 0; c < P.n_cpl; ++c) {
-    const double* t = P.Tcpl + ((s * P.n_cpl + c) * P.nE + e) * 8;
-    acc += (2.0 * P.J_cpl[c] + 1.0) * (f * t[1] + f * t[7]);
+  if (P.dE == nullptr) {  // the inputs are S-matrices (e.g. from wpcd_mi_solve): Re(1 - S_ll) = 1 - Re S_ll
+    for (int c = 0; c < P.n_unc; ++c)
+      acc += (2.0 * P.J_unc[c] + 1.0) * (1.0 - P.Tunc[((s * P.n_unc + c) * P.nE + e) * 2]);
+    for (int c = 0; c < P.n_cpl; ++c) {
+      const double* t = P.Tcpl + ((s * P.n_cpl + c) * P.nE + e) * 8;
+      acc += (2.0 * P.J_cpl[c] + 1.0) * ((1.0 - t[0]) + (1.0 - t[6]));
+    }
+  } else {
+    const int b = P.bin[e];
+    if (b < 0) { P.sigma[idx] = nan(""); return; }
+    const double f = -2.0 * WPCD_PI / P.dE[b];
+    for (int c = 0; c < P.n_unc; ++c) {
+      const double ti = P.Tunc[((s * P.n_unc + c) * P.nE + e) * 2 + 1];
+      acc += (2.0 * P.J_unc[c] + 1.0) * (f * ti);
+    }
+    for (int c = 0; c < P.n_cpl; ++c) {
+      const double* t = P.Tcpl + ((s * P.n_cpl + c) * P.nE + e) * 8;
+      acc += (2.0 * P.J_cpl[c] + 1.0) * (f * t[1] + f * t[7]);
+    }
   }
   const double p2 = P.Ecm[e] / P.cE;
   P.sigma[idx] = 10.0 * WPCD_PI / (2.0 * p2) * acc;  // fm^2 -> mb

@@ -614,3 +614,14 @@ def test_mi_solver_on_gpu(ctx):
     # sizes that do not fit one CTA's shared memory are refused
     with pytest.raises(RuntimeError):
         h.mi_solve([(1, 1)], dE, NQ=96, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+    # wpcd_sigma_tot on S-matrices (d_bin = d_dE = NULL) against the oracle's Clebsch-Gordan chain on the oracle's MI S
+    names = [c[0] for c in inp.CHANNELS_J4]; sJ = [inp.channel_sJ(nm) for nm in names]
+    S_unc, S_cpl = h.mi_solve(channels, dE, NQ=24, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+    Ju = [J for (k, _), (_, J) in zip(channels, sJ) if not k]; Jc = [J for (k, _), (_, J) in zip(channels, sJ) if k]
+    sig = h.sigma_tot(Ju, S_unc, Jc, S_cpl, None, None, dE).cpu().numpy()[0]
+    for e, t in enumerate(tl):
+        Su = [hp.o.mi_solve(t, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=lJ, NQ=24)[0] for (k, lJ) in channels if not k]
+        Sc = [hp.o.mi_solve(t, coupled=True, V0=inp.MT_V0, mu=inp.MT_MU, l_or_J=lJ, VT=inp.TENSOR_V, muT=inp.TENSOR_MU, NQ=24)[0]
+              for (k, lJ) in channels if k]
+        ref = hp.o.sigma_tot(hp.o.partial_waves(channels, sJ, Su, Sc), np.sqrt(inp.MU * t) / inp.HBARC)
+        assert abs(sig[e] - ref) < 1e-10 * ref, (t, sig[e], ref)
