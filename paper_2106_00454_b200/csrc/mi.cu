@@ -32,7 +32,25 @@ struct MiParams {
   int VT_sidx;
   double lambdaA, beta;
   double hbarc, mured;
+  const double* basis;                                   // [nbasis][NQ][NQ]: Q_l(z(k_i,k_j))/(2 k_i k_j) per distinct (l, mu)
+  int id_mm[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // basis matrix of term t in the block l = lJ (uncoupled) / J-1
+  int id_pp[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // ... in the block l = J+1
+  int id_mp[WPCD_MAX_CHANNELS];                           // ... of the off-diagonal Yukawa
 };
+
+struct MiBasisTable { int n; int l[WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1)]; double mu[WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1)]; };
+
+// The grid x grid part of V does not depend on the energy or the sample: one matrix per distinct (l, mu), computed once
+// per call; only the on-shell row and column are evaluated per system.
+__global__ void k_mi_basis(int NQ, MiBasisTable tab, const double* __restrict__ kq, double* __restrict__ basis) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= NQ * NQ) return;
+  const int i = idx / NQ, j = idx - i * NQ;
+  const double kp = kq[i], k = kq[j], mu = tab.mu[blockIdx.y];
+  const double diff = kp - k;
+  const double zm1 = fma(diff, diff, mu * mu) / (2.0 * kp * k);
+  basis[(size_t)blockIdx.y * NQ * NQ + idx] = legendre_q(tab.l[blockIdx.y], zm1);
+}
 
 // k_j, w_j of the MI grid: root a of P_NQ by Newton, mapped with c tan(pi(1+x)/4)
 __global__ void k_mi_grid(int NQ, double cmap, double* __restrict__ kq, double* __restrict__ wq) {
@@ -119,8 +137,19 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
     const int r = idx / n, c = idx - r * n;
     const int a = r / M, i = r - a * M, b = c / M, j = c - b * M;
     double v;
-    if (P.kind == 1) v = -P.lambdaA / ((q[i] * q[i] + P.beta * P.beta) * (q[j] * q[j] + P.beta * P.beta));
-    else if (!P.coupled) v = yukawa_A(lJ, P.nterms, sV0, P.mu, q[i], q[j]);
+    if (P.kind == 1) {
+      v = -P.lambdaA / ((q[i] * q[i] + P.beta * P.beta) * (q[j] * q[j] + P.beta * P.beta));
+    } else if (i < NQ && j < NQ) {  // grid x grid: tabulated Q_l, same arithmetic as yukawa_A
+      const size_t o = (size_t)i * NQ + j, nn = (size_t)NQ * NQ;
+      double sacc = 0.0;
+      if (a == b) {
+        const int* id = (P.coupled && a == 1) ? P.id_pp[ch] : P.id_mm[ch];
+        for (int t = 0; t < P.nterms; ++t) sacc += sV0[t] * P.basis[id[t] * nn + o];
+      } else {
+        sacc += sVT * P.basis[P.id_mp[ch] * nn + o];
+      }
+      v = sacc / (2.0 * q[i] * q[j]);
+    } else if (!P.coupled) v = yukawa_A(lJ, P.nterms, sV0, P.mu, q[i], q[j]);
     else if (a == b) v = yukawa_A(a == 0 ? lJ - 1 : lJ + 1, P.nterms, sV0, P.mu, q[i], q[j]);
     else v = yukawa_A(lJ, 1, &sVT, &P.muT, q[i], q[j]);
     const double2 d = D[j];
@@ -137,17 +166,26 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
       const double v = hypot(x.x, x.y);
       if (v > best) { best = v; bi = r; }
     }
-    s_red[tid] = best; s_idx[tid] = bi;
-    __syncthreads();
-    for (int s = kMiThreads / 2; s > 0; s >>= 1) {
-      if (tid < s) {
-        const double o = s_red[tid + s];
-        const int oi = s_idx[tid + s];
-        if (o > s_red[tid] || (o == s_red[tid] && oi < s_idx[tid])) { s_red[tid] = o; s_idx[tid] = oi; }
-      }
-      __syncthreads();
+    // arg-max over the CTA: shuffles inside a warp, one round through shared memory across the warps
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
     }
-    const int piv = s_idx[0];
+    if ((tid & 31) == 0) { s_red[tid >> 5] = best; s_idx[tid >> 5] = bi; }
+    __syncthreads();
+    if (tid < 32) {
+      best = tid < kMiThreads / 32 ? s_red[tid] : -1.0;
+      bi = tid < kMiThreads / 32 ? s_idx[tid] : n;
+      for (int o = 16; o > 0; o >>= 1) {
+        const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+      }
+      if (tid == 0) s_idx[kMiThreads / 32] = bi;
+    }
+    __syncthreads();
+    const int piv = s_idx[kMiThreads / 32];
     if (piv != c)
       for (int k = c + tid; k < ld; k += kMiThreads) {
         const double2 t = F[(size_t)c * ld + k];
@@ -158,14 +196,15 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
     const double2 dcc = F[(size_t)c * ld + c];
     for (int r = c + 1 + tid; r < n; r += kMiThreads) F[(size_t)r * ld + c] = cdiv(F[(size_t)r * ld + c], dcc);  // multiplier
     __syncthreads();
-    const int w = ld - (c + 1), rows = n - (c + 1);
-    for (int idx = tid; idx < rows * w; idx += kMiThreads) {
-      const int r = c + 1 + idx / w, k = c + 1 + idx % w;
-      const double2 m = F[(size_t)r * ld + c];
-      const double2 x = cmul(m, F[(size_t)c * ld + k]);
-      double2 y = F[(size_t)r * ld + k];
-      y.x -= x.x; y.y -= x.y;
-      F[(size_t)r * ld + k] = y;
+    // rank-one update of the trailing block: a warp walks along a row (conflict-free 16-byte accesses), 8 rows at a time
+    for (int k = c + 1 + (tid & 31); k < ld; k += 32) {
+      const double2 pk = F[(size_t)c * ld + k];
+      for (int r = c + 1 + (tid >> 5); r < n; r += kMiThreads / 32) {
+        const double2 x = cmul(F[(size_t)r * ld + c], pk);
+        double2 y = F[(size_t)r * ld + k];
+        y.x -= x.x; y.y -= x.y;
+        F[(size_t)r * ld + k] = y;
+      }
     }
     __syncthreads();
   }
@@ -200,7 +239,8 @@ size_t mi_smem(int NQ, int coupled) {
 
 }  // namespace
 
-size_t wpcd_mi_workspace(int NQ) { return (size_t)2 * ((NQ * 8 + 255) & ~255); }
+constexpr int kMiMaxBasis = WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1);
+size_t wpcd_mi_workspace(int NQ) { return (size_t)2 * ((NQ * 8 + 255) & ~255) + (size_t)kMiMaxBasis * NQ * NQ * 8; }
 
 // does the system of this kind fit one CTA's shared memory?
 bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled) { return mi_smem(NQ, coupled) + 4096 <= (size_t)h->max_smem_optin; }
@@ -210,13 +250,35 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
                    double* d_S_cpl, void* d_work, cudaStream_t st) {
   double* kq = static_cast<double*>(d_work);
   double* wq = reinterpret_cast<double*>(static_cast<char*>(d_work) + ((NQ * 8 + 255) & ~255));
+  double* basis = reinterpret_cast<double*>(static_cast<char*>(d_work) + 2 * ((NQ * 8 + 255) & ~255));
   k_mi_grid<<<(NQ + 127) / 128, 128, 0, st>>>(NQ, cmap, kq, wq);
+  // distinct (l, mu) of all channel blocks
+  MiBasisTable bt; bt.n = 0;
+  auto find_or_add = [&](int l, double mu_) {
+    for (int b = 0; b < bt.n; ++b) if (bt.l[b] == l && bt.mu[b] == mu_) return b;
+    bt.l[bt.n] = l; bt.mu[bt.n] = mu_;
+    return bt.n++;
+  };
+  int ids_mm[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS] = {}, ids_pp[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS] = {}, ids_mp[WPCD_MAX_CHANNELS] = {};
+  if (pot->kind == 0) {
+    for (int c = 0; c < n_chan; ++c)
+      for (int t = 0; t < pot->n_terms; ++t) {
+        if (!chan[c].coupled) ids_mm[c][t] = find_or_add(chan[c].lJ, pot->mu[t]);
+        else { ids_mm[c][t] = find_or_add(chan[c].lJ - 1, pot->mu[t]); ids_pp[c][t] = find_or_add(chan[c].lJ + 1, pot->mu[t]); }
+      }
+    for (int c = 0; c < n_chan; ++c) if (chan[c].coupled) ids_mp[c] = find_or_add(chan[c].lJ, pot->muT);
+    k_mi_basis<<<dim3((NQ * NQ + 255) / 256, bt.n), 256, 0, st>>>(NQ, bt, kq, basis);
+  }
   for (int coupled = 0; coupled < 2; ++coupled) {
     MiParams Q;
     Q.kq = kq; Q.wq = wq; Q.Ecm = d_Ecm; Q.scales = d_scales; Q.Sout = coupled ? d_S_cpl : d_S_unc;
-    Q.NQ = NQ; Q.nE = nE; Q.P = P; Q.coupled = coupled; Q.nch = 0;
+    Q.NQ = NQ; Q.nE = nE; Q.P = P; Q.coupled = coupled; Q.nch = 0; Q.basis = basis;
     for (int c = 0; c < n_chan; ++c)
-      if ((chan[c].coupled ? 1 : 0) == coupled) Q.lJ[Q.nch++] = chan[c].lJ;
+      if ((chan[c].coupled ? 1 : 0) == coupled) {
+        for (int t = 0; t < WPCD_MAX_TERMS; ++t) { Q.id_mm[Q.nch][t] = ids_mm[c][t]; Q.id_pp[Q.nch][t] = ids_pp[c][t]; }
+        Q.id_mp[Q.nch] = ids_mp[c];
+        Q.lJ[Q.nch++] = chan[c].lJ;
+      }
     if (!Q.nch) continue;
     Q.kind = pot->kind; Q.nterms = pot->kind == 0 ? pot->n_terms : 0;
     for (int t = 0; t < WPCD_MAX_TERMS; ++t) {
