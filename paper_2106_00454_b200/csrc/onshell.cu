@@ -212,6 +212,7 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
   double* sW = reinterpret_cast<double*>(smem_raw);  // [n]
   double* sLo = sW + n;                                // [n]
   double* sHi = sLo + n;                               // [n]
+  double* sIw = sHi + n;                               // [n] 1/(hi - lo) of the positive states
   __shared__ int s_nb;
   const size_t mat = blockIdx.x;
   const double* H = P.H + mat * (size_t)n * n;
@@ -243,6 +244,7 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
       }
     }
     sLo[k] = lo; sHi[k] = hi;
+    sIw[k] = k >= nbd ? 1.0 / (hi - lo) : 0.0;
   }
   __syncthreads();
   for (int e = warp; e < nE; e += nwarps) {
@@ -257,7 +259,18 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
     double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
     for (int k = lane; k < n; k += 32) {
       double gr, gi;
-      resolvent_k(P.mode, E, b, k, nbd, nc, sW, sLo, sHi, gr, gi);
+      if (P.mode == 0) {  // point-wise resolvent (resolvent_k, mode 0) with the tabulated reciprocal bin width
+        gi = 0.0;
+        if (k < nbd) {
+          gr = 1.0 / (E - sW[k]);
+        } else {
+          const double lo = sLo[k], hi = sHi[k], iw = sIw[k];
+          gr = log(fabs((E - lo) / (E - hi))) * iw;
+          if (E >= lo && E < hi) gi = -WPCD_PI * iw;
+        }
+      } else {
+        resolvent_k(P.mode, E, b, k, nbd, nc, sW, sLo, sHi, gr, gi);
+      }
       const double w = sW[k] - e0b;
       const double a = c0[k] * w;
       re00 = fma(a * a, gr, re00); im00 = fma(a * a, gi, im00);
@@ -459,7 +472,7 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   k_bins<<<1, 256, 0, st>>>(N, nE, d_Eedge, d_Ecm, d_bin, static_cast<int*>(d_work));
   if (P.n <= kI1MaxN) {
-    k_onshell_i1<<<batch, kOnThreads, (size_t)3 * P.n * 8, st>>>(P);
+    k_onshell_i1<<<batch, kOnThreads, (size_t)4 * P.n * 8, st>>>(P);
     return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
   }
   int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
