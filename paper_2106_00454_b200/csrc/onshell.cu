@@ -2,7 +2,8 @@
 //   k_bins   : FWP bin of every on-shell energy (Eedge_i <= E < Eedge_{i+1}) and the range of bins in use
 //   k_onshell: one CTA per matrix.  Pseudostate bin edges from the sorted eigenvalues (Eq. 23 as printed,
 //              PAPER.md:166-173; bound states eps < 0 separate; coupled channels: two branches by rank parity),
-//              then for chunks of on-shell bins: rows of VC = (H - diag e0) C, and for every energy in the chunk
+//              then for chunks of 16 on-shell rows: VC = (H - diag e0) C as fp64 tensor-core products (mma.sync
+//              m8n8k4; A fragments from shared memory, B fragments straight from C), and for every energy in the chunk
 //              (one warp per energy, lanes over eigenstates) T = V_ii + sum_k (VC)_ik (VC)_i'k g_k(E) with the
 //              analytic resolvent g_k of Eqs. B.3-B.6 (sign of the printed last line corrected).
 //   k_phase  : S = 1 - 2 pi i T/dE_i, Eqs. A.3-A.5.
@@ -13,6 +14,13 @@
 namespace {
 
 constexpr int kOnThreads = 256;
+constexpr int kOnGemmThreads = 512;  // k_onshell (direct product, n > kI1MaxN)
+
+__device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {  // fp64 tensor-core MMA, D (8x8) += A (8x4) B (4x8)
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d[0]), "+d"(d[1])
+               : "d"(a), "d"(b));
+}
 
 __device__ __forceinline__ double xlnx(double x) { return x == 0.0 ? 0.0 : x * log(fabs(x)); }
 
@@ -74,18 +82,20 @@ struct OnshellParams {
   const int* range;
   double* T;
   int N, n, nc, nE, R;  // R = bins per chunk
+  int ldv, gemm;        // k_onshell: row stride of the V rows in shared memory; 1 = tensor-core product
   int mode;             // 0 point-wise resolvent (B.5-B.6), 1 energy-averaged (Eq. 28, B.7-B.8)
 };
 
-__global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
+__global__ void __launch_bounds__(kOnGemmThreads) k_onshell(OnshellParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int N = P.N, n = P.n, nc = P.nc, nE = P.nE, R = P.R;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kOnThreads / 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kOnGemmThreads / 32;
+  const int ldv = P.ldv, vrows = R * nc < 8 ? 8 : R * nc;
   double* sW = reinterpret_cast<double*>(smem_raw);  // [n]
   double* sLo = sW + n;                                // [n]
   double* sHi = sLo + n;                               // [n]
-  double* sV = sHi + n;                                // [R*nc][n]
-  double* sVC = sV + (size_t)R * nc * n;               // [R*nc][n]
+  double* sV = sHi + n;                                // [max(R*nc, 8)][ldv]
+  double* sVC = sV + (size_t)vrows * ldv;              // [R*nc][n]
   __shared__ int s_nb;
   const size_t mat = blockIdx.x;
   const double* H = P.H + mat * (size_t)n * n;
@@ -94,16 +104,16 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
   double* T = P.T + mat * (size_t)nE * nc * nc * 2;
 
   if (tid == 0) s_nb = 0;
-  for (int k = tid; k < n; k += kOnThreads) sW[k] = W[k];
+  for (int k = tid; k < n; k += kOnGemmThreads) sW[k] = W[k];
   __syncthreads();
   {  // number of bound states = number of negative eigenvalues (ascending order)
     int cnt = 0;
-    for (int k = tid; k < n; k += kOnThreads) cnt += sW[k] < 0.0;
+    for (int k = tid; k < n; k += kOnGemmThreads) cnt += sW[k] < 0.0;
     if (cnt) atomicAdd(&s_nb, cnt);
   }
   __syncthreads();
   const int nbd = s_nb;
-  for (int k = tid; k < n; k += kOnThreads) {
+  for (int k = tid; k < n; k += kOnGemmThreads) {
     double lo = 0.0, hi = 0.0;
     if (k >= nbd) {
       int br = (k - nbd) % nc, i = (k - nbd) / nc;
@@ -120,7 +130,7 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
     sLo[k] = lo; sHi[k] = hi;
   }
   // energies outside the grid: T = 0
-  for (int e = tid; e < nE; e += kOnThreads)
+  for (int e = tid; e < nE; e += kOnGemmThreads)
     if (P.bin[e] < 0 || (P.mode == 1 && nbd + nc * P.bin[e] + nc - 1 >= n))
       for (int x = 0; x < nc * nc * 2; ++x) T[(size_t)e * nc * nc * 2 + x] = 0.0;
   const int bmin = P.range[0], bmax = P.range[1];
@@ -128,28 +138,81 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
     const int nbins = min(R, bmax - b0 + 1), nrows = nbins * nc;
     __syncthreads();
     // V rows of this chunk: chunk row rr = (b - b0)*nc + alpha  <->  matrix row alpha*N + b
-    for (int e = tid; e < nrows * n; e += kOnThreads) {
+    for (int e = tid; e < nrows * n; e += kOnGemmThreads) {
       int rr = e / n, j = e - rr * n;
       int row = (rr % nc) * N + b0 + rr / nc;
       double v = H[(size_t)row * n + j];
       if (j == row) v -= P.e0[b0 + rr / nc];
-      sV[(size_t)rr * n + j] = v;
+      sV[(size_t)rr * ldv + j] = v;
     }
     __syncthreads();
-    // VC rows: thread per column k, 16 accumulators
-    for (int k = tid; k < n; k += kOnThreads) {
-      double acc[16];
+    // VC rows of the chunk = sV (<= 16 x n) times C (n x n), C read ONCE per chunk (from L2 after the first chunk).
+    if (P.gemm) {
+      // fp64 tensor-core product (mma.sync m8n8k4): a warp takes 32 columns at a time (2 x 4 accumulator tiles); A
+      // fragments from shared memory (row stride ldv = 4 mod 16: conflict-free), B fragments straight from global memory
+      // (lane (g, t) reads C[j0 + t][k0 + 8q + g]: four 64-byte row segments per load), unrolled so that 16 loads per warp
+      // are in flight.
+      const int g = lane >> 2, t = lane & 3, mt = (nrows + 7) >> 3, nfull = n & ~3;
+      for (int grp = warp; grp < ((n + 31) >> 5); grp += nwarps) {
+        const int k0 = grp << 5;
+        double acc[2][4][2];
 #pragma unroll
-      for (int r = 0; r < 16; ++r) acc[r] = 0.0;
-      for (int j = 0; j < n; ++j) {
-        double c = C[(size_t)j * n + k];
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+          for (int q = 0; q < 4; ++q) acc[i][q][0] = acc[i][q][1] = 0.0;
+        const double* a0 = sV + (size_t)g * ldv + t;
+        const double* a1 = a0 + (size_t)8 * ldv;
+        const double* bp = C + (size_t)t * n + k0 + g;
+        bool kin[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) kin[q] = k0 + 8 * q + g < n;
+#pragma unroll 4
+        for (int j0 = 0; j0 < nfull; j0 += 4) {
+          double b[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) b[q] = kin[q] ? __ldg(bp + (size_t)j0 * n + 8 * q) : 0.0;
+          const double av0 = a0[j0], av1 = mt > 1 ? a1[j0] : 0.0;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            dmma(acc[0][q], av0, b[q]);
+            if (mt > 1) dmma(acc[1][q], av1, b[q]);
+          }
+        }
+        if (nfull < n) {  // ragged tail of the contraction index
+          const bool jin = nfull + t < n;
+          const double av0 = jin ? a0[nfull] : 0.0, av1 = (jin && mt > 1) ? a1[nfull] : 0.0;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const double b = (jin && kin[q]) ? __ldg(bp + (size_t)nfull * n + 8 * q) : 0.0;
+            dmma(acc[0][q], av0, b);
+            if (mt > 1) dmma(acc[1][q], av1, b);
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int row = 8 * i + g, col = k0 + 8 * q + 2 * t;
+            if (row < nrows && col < n) sVC[(size_t)row * n + col] = acc[i][q][0];
+            if (row < nrows && col + 1 < n) sVC[(size_t)row * n + col + 1] = acc[i][q][1];
+          }
+      }
+    } else {
+      // very large n (fewer than 8 chunk rows fit shared memory): thread per column k, 16 accumulators
+      for (int k = tid; k < n; k += kOnGemmThreads) {
+        double acc[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) acc[r] = 0.0;
+        for (int j = 0; j < n; ++j) {
+          double c = C[(size_t)j * n + k];
+#pragma unroll
+          for (int r = 0; r < 16; ++r)
+            if (r < nrows) acc[r] = fma(sV[(size_t)r * ldv + j], c, acc[r]);
+        }
 #pragma unroll
         for (int r = 0; r < 16; ++r)
-          if (r < nrows) acc[r] = fma(sV[(size_t)r * n + j], c, acc[r]);
+          if (r < nrows) sVC[(size_t)r * n + k] = acc[r];
       }
-#pragma unroll
-      for (int r = 0; r < 16; ++r)
-        if (r < nrows) sVC[(size_t)r * n + k] = acc[r];
     }
     __syncthreads();
     // energies of this chunk: one warp per energy
@@ -181,12 +244,12 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell(OnshellParams P) {
         }
       }
       if (lane == 0) {
-        const double* v0 = sV + (size_t)((b - b0) * nc) * n;  // row (0, b)
+        const double* v0 = sV + (size_t)((b - b0) * nc) * ldv;  // row (0, b)
         if (nc == 1) {
           T[(size_t)e * 2] = v0[b] + re00;
           T[(size_t)e * 2 + 1] = im00;
         } else {
-          const double* v1 = v0 + n;  // row (1, b)
+          const double* v1 = v0 + ldv;  // row (1, b)
           double* t = T + (size_t)e * 8;
           t[0] = v0[b] + re00;     t[1] = im00;
           t[2] = v0[N + b] + re01; t[3] = im01;
@@ -450,10 +513,11 @@ __global__ void k_sigma(SigmaParams P) {
   P.sigma[idx] = 10.0 * WPCD_PI / (2.0 * p2) * acc;  // fm^2 -> mb
 }
 
-int chunk_bins(int n, int nc, int max_smem) {
-  int R = 16 / nc;  // at most 16 accumulator rows
-  while (R > 1 && (size_t)(3 * n + 2 * R * nc * n) * 8 > (size_t)max_smem - 1024) R >>= 1;
-  return R;
+// Shared memory of k_onshell: eigenvalues and bin edges, the chunk's rows of V (at least 8 rows are laid out: the MMA
+// A fragment spans 8) and of VC.
+size_t onshell_smem(int n, int nc, int R, int ldv) {
+  const int rows = R * nc;
+  return ((size_t)3 * n + (size_t)(rows < 8 ? 8 : rows) * ldv + (size_t)rows * n) * 8;
 }
 
 }  // namespace
@@ -466,9 +530,18 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   OnshellParams P;
   P.e0 = d_e0; P.H = d_H; P.W = d_W; P.C = d_C; P.Ecm = d_Ecm; P.bin = d_bin; P.range = static_cast<int*>(d_work);
   P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE; P.mode = mode;
-  int budget = h->max_smem_optin < 100 * 1024 ? h->max_smem_optin : 100 * 1024;
-  P.R = chunk_bins(P.n, P.nc, budget);
-  size_t smem = (size_t)(3 * P.n + 2 * P.R * P.nc * P.n) * 8;
+  // chunk of 16 (else 8) rows of VC per pass over C on the tensor-core path; beyond that (n > ~1500) the plain loop
+  // with as many bins per chunk as fit
+  const size_t cap = (size_t)h->max_smem_optin - 1024;
+  P.ldv = (P.n + 11) / 16 * 16 + 4;  // == 4 mod 16: conflict-free A fragments
+  P.gemm = 1;
+  P.R = 16 / P.nc;
+  if (onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) P.R = 8 / P.nc;
+  if (onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) {
+    P.gemm = 0; P.ldv = P.n; P.R = 16 / P.nc;
+    while (P.R > 1 && onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) P.R >>= 1;
+  }
+  const size_t smem = onshell_smem(P.n, P.nc, P.R, P.ldv);
   if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   k_bins<<<1, 256, 0, st>>>(N, nE, d_Eedge, d_Ecm, d_bin, static_cast<int*>(d_work));
   if (P.n <= kI1MaxN) {
@@ -477,7 +550,7 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   }
   int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
   if (rc) return rc;
-  k_onshell<<<batch, kOnThreads, smem, st>>>(P);
+  k_onshell<<<batch, kOnGemmThreads, smem, st>>>(P);
   return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
 }
 
