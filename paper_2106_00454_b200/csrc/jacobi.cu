@@ -42,9 +42,6 @@ __device__ long long wpcd_prof[8];
 constexpr int LDQ = 16;   // row stride of a slot's Q (doubles), column pairs XOR-swizzled by the storage row
 constexpr int kQSlot = 16 * LDQ;
 
-// A: XOR swizzle of the column index (bits 2,3) by the row index; row stride must be a multiple of 16 doubles.
-__device__ __forceinline__ int swz(int r, int c) { return c ^ (((r & 6) << 1) ^ ((r & 1) << 3)); }
-
 __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(d[0]), "+d"(d[1])
@@ -58,50 +55,34 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
 __device__ __forceinline__ int qoff(int sr, int c) { return sr * LDQ + 2 * ((c & 7) ^ (2 * (sr & 3))) + (c >> 3); }
 __device__ __forceinline__ int qrow(int k) { return (k & 8) | ((k & 1) << 2) | ((k >> 1) & 3); }
 
-// View of the symmetric working matrix A.
-//   kHalf = false: full np x ld array, XOR-swizzled, both triangles kept up to date (mirror stores).
-//   kHalf = true : only the blocks (rb <= cb) are stored, 64 contiguous doubles each; a block below the diagonal is
-//                  read/written through its transpose.  Halves the footprint: n = 200 fits shared memory.
-//                  Inside a block row r sits in row slot prow(r) = 0,4,1,5,2,6,3,7: a row is 8 doubles = half the
-//                  banks, and with this order the transposed fragment access (rows 2t resp. 2t+1, t = 0..3, column g)
-//                  spreads over both halves -- 2 wavefronts instead of 4-6 -- while the direct access stays
-//                  conflict free.
+// View of the symmetric working matrix A (shared memory in mode 1, global workspace in modes 2 and 3): only the 8x8
+// blocks (rb <= cb) are stored, 64 contiguous doubles each; a block below the diagonal is read/written through its
+// transpose.  Half the footprint of a full mirrored array (which the workspace modes used at first: 20 % slower):
+// n = 200 fits shared memory.  Inside a block row r sits in row slot prow(r) = 0,4,1,5,2,6,3,7: a row is 8 doubles = half
+// the banks, and with this order the transposed fragment access (rows 2t resp. 2t+1, t = 0..3, column g) spreads over
+// both halves -- 2 wavefronts instead of 4-6 -- while the direct access stays conflict free.
 __device__ __forceinline__ int prow(int r) { return ((r & 1) << 2) | (r >> 1); }
 
-template <bool kHalf>
 struct AView {
   double* p;
-  int ld, nb;
+  int nb;
   __device__ __forceinline__ size_t blk(int rb, int cb) const { return (size_t)(rb * nb - ((rb * (rb - 1)) >> 1) + (cb - rb)) << 6; }
   __device__ __forceinline__ double get(int r, int c) const {
-    if (!kHalf) return p[(size_t)r * ld + swz(r, c)];
     const int rb = r >> 3, cb = c >> 3;
     return rb <= cb ? p[blk(rb, cb) + (prow(r & 7) << 3) + (c & 7)] : p[blk(cb, rb) + (prow(c & 7) << 3) + (r & 7)];
   }
   // element (r,c) of a symmetric update where the caller visits BOTH (r,c) and (c,r)
   __device__ __forceinline__ void put(int r, int c, double v) const {
-    if (!kHalf) { p[(size_t)r * ld + swz(r, c)] = v; return; }
     const int rb = r >> 3, cb = c >> 3;
     if (rb <= cb) p[blk(rb, cb) + (prow(r & 7) << 3) + (c & 7)] = v;
   }
   // fragment of the off-diagonal block (rb != cb): rows 8rb+g, columns 8cb+2t, 8cb+2t+1
   __device__ __forceinline__ double2 load_frag(int rb, int cb, int g, int t) const {
-    if (!kHalf) {
-      const int r = 8 * rb + g, c = 8 * cb + 2 * t;
-      return *reinterpret_cast<const double2*>(p + (size_t)r * ld + swz(r, c));
-    }
     if (rb < cb) return *reinterpret_cast<const double2*>(p + blk(rb, cb) + (prow(g) << 3) + 2 * t);
     const double* q = p + blk(cb, rb) + (t << 3) + g;  // rows 2t, 2t+1 of the stored block: slots t, 4+t
     return make_double2(q[0], q[32]);
   }
   __device__ __forceinline__ void store_frag(int rb, int cb, int g, int t, double v0, double v1) const {
-    if (!kHalf) {
-      const int r = 8 * rb + g, c = 8 * cb + 2 * t;
-      *reinterpret_cast<double2*>(p + (size_t)r * ld + swz(r, c)) = make_double2(v0, v1);
-      p[(size_t)c * ld + swz(c, r)] = v0;
-      p[(size_t)(c + 1) * ld + swz(c + 1, r)] = v1;
-      return;
-    }
     if (rb < cb) { *reinterpret_cast<double2*>(p + blk(rb, cb) + (prow(g) << 3) + 2 * t) = make_double2(v0, v1); return; }
     double* q = p + blk(cb, rb) + (t << 3) + g;
     q[0] = v0; q[32] = v1;
@@ -109,7 +90,7 @@ struct AView {
 };
 
 struct Smem {
-  double* A;     // [np][ld] swizzled, full symmetric (shared or global)
+  double* A;     // upper 8x8 blocks of the symmetric working matrix, see AView (shared or global)
   double* V;     // [np][ldv] plain (shared or global)
   double* Q;     // [2][nslots][16][LDQ] (shared or global), double buffered over the steps
   double* wsort; // [np]
@@ -172,8 +153,7 @@ __device__ __forceinline__ int kPiCross(int x) { return (x & 1) ? (((x >> 1) + 1
 // in registers (the columns travel between the lanes of a k0 group by shuffle).  One round = S <- R^T S R, Q <- Q R
 // with R the product of the round's 8 disjoint rotations.  The next round's pivots (a_pp, a_qq, a_pq) are fetched by
 // shuffle right after the update, so that the next rotation (a long dependent chain) overlaps this round's stores.
-template <bool kHalf>
-__device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __restrict__ S, int I, int J, double tol,
+__device__ __forceinline__ bool inner_solve(const AView& A, double* __restrict__ S, int I, int J, double tol,
                                             bool full, int lane) {
   constexpr int LDS_ = 16;  // S is the slot's 16 x LDQ array: a row = all 32 banks
   const int j = lane & 7, k0 = lane >> 3;
@@ -181,7 +161,7 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
   bool need = false;  // early exit: no pair of this sweep passes the rotation test (the usual case in the last sweeps)
   // Lane (h = lane >> 4, gam = lane & 15) moves column gam of the rows 2k + h of S: always the same block of A.
   const int h = lane >> 4, gam = lane & 15, bet = gam & 1;
-  if (kHalf) {
+  {
     const int b = gam >> 1;
     const double* src;
     int stride = 8;
@@ -198,18 +178,6 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
       const int rho = 2 * k + h;
       const double x = S[rho * LDS_ + gam];
       need |= par && (rho < gam) && (x * x > tol2 * fabs(S[rho * (LDS_ + 1)] * dg));
-    }
-  } else {
-    for (int e = lane; e < 256; e += 32) {
-      const int a = e >> 4, b = e & 15;
-      const int r = 8 * ((a & 1) ? J : I) + (a >> 1), c = 8 * ((b & 1) ? J : I) + (b >> 1);
-      S[a * LDS_ + b] = A.get(r, c);
-    }
-    __syncwarp();
-    for (int e = lane; e < 256; e += 32) {
-      const int a = e >> 4, b = e & 15;
-      const double x = S[a * LDS_ + b];
-      need |= (a < b) && (full || ((a ^ b) & 1)) && (x * x > tol2 * fabs(S[a * LDS_ + a] * S[b * LDS_ + b]));
     }
   }
   need = __any_sync(0xffffffffu, need);
@@ -328,8 +296,8 @@ __device__ __forceinline__ bool inner_solve(const AView<kHalf>& A, double* __res
 
 // ---------------------------------------------------------------------------------------------- apply
 // T = A[P1,P2] <- Q1^T T Q2 (P = rows/cols of the slot's one or two blocks), mirrored into A[P2,P1].
-template <bool kHalf, int n1, int n2>
-__device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double* __restrict__ Q1,
+template <int n1, int n2>
+__device__ __forceinline__ void apply_tile_n(const AView& A, const double* __restrict__ Q1,
                                              const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int rb[2] = {I1, J1}, cb[2] = {I2, J2};
@@ -398,13 +366,12 @@ __device__ __forceinline__ void apply_tile_n(const AView<kHalf>& A, const double
 }
 
 // the usual case (two full slots) gets code without predication
-template <bool kHalf>
-__device__ __forceinline__ void apply_tile(const AView<kHalf>& A, const double* __restrict__ Q1,
+__device__ __forceinline__ void apply_tile(const AView& A, const double* __restrict__ Q1,
                                            const double* __restrict__ Q2, int I1, int J1, int I2, int J2, int lane) {
-  if (J1 >= 0 && J2 >= 0) apply_tile_n<kHalf, 2, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
-  else if (J1 >= 0) apply_tile_n<kHalf, 2, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
-  else if (J2 >= 0) apply_tile_n<kHalf, 1, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
-  else apply_tile_n<kHalf, 1, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  if (J1 >= 0 && J2 >= 0) apply_tile_n<2, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else if (J1 >= 0) apply_tile_n<2, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else if (J2 >= 0) apply_tile_n<1, 2>(A, Q1, Q2, I1, J1, I2, J2, lane);
+  else apply_tile_n<1, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
 }
 
 // V[rows of the given row blocks][P] <- V[..][P] Q (V lives in global memory in every mode: L2 latency, so all loads of
@@ -459,11 +426,11 @@ struct JacobiParams {
   double* W;
   double* C;
   int* info;
-  double* gwork;   // per-CTA global workspace: [A np*ld] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
+  double* gwork;   // per-CTA global workspace: [A nb(nb+1)/2 blocks of 64] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
   size_t gstride;  // doubles per CTA
   const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
   int* next;       // global counter of the next matrix to hand out (behind the tables; k_schedule sets it to the grid size)
-  int n, batch, nb, np, ld, ldv, m, nslots, max_sweeps;
+  int n, batch, nb, np, ldv, m, nslots, max_sweeps;
   int nranges, row_lo[4], row_hi[4];  // rows of C that are wanted (nranges = 0: all); the others are returned as zeros
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
@@ -515,8 +482,7 @@ __device__ __forceinline__ void decode_slot(int x, int& I, int& J) {
 template <int kMode>
 __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams& P, int tn, int sn, int bn, bool has_cur,
                                              int t, int bc, int parity, int lane, int widx) {
-  constexpr bool kHalf = true;
-  const AView<kHalf> A{sm.A, P.ld, P.nb};
+  const AView A{sm.A, P.nb};
   const int m = P.m, nslots = P.nslots;
   double* Qn = sm.Q + (size_t)(bn * nslots + sn) * kQSlot;
   int I, J;
@@ -563,10 +529,9 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 template <int kMode, int kThr>
 __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
-  constexpr bool kHalf = true;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = P.n, np = P.np, ld = P.ld, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
+  const int n = P.n, np = P.np, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
   Smem sm;
   {
     double* d = reinterpret_cast<double*>(smem_raw);
@@ -598,7 +563,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   // (Keeping the pivot solves on the warps of two SM sub-partitions and the update queue on the other two was measured
   // slower: the pivots then contend with each other for issue slots and the fp64 pipe.)
   const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
-  const AView<kHalf> Av{sm.A, ld, nb};
+  const AView Av{sm.A, nb};
   const int ntiles = nslots * (nslots - 1) / 2;
   constexpr int kVRowBlocksPerItem = (kMode == 1) ? 4 : 2;
 
@@ -767,7 +732,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
 
 struct Geometry {
   size_t tab_bytes;  // schedule tables at the head of the workspace
-  int nb, np, ld, ldv, m, nslots;
+  int nb, np, ldv, m, nslots;
   int mode;        // k_jacobi<mode, threads>
   int threads;
   size_t gstride;  // doubles of global workspace per CTA
@@ -779,7 +744,6 @@ Geometry geometry(const WpcdHandle* h, int n) {
   g.nb = (n + 7) / 8;
   if (g.nb < 2) g.nb = 2;
   g.np = 8 * g.nb;
-  g.ld = (g.np + 15) / 16 * 16;
   g.ldv = (g.np % 16 == 8) ? g.np : g.np + 8;  // == 8 mod 16: conflict-free row-fragment access without swizzle
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
@@ -788,7 +752,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + 2 * g.np + 4 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
-  const size_t a_full = (size_t)g.np * g.ld * 8, a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
+  const size_t a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
   const size_t cap = (size_t)h->max_smem_optin;
   g.threads = 640;
   const size_t smem1 = misc + tabs + q + a_half;
@@ -832,7 +796,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gstride = g.gstride;
   P.tab = static_cast<const int*>(d_work);
   P.gwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + g.tab_bytes);
-  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ld = g.ld; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
+  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.nranges = n_ranges;
   for (int r = 0; r < 4; ++r) { P.row_lo[r] = r < n_ranges ? h_rows[2 * r] : 0; P.row_hi[r] = r < n_ranges ? h_rows[2 * r + 1] : 0; }
