@@ -377,8 +377,8 @@ __device__ __forceinline__ void apply_tile(const AView& A, const double* __restr
 // V[rows of the given row blocks][P] <- V[..][P] Q (V lives in global memory in every mode: L2 latency, so all loads of
 // a pair of row blocks are in flight before the first product).
 // One V item: row blocks rb[0..nrb-1] of V times the same Q, two row blocks at a time; the Q fragments are loaded once.
-// Items of 4 row blocks where A sits in shared memory (half the queue traffic and Q loads: n=200 6 % faster), 2 where A
-// goes through L2 as well (measured: 4 is 5 % slower at n=400).
+// Items of 4 row blocks (half the queue traffic and Q loads of items of 2: n=200 6 % faster; with A's upper-block layout
+// in the workspace modes too: n=300 3 % faster, together with the interleaved queue order 11 %; items of 8: slower).
 
 template <int nbk>
 __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
@@ -565,7 +565,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   const int widx = warp;  // every warp first solves pivots (slot widx, widx + kPivotWarps, ...), then joins the queue
   const AView Av{sm.A, nb};
   const int ntiles = nslots * (nslots - 1) / 2;
-  constexpr int kVRowBlocksPerItem = (kMode == 1) ? 4 : 2;
+  constexpr int kVRowBlocksPerItem = 4;
 
   // matrices are handed out dynamically (they need 6-8 sweeps each): the first one is the CTA's own index, the next ones
   // come from a global counter that k_schedule set to gridDim.x
@@ -658,7 +658,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
           if (lane == 0) it = atomicAdd(queue, 1);
           it = __shfl_sync(0xffffffffu, it, 0);
           if (it >= nitems) break;
-          if (kMode == 1) {  // V lives in global memory, A in shared: interleave the (L2-latency bound) V items with the tiles
+          {  // interleave the (L2/DRAM-latency bound) V items with the tiles (all modes: n=300 6 % faster than tiles first)
             const int nv = nitems - ntiles, nmix = 2 * (ntiles < nv ? ntiles : nv);
             if (it < nmix) it = (it & 1) ? ntiles + (it >> 1) : (it >> 1);
             else if (nv < ntiles) it -= nv;  // the remaining tiles (remaining V items keep their index)
