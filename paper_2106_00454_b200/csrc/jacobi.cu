@@ -91,7 +91,7 @@ struct AView {
 
 struct Smem {
   double* A;     // upper 8x8 blocks of the symmetric working matrix, see AView (shared or global)
-  double* V;     // [np][ldv] plain (shared or global)
+  double* V;     // [nb][nb] blocks of 8x8 (64 contiguous doubles, row-major inside), global workspace: see vidx
   double* Q;     // [2][nslots][16][LDQ] (shared or global), double buffered over the steps
   double* wsort; // [np]
   int* rot;      // [2][nslots] slot rotated something
@@ -374,6 +374,13 @@ __device__ __forceinline__ void apply_tile(const AView& A, const double* __restr
   else apply_tile_n<1, 1>(A, Q1, Q2, I1, J1, I2, J2, lane);
 }
 
+// V (the accumulated eigenvectors) is kept block-wise: element (r, c) of block (r/8, c/8) at 8 (r%8) + c%8 inside 64
+// contiguous doubles.  An update item then reads and writes whole 512-byte blocks instead of 64-byte pieces of rows
+// 8 ld bytes apart (what the DRAM-bound workspace modes want; the L2-resident shared-memory mode does not care).
+__device__ __forceinline__ size_t vidx(int nb, int r, int c) {
+  return ((size_t)((r >> 3) * nb + (c >> 3)) << 6) + ((r & 7) << 3) + (c & 7);
+}
+
 // V[rows of the given row blocks][P] <- V[..][P] Q (V lives in global memory in every mode: L2 latency, so all loads of
 // a pair of row blocks are in flight before the first product).
 // One V item: row blocks rb[0..nrb-1] of V times the same Q, two row blocks at a time; the Q fragments are loaded once.
@@ -381,7 +388,7 @@ __device__ __forceinline__ void apply_tile(const AView& A, const double* __restr
 // in the workspace modes too: n=300 3 % faster, together with the interleaved queue order 11 %; items of 8: slower).
 
 template <int nbk>
-__device__ __forceinline__ void apply_V_item(double* __restrict__ V, int ld, const double* __restrict__ Q, int I, int J,
+__device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, const double* __restrict__ Q, int I, int J,
                                              const int* __restrict__ rb, int nrb, int lane) {
   const int g = lane >> 2, t = lane & 3;
   const int cb[2] = {I, J};
@@ -393,13 +400,13 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int ld, con
 #pragma unroll 1
   for (int k = 0; k < nrb; k += 2) {
     const bool two = k + 1 < nrb;
-    double* v0 = V + (size_t)(8 * rb[k] + g) * ld + 2 * t;
-    double* v1 = V + (size_t)(8 * rb[two ? k + 1 : k] + g) * ld + 2 * t;
+    double* v0 = V + ((size_t)(rb[k] * nb) << 6) + 8 * g + 2 * t;
+    double* v1 = V + ((size_t)(rb[two ? k + 1 : k] * nb) << 6) + 8 * g + 2 * t;
     double2 f0[2], f1[2];
 #pragma unroll
     for (int c = 0; c < nbk; ++c) {
-      f0[c] = *reinterpret_cast<const double2*>(v0 + 8 * cb[c]);
-      f1[c] = *reinterpret_cast<const double2*>(v1 + 8 * cb[c]);
+      f0[c] = *reinterpret_cast<const double2*>(v0 + 64 * cb[c]);
+      f1[c] = *reinterpret_cast<const double2*>(v1 + 64 * cb[c]);
     }
     double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
@@ -414,8 +421,8 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int ld, con
         }
 #pragma unroll
     for (int ni = 0; ni < nbk; ++ni) {
-      *reinterpret_cast<double2*>(v0 + 8 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
-      if (two) *reinterpret_cast<double2*>(v1 + 8 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+      *reinterpret_cast<double2*>(v0 + 64 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
+      if (two) *reinterpret_cast<double2*>(v1 + 64 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
     }
   }
 }
@@ -426,11 +433,11 @@ struct JacobiParams {
   double* W;
   double* C;
   int* info;
-  double* gwork;   // per-CTA global workspace: [A nb(nb+1)/2 blocks of 64] (modes 2,3) [V np*ldv] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
+  double* gwork;   // per-CTA global workspace: [A nb(nb+1)/2 blocks of 64] (modes 2,3) [V np*np, blocked] (modes 1,2,3) [Q 2*nslots*16*LDQ] (mode 3)
   size_t gstride;  // doubles per CTA
   const int* tab;  // schedule tables written by k_schedule: [m-1][nslots] slots, [m-1][nslots] feeds, [m-1][ntiles] tiles
   int* next;       // global counter of the next matrix to hand out (behind the tables; k_schedule sets it to the grid size)
-  int n, batch, nb, np, ldv, m, nslots, max_sweeps;
+  int n, batch, nb, np, m, nslots, max_sweeps;
   int nranges, row_lo[4], row_hi[4];  // rows of C that are wanted (nranges = 0: all); the others are returned as zeros
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
@@ -531,17 +538,17 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
   constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int n = P.n, np = P.np, ldv = P.ldv, nslots = P.nslots, m = P.m, nb = P.nb;
+  const int n = P.n, np = P.np, nslots = P.nslots, m = P.m, nb = P.nb;
   Smem sm;
   {
     double* d = reinterpret_cast<double*>(smem_raw);
     double* g = P.gwork + (size_t)blockIdx.x * P.gstride;
     if (kMode == 1) {
       sm.A = d; d += (size_t)(nb * (nb + 1) / 2) * 64;
-      sm.V = g; g += (size_t)np * ldv;
+      sm.V = g; g += (size_t)np * np;
     } else {
       sm.A = g; g += (size_t)(nb * (nb + 1) / 2) * 64;
-      sm.V = g; g += (size_t)np * ldv;
+      sm.V = g; g += (size_t)np * np;
     }
     if (kMode == 3) sm.Q = g;
     else { sm.Q = d; d += (size_t)2 * nslots * kQSlot; }
@@ -616,7 +623,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
       int r = e / np, c = e - r * np;
       double a = (r < n && c < n) ? H[(size_t)(sm.perm[r] & 0xFFFF) * n + (sm.perm[c] & 0xFFFF)] : 0.0;
       Av.put(r, c, a);
-      sm.V[(size_t)r * ldv + c] = (r == c) ? 1.0 : 0.0;
+      sm.V[vidx(nb, r, c)] = (r == c) ? 1.0 : 0.0;
     }
     if (tid < 4) sm.ctr[tid] = 0;
     __syncthreads();
@@ -681,8 +688,8 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
             decode_slot(tab_slot[s], I, J);
             const int r0 = kVRowBlocksPerItem * grp;
             const int nrb = nact - r0 < kVRowBlocksPerItem ? nact - r0 : kVRowBlocksPerItem;
-            if (J >= 0) apply_V_item<2>(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
-            else apply_V_item<1>(sm.V, ldv, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
+            if (J >= 0) apply_V_item<2>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
+            else apply_V_item<1>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
           }
         }
 #ifdef WPCD_PROFILE
@@ -719,7 +726,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
       int i = e / n, k = e - i * n;
       int c = sm.src[k];
       const int pi = sm.perm[i];
-      Co[(size_t)(pi & 0xFFFF) * n + k] = (pi >> 16) ? sm.V[(size_t)i * ldv + c] : 0.0;
+      Co[(size_t)(pi & 0xFFFF) * n + k] = (pi >> 16) ? sm.V[vidx(nb, i, c)] : 0.0;
     }
     if (tid == 0) {
       P.info[mat] = converged ? sweeps : -1;
@@ -732,7 +739,7 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
 
 struct Geometry {
   size_t tab_bytes;  // schedule tables at the head of the workspace
-  int nb, np, ldv, m, nslots;
+  int nb, np, m, nslots;
   int mode;        // k_jacobi<mode, threads>
   int threads;
   size_t gstride;  // doubles of global workspace per CTA
@@ -744,7 +751,6 @@ Geometry geometry(const WpcdHandle* h, int n) {
   g.nb = (n + 7) / 8;
   if (g.nb < 2) g.nb = 2;
   g.np = 8 * g.nb;
-  g.ldv = (g.np % 16 == 8) ? g.np : g.np + 8;  // == 8 mod 16: conflict-free row-fragment access without swizzle
   g.m = (g.nb & 1) ? g.nb + 1 : g.nb;
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
@@ -752,7 +758,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + 2 * g.np + 4 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
-  const size_t a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.ldv * 8;
+  const size_t a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.np * 8;
   const size_t cap = (size_t)h->max_smem_optin;
   g.threads = 640;
   const size_t smem1 = misc + tabs + q + a_half;
@@ -796,7 +802,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   P.H = d_A; P.W = d_W; P.C = d_C; P.info = d_info; P.gstride = g.gstride;
   P.tab = static_cast<const int*>(d_work);
   P.gwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + g.tab_bytes);
-  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.ldv = g.ldv; P.m = g.m; P.nslots = g.nslots;
+  P.n = n; P.batch = batch; P.nb = g.nb; P.np = g.np; P.m = g.m; P.nslots = g.nslots;
   P.max_sweeps = max_sweeps;
   P.nranges = n_ranges;
   for (int r = 0; r < 4; ++r) { P.row_lo[r] = r < n_ranges ? h_rows[2 * r] : 0; P.row_hi[r] = r < n_ranges ? h_rows[2 * r + 1] : 0; }
