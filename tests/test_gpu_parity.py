@@ -210,6 +210,29 @@ def test_diag_ragged_sizes_random(ctx, n):
     _diag_check(ctx, A)
 
 
+def test_diag_largest_mode_q_in_workspace(ctx):
+    """Maximum sizes: n = 904 (57 slots) no longer holds the Q buffers in shared memory -- the kernel mode with A, V and Q
+    all in the global workspace.  The oracle's cyclic Jacobi needs minutes at this size, so the check is by what holds
+    at any size: orthonormal C, small residual, trace and Frobenius norm, and the eigenvalues against
+    LAPACK (normwise)."""
+    n = 904
+    rng = np.random.default_rng(n)
+    A = rng.standard_normal((2, n, n)); A = A + A.transpose(0, 2, 1)
+    A[1] *= np.geomspace(1e-3, 1e3, n)[:, None] * np.geomspace(1e-3, 1e3, n)[None, :]   # graded like the Hamiltonians
+    W, C, info = ctx["h"].diag_batched(_to_dev(ctx, A))
+    ctx["torch"].cuda.synchronize()
+    W = W.cpu().numpy(); C = C.cpu().numpy(); info = info.cpu().numpy()
+    for b in range(2):
+        nrm = np.abs(A[b]).max()
+        assert info[b] >= 1
+        assert np.all(np.diff(W[b]) >= 0)
+        assert np.abs(C[b].T @ C[b] - np.eye(n)).max() < 1e-12
+        assert np.abs(A[b] @ C[b] - C[b] * W[b]).max() < 1e-13 * n * nrm
+        assert abs(W[b].sum() - np.trace(A[b])) <= 1e-12 * n * nrm
+        assert abs((W[b] ** 2).sum() - (A[b] ** 2).sum()) <= 1e-12 * (A[b] ** 2).sum()
+        assert np.abs(W[b] - np.linalg.eigvalsh(A[b])).max() <= 1e-11 * np.abs(W[b]).max()
+
+
 def test_diag_degenerate_cases(ctx):
     n = 24
     A = np.zeros((4, n, n))
