@@ -26,7 +26,7 @@ from paper_2106_00454_b200 import inputs as inp  # noqa: E402
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 # DRAM traffic of one Jacobi launch at the bench workload (4096 matrices) from the committed ncu --set full capture
 # (profiles/r1_jacobi_ncu.md), keyed by n; algorithmic minimum = read H + write C + W = 16 n^2 + 8 n bytes per matrix.
-NCU_DRAM_BYTES = {100: 0.657720e9, 200: 3.152912e9}
+NCU_DRAM_BYTES = {100: 0.658889e9, 200: 3.122341e9}
 METRIC = "channel-solves/s (fp64 H diag + on-shell T at all E)"
 CHANNELS = [(0, 0), (1, 1)]   # single 1S0 (n=N) and coupled 3S1-3D1 (n=2N)
 
