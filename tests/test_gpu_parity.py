@@ -257,6 +257,34 @@ def test_onshell_energy_outside_grid_and_empty_like_inputs(ctx):
     assert np.abs(res[0]["T"][0, 0, 1:3] - ref["T"][1:3]).max() < 1e-9 * np.abs(ref["T"][1:3]).max()
 
 
+def test_onshell_largest_n_plain_loop_path(ctx):
+    """Maximum sizes: beyond n ~ 1530 fewer than 8 rows of VC fit shared memory and wpcd_onshell_T leaves the tensor-core
+    product for the plain loop.  The step only needs (H, W, C) of the right shapes, so the inputs are synthetic (no
+    eigen-solve at this size); compared element by element with the oracle's on-shell T on identical inputs."""
+    from oracle import oracle as o
+    N = 1552
+    p = inp.grid_edges(N)
+    e0, dE, Ee = o.fwp(p)
+    rng = np.random.default_rng(N)
+    G = rng.standard_normal((N, N))
+    H = np.diag(e0) + 20.0 * (G + G.T) / np.sqrt(N)
+    V = H.copy(); V[np.arange(N), np.arange(N)] -= e0            # what the kernel forms: V = H - diag(e0)
+    W = np.sort(e0 * (1.0 + 0.01 * rng.standard_normal(N))); W[0] = -2.2   # one bound state
+    Cm = rng.standard_normal((N, N)) / np.sqrt(N)
+    Ecm = np.array([-1.0, 20.0, 20.7, 21.3, 22.0, 1e12])
+    T, bins = ctx["h"].onshell_T(N, False, _to_dev(ctx, e0), _to_dev(ctx, Ee), _to_dev(ctx, H[None]), _to_dev(ctx, W[None]),
+                                 _to_dev(ctx, Cm[None]), _to_dev(ctx, Ecm))
+    ctx["torch"].cuda.synchronize()
+    T = T.cpu().numpy()[0]; T = T[:, 0] + 1j * T[:, 1]
+    Tr, br = o.onshell_T(N, False, Ee, V, W, Cm, Ecm)
+    assert list(bins.cpu().numpy()) == list(br) and br[0] == -1 and br[-1] == -1 and len(set(br[1:5])) == 4
+    assert T[0] == 0 and T[-1] == 0
+    ok = hp.swp_edge_distance(W, 0, Ecm) > hp.EDGE_GUARD
+    ok[0] = ok[-1] = False
+    assert ok.sum() >= 3
+    assert np.abs(T[ok] - Tr[ok]).max() <= 1e-11 * np.abs(Tr[ok]).max()
+
+
 def test_abi_argument_errors(ctx):
     import ctypes as C
     wp = ctx["wpcd"]
