@@ -389,7 +389,7 @@ __device__ __forceinline__ size_t vidx(int nb, int r, int c) {
 
 template <int nbk>
 __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, const double* __restrict__ Q, int I, int J,
-                                             const int* __restrict__ rb, int nrb, int lane) {
+                                             const int* __restrict__ rb, int nrb, int lane, bool kStream) {
   const int g = lane >> 2, t = lane & 3;
   const int cb[2] = {I, J};
   double2 bq[2][2];
@@ -405,8 +405,13 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, con
     double2 f0[2], f1[2];
 #pragma unroll
     for (int c = 0; c < nbk; ++c) {
-      f0[c] = *reinterpret_cast<const double2*>(v0 + 64 * cb[c]);
-      f1[c] = *reinterpret_cast<const double2*>(v1 + 64 * cb[c]);
+      if (kStream) {  // workspace modes, while all CTAs' A blocks together fit L2: V streams through L2 (evict first) and A stays resident
+        f0[c] = __ldcs(reinterpret_cast<const double2*>(v0 + 64 * cb[c]));
+        f1[c] = __ldcs(reinterpret_cast<const double2*>(v1 + 64 * cb[c]));
+      } else {
+        f0[c] = *reinterpret_cast<const double2*>(v0 + 64 * cb[c]);
+        f1[c] = *reinterpret_cast<const double2*>(v1 + 64 * cb[c]);
+      }
     }
     double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
@@ -421,8 +426,13 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, con
         }
 #pragma unroll
     for (int ni = 0; ni < nbk; ++ni) {
-      *reinterpret_cast<double2*>(v0 + 64 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
-      if (two) *reinterpret_cast<double2*>(v1 + 64 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+      if (kStream) {
+        __stcs(reinterpret_cast<double2*>(v0 + 64 * cb[ni]), make_double2(o0[ni][0], o0[ni][1]));
+        if (two) __stcs(reinterpret_cast<double2*>(v1 + 64 * cb[ni]), make_double2(o1[ni][0], o1[ni][1]));
+      } else {
+        *reinterpret_cast<double2*>(v0 + 64 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
+        if (two) *reinterpret_cast<double2*>(v1 + 64 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+      }
     }
   }
 }
@@ -439,6 +449,7 @@ struct JacobiParams {
   int* next;       // global counter of the next matrix to hand out (behind the tables; k_schedule sets it to the grid size)
   int n, batch, nb, np, m, nslots, max_sweeps;
   int nranges, row_lo[4], row_hi[4];  // rows of C that are wanted (nranges = 0: all); the others are returned as zeros
+  int stream_v;    // workspace modes: 1 = V accesses carry the evict-first hint (see wpcd_jacobi_launch)
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
 };
@@ -688,8 +699,8 @@ __global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
             decode_slot(tab_slot[s], I, J);
             const int r0 = kVRowBlocksPerItem * grp;
             const int nrb = nact - r0 < kVRowBlocksPerItem ? nact - r0 : kVRowBlocksPerItem;
-            if (J >= 0) apply_V_item<2>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
-            else apply_V_item<1>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane);
+            if (J >= 0) apply_V_item<2>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane, kMode != 1 && P.stream_v);
+            else apply_V_item<1>(sm.V, nb, Qc + (size_t)s * kQSlot, I, J, sm.act + r0, nrb, lane, kMode != 1 && P.stream_v);
           }
         }
 #ifdef WPCD_PROFILE
@@ -813,6 +824,10 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   const int grid = global_grid(h, g, batch);
+  // Workspace modes: while the A blocks of all CTAs together fit L2 (n <= ~390 with 148 CTAs) V is streamed through it
+  // with the evict-first hint and A stays resident: a third less DRAM traffic (n=300: 320 -> 280 ms per 4096 matrices;
+  // n=600, where A does not fit either, was 4 % slower with the hint).
+  P.stream_v = (size_t)grid * (size_t)(g.nb * (g.nb + 1) / 2) * 512 <= ((size_t)96 << 20);
   if (work_bytes < g.tab_bytes + (size_t)grid * g.gstride * 8) return WPCD_EWORK;
   P.next = reinterpret_cast<int*>(static_cast<char*>(d_work) + g.tab_bytes - 256);
   k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work), P.next, grid);
