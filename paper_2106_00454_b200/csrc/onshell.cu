@@ -2,7 +2,7 @@
 //   k_bins   : FWP bin of every on-shell energy (Eedge_i <= E < Eedge_{i+1}) and the range of bins in use
 //   k_onshell: one CTA per matrix.  Pseudostate bin edges from the sorted eigenvalues (Eq. 23 as printed,
 //              PAPER.md:166-173; bound states eps < 0 separate; coupled channels: two branches by rank parity),
-//              then for chunks of 16 on-shell rows: VC = (H - diag e0) C as fp64 tensor-core products (mma.sync
+//              then for chunks of 32 or 16 on-shell rows: VC = (H - diag e0) C as fp64 tensor-core products (mma.sync
 //              m8n8k4; A fragments from shared memory, B fragments straight from C), and for every energy in the chunk
 //              (one warp per energy, lanes over eigenstates) T = V_ii + sum_k (VC)_ik (VC)_i'k g_k(E) with the
 //              analytic resolvent g_k of Eqs. B.3-B.6 (sign of the printed last line corrected).
@@ -74,6 +74,65 @@ __global__ void k_bins(int N, int nE, const double* __restrict__ Eedge, const do
   }
   __syncthreads();
   if (threadIdx.x == 0) { range[0] = smin; range[1] = smax; }
+}
+
+// Rows of VC for one chunk: sVC[nrows x n] = sV[nrows x n] (row stride ldv) times C (n x n) as fp64 tensor-core products
+// (mma.sync m8n8k4).  A warp takes 8 NT columns at a time (MT x NT accumulator tiles: 2 x 4 for chunks of 16 rows, 4 x 2
+// for chunks of 32 rows, which halve the passes over C where shared memory allows them, n <= ~430); A fragments from
+// shared memory (row stride ldv = 4 mod 16: conflict-free), B fragments straight from global memory (lane (g, t) reads
+// C[j0 + t][k0 + 8q + g]: four 64-byte row segments per load), unrolled so that 4 NT loads per warp are in flight.
+template <int MT, int NT>
+__device__ __forceinline__ void vc_rows_mma(const double* __restrict__ sV, int ldv, const double* __restrict__ C, int n,
+                                            int nrows, double* __restrict__ sVC, int warp, int nwarps, int lane) {
+  const int g = lane >> 2, t = lane & 3, mt = (nrows + 7) >> 3, nfull = n & ~3;
+  constexpr int kCols = 8 * NT;
+  for (int grp = warp; grp < (n + kCols - 1) / kCols; grp += nwarps) {
+    const int k0 = grp * kCols;
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+      for (int q = 0; q < NT; ++q) acc[i][q][0] = acc[i][q][1] = 0.0;
+    const double* a0 = sV + (size_t)g * ldv + t;
+    const double* bp = C + (size_t)t * n + k0 + g;
+    bool kin[NT];
+#pragma unroll
+    for (int q = 0; q < NT; ++q) kin[q] = k0 + 8 * q + g < n;
+#pragma unroll 4
+    for (int j0 = 0; j0 < nfull; j0 += 4) {
+      double b[NT], av[MT];
+#pragma unroll
+      for (int q = 0; q < NT; ++q) b[q] = kin[q] ? __ldg(bp + (size_t)j0 * n + 8 * q) : 0.0;
+#pragma unroll
+      for (int i = 0; i < MT; ++i) av[i] = i < mt ? a0[(size_t)8 * i * ldv + j0] : 0.0;
+#pragma unroll
+      for (int q = 0; q < NT; ++q)
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+          if (i < mt) dmma(acc[i][q], av[i], b[q]);
+    }
+    if (nfull < n) {  // ragged tail of the contraction index
+      const bool jin = nfull + t < n;
+      double av[MT];
+#pragma unroll
+      for (int i = 0; i < MT; ++i) av[i] = (jin && i < mt) ? a0[(size_t)8 * i * ldv + nfull] : 0.0;
+#pragma unroll
+      for (int q = 0; q < NT; ++q) {
+        const double b = (jin && kin[q]) ? __ldg(bp + (size_t)nfull * n + 8 * q) : 0.0;
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+          if (i < mt) dmma(acc[i][q], av[i], b);
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+      for (int q = 0; q < NT; ++q) {
+        const int row = 8 * i + g, col = k0 + 8 * q + 2 * t;
+        if (row < nrows && col < n) sVC[(size_t)row * n + col] = acc[i][q][0];
+        if (row < nrows && col + 1 < n) sVC[(size_t)row * n + col + 1] = acc[i][q][1];
+      }
+  }
 }
 
 struct OnshellParams {
@@ -148,55 +207,8 @@ __global__ void __launch_bounds__(kOnGemmThreads) k_onshell(OnshellParams P) {
     __syncthreads();
     // VC rows of the chunk = sV (<= 16 x n) times C (n x n), C read ONCE per chunk (from L2 after the first chunk).
     if (P.gemm) {
-      // fp64 tensor-core product (mma.sync m8n8k4): a warp takes 32 columns at a time (2 x 4 accumulator tiles); A
-      // fragments from shared memory (row stride ldv = 4 mod 16: conflict-free), B fragments straight from global memory
-      // (lane (g, t) reads C[j0 + t][k0 + 8q + g]: four 64-byte row segments per load), unrolled so that 16 loads per warp
-      // are in flight.
-      const int g = lane >> 2, t = lane & 3, mt = (nrows + 7) >> 3, nfull = n & ~3;
-      for (int grp = warp; grp < ((n + 31) >> 5); grp += nwarps) {
-        const int k0 = grp << 5;
-        double acc[2][4][2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i)
-#pragma unroll
-          for (int q = 0; q < 4; ++q) acc[i][q][0] = acc[i][q][1] = 0.0;
-        const double* a0 = sV + (size_t)g * ldv + t;
-        const double* a1 = a0 + (size_t)8 * ldv;
-        const double* bp = C + (size_t)t * n + k0 + g;
-        bool kin[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) kin[q] = k0 + 8 * q + g < n;
-#pragma unroll 4
-        for (int j0 = 0; j0 < nfull; j0 += 4) {
-          double b[4];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) b[q] = kin[q] ? __ldg(bp + (size_t)j0 * n + 8 * q) : 0.0;
-          const double av0 = a0[j0], av1 = mt > 1 ? a1[j0] : 0.0;
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            dmma(acc[0][q], av0, b[q]);
-            if (mt > 1) dmma(acc[1][q], av1, b[q]);
-          }
-        }
-        if (nfull < n) {  // ragged tail of the contraction index
-          const bool jin = nfull + t < n;
-          const double av0 = jin ? a0[nfull] : 0.0, av1 = (jin && mt > 1) ? a1[nfull] : 0.0;
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const double b = (jin && kin[q]) ? __ldg(bp + (size_t)nfull * n + 8 * q) : 0.0;
-            dmma(acc[0][q], av0, b);
-            if (mt > 1) dmma(acc[1][q], av1, b);
-          }
-        }
-#pragma unroll
-        for (int i = 0; i < 2; ++i)
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int row = 8 * i + g, col = k0 + 8 * q + 2 * t;
-            if (row < nrows && col < n) sVC[(size_t)row * n + col] = acc[i][q][0];
-            if (row < nrows && col + 1 < n) sVC[(size_t)row * n + col + 1] = acc[i][q][1];
-          }
-      }
+      if (R * nc > 16) vc_rows_mma<4, 2>(sV, ldv, C, n, nrows, sVC, warp, nwarps, lane);
+      else vc_rows_mma<2, 4>(sV, ldv, C, n, nrows, sVC, warp, nwarps, lane);
     } else {
       // very large n (fewer than 8 chunk rows fit shared memory): thread per column k, 16 accumulators
       for (int k = tid; k < n; k += kOnGemmThreads) {
@@ -530,12 +542,13 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   OnshellParams P;
   P.e0 = d_e0; P.H = d_H; P.W = d_W; P.C = d_C; P.Ecm = d_Ecm; P.bin = d_bin; P.range = static_cast<int*>(d_work);
   P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE; P.mode = mode;
-  // chunk of 16 (else 8) rows of VC per pass over C on the tensor-core path; beyond that (n > ~1500) the plain loop
+  // chunk of 32 (else 16, else 8) rows of VC per pass over C on the tensor-core path; beyond that (n > ~1500) the plain loop
   // with as many bins per chunk as fit
   const size_t cap = (size_t)h->max_smem_optin - 1024;
   P.ldv = (P.n + 11) / 16 * 16 + 4;  // == 4 mod 16: conflict-free A fragments
   P.gemm = 1;
-  P.R = 16 / P.nc;
+  P.R = 32 / P.nc;
+  if (onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) P.R = 16 / P.nc;
   if (onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) P.R = 8 / P.nc;
   if (onshell_smem(P.n, P.nc, P.R, P.ldv) > cap) {
     P.gemm = 0; P.ldv = P.n; P.R = 16 / P.nc;
