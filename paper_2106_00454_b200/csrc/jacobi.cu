@@ -542,10 +542,11 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 //       3: as 2 with Q in the global workspace too (very large n)
 // The pivot scratch is always the slot's own Q array.
 // kThr: 640 threads (one CTA per SM; 20 warps at 96 registers measured faster than 16 at 128 or 24 at 80), or 320 /
-// 160 (two / four CTAs per SM) where shared memory allows and a step has no more pivots than the CTA has warps:
+// 160 / 128 (two / four / five CTAs per SM; 128 for n <= 64: 1.45 -> 1.31 ms at n=32, 2.52 -> 2.20 at n=48, 3.28 -> 3.09
+// at n=64 per 4096 matrices) where shared memory allows and a step has no more pivots than the CTA has warps:
 // several matrices in flight per SM fill each other's pivot-chain bubbles.
 template <int kMode, int kThr>
-__global__ void __launch_bounds__(kThr, 640 / kThr) k_jacobi(JacobiParams P) {
+__global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(JacobiParams P) {
   constexpr int kThreads = kThr, kPivotWarps = kThr / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -773,7 +774,8 @@ Geometry geometry(const WpcdHandle* h, int n) {
   const size_t cap = (size_t)h->max_smem_optin;
   g.threads = 640;
   const size_t smem1 = misc + tabs + q + a_half;
-  if (g.nslots <= 5 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 160; g.smem = smem1; g.gstride = v / 8; }
+  if (g.nslots <= 4 && 5 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 128; g.smem = smem1; g.gstride = v / 8; }
+  else if (g.nslots <= 5 && 4 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 160; g.smem = smem1; g.gstride = v / 8; }
   else if (g.nslots <= 10 && 2 * (smem1 + 1024) <= cap) { g.mode = 1; g.threads = 320; g.smem = smem1; g.gstride = v / 8; }
   else if (misc + tabs + q + a_half <= cap) { g.mode = 1; g.smem = misc + tabs + q + a_half; g.gstride = v / 8; }
   else if (misc + q <= cap) { g.mode = 2; g.smem = misc + q; g.gstride = (a_half + v) / 8; }
@@ -785,7 +787,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
 // workspace.  All workspaces together must stay inside L2 (measured: a 100 MB working set already spills to HBM -- the
 // 126 MB L2 is split over two dies); the mode-1 sets are 25-50 MB.
 int global_grid(const WpcdHandle* h, const Geometry& g, int batch) {
-  const int grid = (640 / g.threads) * h->num_sms;
+  const int grid = (g.threads == 128 ? 5 : 640 / g.threads) * h->num_sms;
   return batch < grid ? batch : grid;
 }
 
@@ -834,7 +836,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   int rc;
   switch (g.mode) {
     case 1:
-      rc = g.threads == 160   ? launch_mode<1, 160>(h, P, grid, g.smem, st)
+      rc = g.threads == 128   ? launch_mode<1, 128>(h, P, grid, g.smem, st)
+           : g.threads == 160 ? launch_mode<1, 160>(h, P, grid, g.smem, st)
            : g.threads == 320 ? launch_mode<1, 320>(h, P, grid, g.smem, st)
                               : launch_mode<1, 640>(h, P, grid, g.smem, st);
       break;
