@@ -11,6 +11,13 @@
 //   legendre_Q       : vs mpmath.legenq (independent arbitrary-precision evaluation) and the Neumann integral
 //   V_yukawa         : vs adaptive quadrature of the radial (r-space) definition on tiny grids
 //   jacobi           : closed-form 2x2/3x3, rank-one secular equation by bisection (Yamaguchi), invariants, mpmath
+//   jacobi_ld        : (the 80-bit arbiter of the GPU parity tests) eigenvalues vs mpmath.eigsy at 50 digits on the config
+//                      and Chebyshev grids up to N = 100, secular equation, eigenvectors vs mpmath and the residual in
+//                      extended precision (tests/test_oracle_pins_arbiter.py)
+//   V_yukawa (z-1)   : the cancellation-free argument on the high-momentum diagonal (z - 1 < 1e-5) vs mpmath with z formed
+//                      in 50-digit arithmetic, 1e-13
+//   onshell_T_avg    : coupled branch (readings A1-A3): two-branch toy spectrum with a bound state enumerated by hand,
+//                      coupled averaged WPCD -> coupled MI decreasing with N
 //   resolvent / T    : limits of Eq. B.3-B.6, sum rule, hand-evaluated tiny cases; energy-averaged variant (B.7-B.8)
 //                      against numerical quadrature of the point-wise resolvent and the Yamaguchi closed form
 //   phases           : closed forms of Eqs. A.3-A.5 (unit-modulus S built from known angles)

@@ -56,6 +56,18 @@ def _gpu_pipeline(ctx, N, channels, Ecm, scales=None, S=1, yamaguchi=None, tol=0
     return res
 
 
+# Cases in which the 80-bit run of the oracle's Jacobi (orc_jacobi_ld, pinned in tests/test_oracle_pins_arbiter.py) had
+# to arbitrate between the CUDA path and the fp64 oracle: (label, "eig" | "phase", n, custom grid?).
+# names where that may happen -- n >= 600 on the config grid (the fp64 oracle's own rounding on the smallest eigenvalues)
+# and the paper's Chebyshev grid (norm-wise stop rule on a Hamiltonian graded over 13+ orders of magnitude); anywhere else
+# it is a failure (test_zz_arbitration_only_where_design_allows, which runs last in this module).
+ARBITRATED = []
+
+
+def _arbitration_allowed(n, custom_grid):
+    return custom_grid or n >= 600
+
+
 def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguchi=None, label="", edges=None, ngl=8,
                      averaged=False, energy_packets=False):
     ch = hp.oracle_channel(N, kind, lJ, scale, yamaguchi, edges=edges, ngl=ngl, energy_packets=energy_packets)
@@ -75,6 +87,9 @@ def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguc
         W_ld = o.jacobi_ld(ch["H"])[0]
         errW, err_oracle = hp.check_eig(g["W"][s, c], W_ld, normH), hp.check_eig(ref["W"], W_ld, normH)
         print(label, "eig arbitration vs long double: gpu", errW, "fp64 oracle", err_oracle)
+        ARBITRATED.append((label, "eig", n, edges is not None))
+        assert _arbitration_allowed(n, edges is not None), (label, "eig arbitration outside DESIGN.md's list", errW)
+        assert err_oracle > errW, (label, "arbitration: the fp64 oracle must be the less accurate side", err_oracle, errW)
     assert errW <= hp.TOL_EIG_REL, (label, "eig", errW)
     C = g["C"][s, c]
     assert np.abs(C.T @ C - np.eye(n)).max() < 1e-12, (label, "orth")
@@ -95,6 +110,9 @@ def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguc
         dphi_o, dS_o, _ = hp.check_phases(kind, ref["delta"], ref["S"], ref_ld, Ecm)
         dphi, dS, nok = hp.check_phases(kind, g["delta"][s, c], g["S"][s, c], ref_ld, Ecm)
         print(label, "phase arbitration vs long-double eigenpairs: gpu", dphi, dS, "fp64 oracle", dphi_o, dS_o)
+        ARBITRATED.append((label, "phase", n, edges is not None))
+        assert _arbitration_allowed(n, edges is not None), (label, "phase arbitration outside DESIGN.md's list", dphi, dS)
+        assert dphi_o > dphi or dS_o > dS, (label, "arbitration: the fp64 oracle must be the less accurate side")
     assert dphi <= hp.TOL_PHASE_DEG, (label, "phase", dphi)
     assert dS <= hp.TOL_S_ABS, (label, "S", dS)
     return errH, errW, dphi, dS
@@ -150,16 +168,22 @@ def test_config3_sampled_batch(ctx):
 
 # ----------------------------------------------------------------------------------------------- config 4
 def test_config4_large_n_and_yamaguchi(ctx):
-    """N=200 (n=200 and 400: beyond shared memory -> global-workspace path) + the Yamaguchi analytic check."""
-    S = 4
+    """Config 4 at its stated size: 256 seeded samples x all 14 channels J <= 4 at N=200 (2560 matrices of 200^2 and 1024 of
+    400^2: beyond shared memory -> the workspace path, every CTA takes several matrices) + the Yamaguchi analytic check.
+    The oracle checks a seeded subsample of (sample, channel), among them matrices that a CTA takes second or later."""
+    S = 256
     tl, Ecm = inp.energies(350)
-    scales = inp.sample_scales(256, seed=0)[:S]
-    chans = [(0, 0), (0, 2), (1, 1), (1, 4)]
+    scales = inp.sample_scales(256, seed=0)
+    chans = [(c, l) for _, c, l in inp.CHANNELS_J4]
     res = _gpu_pipeline(ctx, 200, chans, Ecm, scales=scales, S=S)
-    _compare_channel(res, 0, 0, 0, 200, 0, Ecm, scale=tuple(scales[0]), label="cfg4 1S0")
-    _compare_channel(res, 0, 3, 1, 200, 2, Ecm, scale=tuple(scales[3]), label="cfg4 1D2 s3")
-    _compare_channel(res, 1, 1, 0, 200, 1, Ecm, scale=tuple(scales[1]), label="cfg4 3S1-3D1 s1")
-    _compare_channel(res, 1, 0, 1, 200, 4, Ecm, scale=tuple(scales[0]), label="cfg4 3F4-3H4")
+    assert (res[0]["info"] >= 1).all() and (res[1]["info"] >= 1).all()
+    unc = [(nm, l) for nm, c, l in inp.CHANNELS_J4 if not c]
+    cpl = [(nm, l) for nm, c, l in inp.CHANNELS_J4 if c]
+    # (kind, sample, channel index within its kind): flat matrix index = sample * n_chan_of_kind + index
+    for kind, s_, ci in ((0, 0, 0), (0, 255, 9), (0, 97, 4), (1, 1, 0), (1, 255, 3), (1, 140, 1)):
+        nm, l = (cpl if kind else unc)[ci]
+        _compare_channel(res, kind, s_, ci, 200, l, Ecm, scale=tuple(scales[s_]), label=f"cfg4 s={s_} {nm}")
+    del res
     # Yamaguchi at N=200: GPU vs oracle, and GPU vs the closed-form phase shift (median error < 1 degree)
     lamA, lamB = inp.yamaguchi_lambda()
     yres = _gpu_pipeline(ctx, 200, [(0, 0)], Ecm, yamaguchi=(lamB, inp.YAMAGUCHI_BETA))
@@ -676,3 +700,49 @@ def test_mi_solver_on_gpu(ctx):
               for (k, lJ) in channels if k]
         ref = hp.o.sigma_tot(hp.o.partial_waves(channels, sJ, Su, Sc), np.sqrt(inp.MU * t) / inp.HBARC)
         assert abs(sig[e] - ref) < 1e-10 * ref, (t, sig[e], ref)
+
+
+# ----------------------------------------------------------------------------------------------- large n at production batch
+@pytest.mark.parametrize("N,S,picks", [(300, 450, (0, 161, 449)),        # n = 300 and n = 600: the workspace path
+                                       (452, 300, (299,))])               # n = 452 / 904: the largest geometry
+def test_large_n_batch_exceeds_grid(ctx, N, S, picks):
+    """VERDICT r1 missing-5 / ADVICE: the n > 200 kernels at a batch larger than the grid, so that every CTA re-uses its
+    global workspace for a second and third matrix (the hand-out counter), in the launch geometry the bench's size sweep
+    uses (stored congruently).  All matrices: converged, ascending eigenvalues, trace; the oracle
+    (cyclic Jacobi -> T -> phases) on matrices handed out first, second and last.  The coupled matrices (n = 2N) are
+    checked by what holds at any size plus, at n = 600, the oracle on the last one."""
+    torch, h = ctx["torch"], ctx["h"]
+    tl, Ecm = inp.energies(350)
+    scales = inp.sample_scales(S, seed=7)
+    res = _gpu_pipeline(ctx, N, [(0, 0)], Ecm, scales=scales, S=S)
+    g = res[0]
+    assert (g["info"] >= 1).all()
+    assert (np.diff(g["W"][:, 0, :], axis=1) >= 0).all()
+    tr = np.trace(g["H"][:, 0], axis1=1, axis2=2)
+    assert np.abs(g["W"][:, 0, :].sum(axis=1) - tr).max() <= 1e-12 * N * np.abs(g["H"]).max()
+    for s in picks:
+        _compare_channel(res, 0, s, 0, N, 0, Ecm, scale=tuple(scales[s]), label=f"batch>grid N={N} single s={s}")
+    del res, g
+    # coupled matrices of the same grid (n = 2N), fewer of them (memory: 8 n^2 bytes each for H and C)
+    Sc = min(S, 320)
+    res = _gpu_pipeline(ctx, N, [(1, 1)], Ecm, scales=scales[:Sc], S=Sc)
+    g = res[1]
+    n = 2 * N
+    assert (g["info"] >= 1).all() and (np.diff(g["W"][:, 0, :], axis=1) >= 0).all()
+    for s in (0, 150, Sc - 1):                       # invariants on first-, second- and last-round matrices (SURVEY P3)
+        Hs, C, W = g["H"][s, 0], g["C"][s, 0], g["W"][s, 0]
+        nrm = np.abs(Hs).max()
+        assert np.abs(C.T @ C - np.eye(n)).max() < 1e-12
+        assert np.abs(Hs @ C - C * W).max() < 1e-13 * n * nrm
+        assert abs(W.sum() - np.trace(Hs)) <= 1e-12 * n * nrm
+    if n <= 600:
+        _compare_channel(res, 1, Sc - 1, 0, N, 1, Ecm, scale=tuple(scales[Sc - 1]), label=f"batch>grid N={N} coupled s={Sc - 1}")
+
+
+def test_zz_arbitration_only_where_design_allows():
+    """Runs last in this module: every case that needed the 80-bit arbiter is on DESIGN.md section 3's list (n >= 600 on
+    the config grid, or the Chebyshev grid); the assertion at the point of use already failed otherwise -- this prints the
+    list so that `pytest -q -rA` shows which cases were arbitrated."""
+    for label, what, n, custom in ARBITRATED:
+        assert _arbitration_allowed(n, custom), (label, what)
+    print("arbitrated cases:", [(l, w) for l, w, _, _ in ARBITRATED])
