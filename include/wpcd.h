@@ -43,6 +43,8 @@ extern "C" {
 
 #define WPCD_MAX_CHANNELS 16
 #define WPCD_MAX_TERMS 4
+#define WPCD_MAX_L 6 /* largest orbital angular momentum l (coupled channels use l = J+1): the range over which the Q_l
+                        evaluation is held to 1e-12 of an independent one (reading C7); beyond: WPCD_ESIZE */
 
 /* Local potential = sum of Yukawas V(r) = sum_t V0_t exp(-mu_t r)/r, projected on partial wave l with the Legendre
  * function of the second kind: <k'|v_l|k> = (1/pi) sum_t V0_t Q_l(z_t)/(k'k), z_t = (k'^2+k^2+mu_t^2)/(2k'k)
@@ -75,7 +77,9 @@ typedef struct {
                                exactly, e_i = E_i + dE_i/2, and Eq. 29 carries the extra factor f(k')f(k) */
 } wpcd_grid;
 
-/* Handle: owns only immutable device tables.  One handle per host thread/stream.  device = CUDA ordinal. */
+/* Handle: owns only immutable device tables.  One handle per host thread/stream.  device = CUDA ordinal.
+ * Every compute call launches on the CALLER's current device and stream: the current device (cudaGetDevice) must be the
+ * handle's device, else the call returns WPCD_EINVAL before any launch. */
 int wpcd_create(void** handle, int device);
 void wpcd_destroy(void* handle);
 const char* wpcd_strerror(int code);
@@ -205,6 +209,14 @@ size_t wpcd_mi_workspace_bytes(void* handle, int NQ);
 int wpcd_mi_solve(void* handle, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales, int S,
                   int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
                   double* d_S_cpl, void* d_work, size_t work_bytes, void* stream);
+
+/* Measurement aid (bench.py "roofline.peak_measured"): one launch of register-only fp64 chains on every SM -- kind 0: eight
+ * independent DFMA chains per thread, kind 1: eight independent mma.sync.m8n8k4.f64 accumulator chains per warp --
+ * `iters` dependent steps each, 2 CTAs of 512 threads per SM.  The caller times the launch with events on `stream`.
+ *   d_sink  : [wpcd_probe_sink_elems(handle)] doubles, written once at the end (keeps the chains alive)
+ *   h_flops : host out, flops executed by the launch (FMA = 2) */
+size_t wpcd_probe_sink_elems(void* handle);
+int wpcd_probe_fp64(void* handle, int kind, int iters, double* d_sink, double* h_flops, void* stream);
 
 /* Test hooks (host only, no GPU needed): the block tournament that wpcd_diag_batched runs (csrc/jacobi_schedule.cuh).
  * m = number of players (8-wide blocks, even, >= 6; players >= nb are padding), a sweep has m-1 steps of m/2 slots.

@@ -61,6 +61,49 @@ size_t wpcd_onshell_workspace_bytes(void* handle, int N, int coupled, int batch,
 
 static bool aligned16(const void* p) { return (reinterpret_cast<size_t>(p) & 15) == 0; }
 
+// Every compute call acts on the CALLER's current device (launches, function attributes, the caller's stream and
+// buffers): it must be the device the handle was created for (include/wpcd.h, "Handle").
+static bool on_handle_device(const WpcdHandle* h) {
+  int cur = -1;
+  return cudaGetDevice(&cur) == cudaSuccess && cur == h->device;
+}
+
+// Checks of a wpcd_potential and a channel list shared by wpcd_build_channels and wpcd_mi_solve, so that the same struct
+// behaves the same way in both: term counts, positive ranges, scale columns inside [0, P) and backed by d_scales,
+// partial waves inside the range the Q_l evaluation is pinned for (reading C7: l <= WPCD_MAX_L).
+static int check_potential_channels(const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales,
+                                    int P, int* n_unc_out, int* n_cpl_out) {
+  if (!pot || !chan || n_chan < 1 || P < 0) return WPCD_EINVAL;
+  if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
+  if (P > 0 && !d_scales) return WPCD_EINVAL;
+  if (pot->kind != 0 && pot->kind != 1) return WPCD_EINVAL;
+  if (pot->kind == 0) {
+    if (pot->n_terms < 1 || !pot->V0 || !pot->mu) return WPCD_EINVAL;
+    if (pot->n_terms > WPCD_MAX_TERMS) return WPCD_ESIZE;
+    for (int t = 0; t < pot->n_terms; ++t) {
+      if (!(pot->mu[t] > 0)) return WPCD_EINVAL;
+      if (pot->scale_idx && (pot->scale_idx[t] >= P || (pot->scale_idx[t] >= 0 && !d_scales))) return WPCD_EINVAL;
+    }
+    if (pot->VT_scale_idx >= P || (pot->VT_scale_idx >= 0 && !d_scales)) return WPCD_EINVAL;
+  } else {
+    if (!(pot->beta > 0)) return WPCD_EINVAL;
+  }
+  int n_unc = 0, n_cpl = 0;
+  for (int c = 0; c < n_chan; ++c) {
+    if (chan[c].coupled) {
+      if (chan[c].lJ < 1 || pot->kind == 1 || !(pot->muT > 0)) return WPCD_EINVAL;
+      if (chan[c].lJ + 1 > WPCD_MAX_L) return WPCD_ESIZE;
+      ++n_cpl;
+    } else {
+      if (chan[c].lJ < 0) return WPCD_EINVAL;
+      if (chan[c].lJ > WPCD_MAX_L) return WPCD_ESIZE;
+      ++n_unc;
+    }
+  }
+  *n_unc_out = n_unc; *n_cpl_out = n_cpl;
+  return WPCD_OK;
+}
+
 int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potential* pot, const wpcd_channel* chan,
                         int n_chan, const double* d_scales, int S, int P, double* d_H_unc, double* d_H_cpl,
                         double* d_e0, double* d_dE, double* d_Eedge, void* d_work, size_t work_bytes, void* stream) {
@@ -69,34 +112,13 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
   if (grid->N < 1 || !grid->h_edges || grid->n_gl < 1 || grid->n_gl > 16 || !(grid->hbarc > 0) || !(grid->mu > 0)) return WPCD_EINVAL;
   if (grid->wp_kind != 0 && grid->wp_kind != 1) return WPCD_EINVAL;
   if (grid->N > 4096) return WPCD_ESIZE;  // 32-bit element indices in the assembly kernels (n = 2N <= 8192)
-  if (n_chan < 1 || S < 1 || P < 0 || (P > 0 && !d_scales)) return WPCD_EINVAL;
-  if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
+  if (S < 1) return WPCD_EINVAL;
   if (!(grid->h_edges[0] >= 0)) return WPCD_EINVAL;
   for (int i = 0; i < grid->N; ++i)
     if (!(grid->h_edges[i + 1] > grid->h_edges[i])) return WPCD_EINVAL;
-  if (pot->kind != 0 && pot->kind != 1) return WPCD_EINVAL;
-  if (pot->kind == 0) {
-    if (pot->n_terms < 1 || !pot->V0 || !pot->mu) return WPCD_EINVAL;
-    if (pot->n_terms > WPCD_MAX_TERMS) return WPCD_ESIZE;
-    for (int t = 0; t < pot->n_terms; ++t) {
-      if (!(pot->mu[t] > 0)) return WPCD_EINVAL;
-      if (pot->scale_idx && pot->scale_idx[t] >= P) return WPCD_EINVAL;
-    }
-    if (pot->VT_scale_idx >= P) return WPCD_EINVAL;
-  } else {
-    if (!(pot->beta > 0)) return WPCD_EINVAL;
-  }
   int n_unc = 0, n_cpl = 0;
-  for (int c = 0; c < n_chan; ++c) {
-    if (chan[c].coupled) {
-      if (chan[c].lJ < 1 || pot->kind == 1 || !(pot->muT > 0)) return WPCD_EINVAL;
-      ++n_cpl;
-    } else {
-      if (chan[c].lJ < 0) return WPCD_EINVAL;
-      ++n_unc;
-    }
-    if (chan[c].lJ > 20) return WPCD_ESIZE;
-  }
+  if (int rc = check_potential_channels(pot, chan, n_chan, d_scales, P, &n_unc, &n_cpl)) return rc;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   if ((n_unc && !d_H_unc) || (n_cpl && !d_H_cpl)) return WPCD_EINVAL;
   if (!aligned16(d_H_unc) || !aligned16(d_H_cpl) || !aligned16(d_work)) return WPCD_EINVAL;
   if (work_bytes < wpcd_build_workspace(grid->N, n_chan) || (!d_work && wpcd_build_workspace(grid->N, n_chan))) return WPCD_EWORK;
@@ -114,6 +136,7 @@ int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double*
     if (h_rows[2 * r] < 0 || h_rows[2 * r + 1] > n || h_rows[2 * r] >= h_rows[2 * r + 1]) return WPCD_EINVAL;
   if (n < 2 || n > 4096) return WPCD_ESIZE;
   if (!aligned16(d_A) || !aligned16(d_C) || !aligned16(d_work)) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   size_t need = wpcd_jacobi_workspace(h, n, batch);
   if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
   return wpcd_jacobi_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, h_rows, n_ranges, d_work, work_bytes,
@@ -126,6 +149,7 @@ int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !d_e0 || !d_Eedge || !d_H || !d_W || !d_C || !d_Ecm || !d_T || !d_bin) return WPCD_EINVAL;
   if (N < 1 || batch < 1 || nE < 1 || (mode != 0 && mode != 1)) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   size_t need = wpcd_onshell_workspace(N, coupled, batch, nE);
   if (work_bytes < need || (need && !d_work)) return WPCD_EWORK;
   return wpcd_onshell_launch(h, N, coupled ? 1 : 0, batch, d_e0, d_Eedge, d_H, d_W, d_C, d_Ecm, nE, mode, d_T, d_bin,
@@ -136,16 +160,16 @@ int wpcd_phase_shifts(void* handle, int coupled, int batch, int nE, const double
                       const double* d_dE, double* d_delta, double* d_S, void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !d_T || !d_bin || !d_dE || !d_delta || batch < 1 || nE < 1) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   return wpcd_phase_launch(h, coupled ? 1 : 0, batch, nE, d_T, d_bin, d_dE, d_delta, d_S,
                            static_cast<cudaStream_t>(stream));
 }
-
-}  // extern "C"
 
 int wpcd_interp_phases(void* handle, int coupled, int batch, int N, const double* d_pedge, const double* d_delta_mid,
                        const double* d_q, int nq, double* d_out, void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !d_pedge || !d_delta_mid || !d_q || !d_out || batch < 1 || N < 1 || nq < 1) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   return wpcd_interp_launch(h, coupled ? 1 : 0, batch, N, d_pedge, d_delta_mid, d_q, nq, d_out,
                             static_cast<cudaStream_t>(stream));
 }
@@ -160,6 +184,7 @@ int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, c
   if (n_unc > WPCD_MAX_CHANNELS || n_cpl > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
   for (int c = 0; c < n_unc; ++c) if (h_J_unc[c] < 0) return WPCD_EINVAL;
   for (int c = 0; c < n_cpl; ++c) if (h_J_cpl[c] < 1) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   return wpcd_sigma_launch(h, S, nE, n_unc, h_J_unc, d_T_unc, n_cpl, h_J_cpl, d_T_cpl, d_bin, d_dE, d_Ecm, hbarc, mu, d_sigma,
                            static_cast<cudaStream_t>(stream));
 }
@@ -174,21 +199,10 @@ int wpcd_mi_solve(void* handle, const wpcd_potential* pot, const wpcd_channel* c
                   double* d_S_cpl, void* d_work, size_t work_bytes, void* stream) {
   WpcdHandle* h = static_cast<WpcdHandle*>(handle);
   if (!h || !pot || !chan || n_chan < 1 || S < 1 || nE < 1 || !d_Ecm || NQ < 2 || !(cmap > 0) || !(hbarc > 0) || !(mu > 0)) return WPCD_EINVAL;
-  if (n_chan > WPCD_MAX_CHANNELS) return WPCD_ESIZE;
-  if (pot->kind != 0 && pot->kind != 1) return WPCD_EINVAL;
-  if (pot->kind == 0 && (pot->n_terms < 1 || pot->n_terms > WPCD_MAX_TERMS || !pot->V0 || !pot->mu)) return WPCD_EINVAL;
   if (d_scales && P < 1) return WPCD_EINVAL;
   int n_unc = 0, n_cpl = 0;
-  for (int c = 0; c < n_chan; ++c) {
-    if (chan[c].coupled) {
-      if (chan[c].lJ < 1 || pot->kind == 1 || !(pot->muT > 0)) return WPCD_EINVAL;
-      ++n_cpl;
-    } else {
-      if (chan[c].lJ < 0) return WPCD_EINVAL;
-      ++n_unc;
-    }
-    if (chan[c].lJ > 20) return WPCD_ESIZE;
-  }
+  if (int rc = check_potential_channels(pot, chan, n_chan, d_scales, P, &n_unc, &n_cpl)) return rc;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
   if ((n_unc && !d_S_unc) || (n_cpl && !d_S_cpl)) return WPCD_EINVAL;
   if ((n_unc && !wpcd_mi_fits(h, NQ, 0)) || (n_cpl && !wpcd_mi_fits(h, NQ, 1))) return WPCD_ESIZE;
   if (!d_work || work_bytes < wpcd_mi_workspace(NQ)) return WPCD_EWORK;
@@ -196,7 +210,18 @@ int wpcd_mi_solve(void* handle, const wpcd_potential* pot, const wpcd_channel* c
                         static_cast<cudaStream_t>(stream));
 }
 
+size_t wpcd_probe_sink_elems(void* handle) { return handle ? wpcd_probe_sink(static_cast<WpcdHandle*>(handle)) : 0; }
+
+int wpcd_probe_fp64(void* handle, int kind, int iters, double* d_sink, double* h_flops, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || (kind != 0 && kind != 1) || iters < 1 || !d_sink || !h_flops) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
+  return wpcd_probe_launch(h, kind, iters, d_sink, h_flops, static_cast<cudaStream_t>(stream));
+}
+
 int wpcd_onshell_rows(const wpcd_grid* grid, int coupled, const double* h_Ecm, int nE, int* h_rows, int* n_ranges) {
   if (!grid || !grid->h_edges || grid->N < 1 || !h_Ecm || nE < 1 || !h_rows || !n_ranges) return WPCD_EINVAL;
   return wpcd_onshell_rows_host(grid->N, coupled ? 1 : 0, grid->h_edges, grid->hbarc, grid->mu, h_Ecm, nE, h_rows, n_ranges);
 }
+
+}  // extern "C"

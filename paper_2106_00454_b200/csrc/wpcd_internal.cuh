@@ -47,3 +47,6 @@ bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled);
 int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales,
                    int S, int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
                    double* d_S_cpl, void* d_work, cudaStream_t st);
+// probe.cu
+size_t wpcd_probe_sink(const WpcdHandle* h);
+int wpcd_probe_launch(WpcdHandle* h, int kind, int iters, double* d_sink, double* h_flops, cudaStream_t st);

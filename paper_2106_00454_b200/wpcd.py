@@ -67,17 +67,23 @@ _lib.wpcd_mi_solve.argtypes = [_vp, C.POINTER(Potential), C.POINTER(Channel), _i
                                _vp, _vp, _sz, _vp]
 _lib.wpcd_mi_solve.restype = _i
 
+_lib.wpcd_probe_sink_elems.argtypes = [_vp]; _lib.wpcd_probe_sink_elems.restype = _sz
+_lib.wpcd_probe_fp64.argtypes = [_vp, _i, _i, _vp, C.POINTER(_d), _vp]; _lib.wpcd_probe_fp64.restype = _i
+
+# every symbol include/wpcd.h declares (tests/test_abi_cpu.py compares this list with the header and the library)
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
-           "wpcd_build_channels", "wpcd_diag_batched", "wpcd_onshell_T", "wpcd_phase_shifts"]
+           "wpcd_build_channels", "wpcd_diag_batched", "wpcd_onshell_T", "wpcd_phase_shifts", "wpcd_onshell_rows",
+           "wpcd_interp_phases", "wpcd_sigma_tot", "wpcd_mi_workspace_bytes", "wpcd_mi_solve",
+           "wpcd_probe_sink_elems", "wpcd_probe_fp64", "wpcd_jacobi_schedule", "wpcd_jacobi_critical_slot"]
 
 
 def _ptr(t):
     return None if t is None else t.data_ptr()
 
 
-def _stream(stream):
-    s = stream if stream is not None else torch.cuda.current_stream()
+def _stream(stream, device=None):
+    s = stream if stream is not None else torch.cuda.current_stream(device)
     return s.cuda_stream
 
 
@@ -108,6 +114,15 @@ class Handle:
 
     def num_sms(self):
         return _lib.wpcd_num_sms(self._h)
+
+    def probe_fp64(self, kind=1, iters=20000, stream=None, sink=None):
+        """wpcd_probe_fp64: launches the register-only fp64 chain kernel (kind 0 DFMA, 1 DMMA); returns the flops of the
+        launch.  The caller times it with CUDA events."""
+        if sink is None:
+            sink = torch.empty(_lib.wpcd_probe_sink_elems(self._h), dtype=torch.float64, device=self.device)
+        fl = _d(0.0)
+        self._check(_lib.wpcd_probe_fp64(self._h, kind, iters, _ptr(sink), C.byref(fl), _stream(stream, self.device)), "wpcd_probe_fp64")
+        return fl.value, sink
 
     def _work(self, nbytes):
         return torch.empty(max(int(nbytes), 16), dtype=torch.uint8, device=self.device)
@@ -151,7 +166,7 @@ class Handle:
             work = self._work(wb); out["work"] = work
         rc = _lib.wpcd_build_channels(self._h, C.byref(grid), C.byref(pot), ch, nch, _ptr(scales), S, P,
                                       _ptr(out["H_unc"]), _ptr(out["H_cpl"]), _ptr(out["e0"]), _ptr(out["dE"]),
-                                      _ptr(out["Eedge"]), _ptr(work), work.numel(), _stream(stream))
+                                      _ptr(out["Eedge"]), _ptr(work), work.numel(), _stream(stream, self.device))
         self._check(rc, "wpcd_build_channels")
         return out
 
@@ -182,7 +197,7 @@ class Handle:
         S_cpl = torch.empty((S, n_cpl, nE, 2, 2, 2), dtype=torch.float64, device=dev) if n_cpl else None
         work = self._work(_lib.wpcd_mi_workspace_bytes(self._h, int(NQ)))
         rc = _lib.wpcd_mi_solve(self._h, C.byref(pot), ch, nch, _ptr(scales), S, P, int(NQ), float(cmap), float(hbarc),
-                                float(mured), _ptr(Ecm), nE, _ptr(S_unc), _ptr(S_cpl), _ptr(work), work.numel(), _stream(stream))
+                                float(mured), _ptr(Ecm), nE, _ptr(S_unc), _ptr(S_cpl), _ptr(work), work.numel(), _stream(stream, self.device))
         self._check(rc, "wpcd_mi_solve")
         return S_unc, S_cpl
 
@@ -204,7 +219,7 @@ class Handle:
         nr = 0 if rows is None else len(rows)
         h_rows = (_i * (2 * nr))(*[int(x) for r in rows for x in r]) if nr else None
         rc = _lib.wpcd_diag_batched(self._h, n, batch, _ptr(A), _ptr(W), _ptr(Cm), _ptr(info), float(tol), int(max_sweeps),
-                                    h_rows, nr, _ptr(work), work.numel(), _stream(stream))
+                                    h_rows, nr, _ptr(work), work.numel(), _stream(stream, self.device))
         self._check(rc, "wpcd_diag_batched")
         return W, Cm, info
 
@@ -219,7 +234,7 @@ class Handle:
         if work is None or work.numel() < wb:
             work = self._work(wb)
         rc = _lib.wpcd_onshell_T(self._h, N, int(coupled), batch, _ptr(e0), _ptr(Eedge), _ptr(H), _ptr(W), _ptr(Cm),
-                                 _ptr(Ecm), nE, int(mode), _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream))
+                                 _ptr(Ecm), nE, int(mode), _ptr(T), _ptr(bins), _ptr(work), work.numel(), _stream(stream, self.device))
         self._check(rc, "wpcd_onshell_T")
         return T, bins
 
@@ -241,7 +256,7 @@ class Handle:
         shape = (batch, nq, 3) if coupled else (batch, nq)
         out = torch.empty(shape, dtype=torch.float64, device=dev) if out is None else out
         rc = _lib.wpcd_interp_phases(self._h, int(coupled), batch, N, _ptr(pedge), _ptr(delta_mid), _ptr(q), nq, _ptr(out),
-                                     _stream(stream))
+                                     _stream(stream, self.device))
         self._check(rc, "wpcd_interp_phases")
         return out
 
@@ -259,7 +274,7 @@ class Handle:
         out = torch.empty((S, nE), dtype=torch.float64, device=Ecm.device) if out is None else out
         ju = (_i * max(n_unc, 1))(*[int(j) for j in J_unc]); jc = (_i * max(n_cpl, 1))(*[int(j) for j in J_cpl])
         rc = _lib.wpcd_sigma_tot(self._h, S, nE, n_unc, ju, _ptr(T_unc), n_cpl, jc, _ptr(T_cpl), _ptr(bins), _ptr(dE),
-                                 _ptr(Ecm), float(hbarc), float(mu), _ptr(out), _stream(stream))
+                                 _ptr(Ecm), float(hbarc), float(mu), _ptr(out), _stream(stream, self.device))
         self._check(rc, "wpcd_sigma_tot")
         return out
 
@@ -271,6 +286,6 @@ class Handle:
         if want_S and S is None:
             S = torch.empty_like(T)
         rc = _lib.wpcd_phase_shifts(self._h, int(coupled), batch, nE, _ptr(T), _ptr(bins), _ptr(dE), _ptr(delta),
-                                    _ptr(S), _stream(stream))
+                                    _ptr(S), _stream(stream, self.device))
         self._check(rc, "wpcd_phase_shifts")
         return delta, S

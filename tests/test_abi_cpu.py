@@ -24,6 +24,16 @@ def test_library_exports_every_declared_symbol():
     assert {"wpcd_build_channels", "wpcd_diag_batched", "wpcd_onshell_T", "wpcd_phase_shifts"} <= set(names)
     for nm in names:
         assert hasattr(lib, nm), nm
+    # the binding's export list is the header's, and every definition has C linkage inside ONE extern "C" block
+    src = open(os.path.join(ROOT, "paper_2106_00454_b200", "wpcd.py")).read()
+    exports = re.search(r"EXPORTS = \[(.*?)\]", src, flags=re.S).group(1)
+    assert sorted(re.findall(r'"(wpcd_[A-Za-z_0-9]+)"', exports)) == names
+    api = open(os.path.join(ROOT, "paper_2106_00454_b200", "csrc", "api.cu")).read()
+    assert api.count('extern "C" {') == 1 and api.rstrip().endswith('}  // extern "C"')
+    # no undeclared debug exports in the product build
+    import subprocess
+    dyn = subprocess.run(["nm", "-D", "--defined-only", build.LIB], capture_output=True, text=True).stdout
+    assert sorted(set(re.findall(r"\bT (wpcd_[A-Za-z_0-9]+)", dyn))) == names
     lib.wpcd_strerror.restype = ctypes.c_char_p
     assert lib.wpcd_strerror(0) == b"ok" and lib.wpcd_strerror(-2) == b"unsupported size"
     # without a device the handle cannot be created and says so (no CPU fallback)
