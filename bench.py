@@ -23,10 +23,42 @@ sys.path.insert(0, ROOT)
 
 from paper_2106_00454_b200 import inputs as inp  # noqa: E402
 
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md)
-# DRAM traffic of one Jacobi launch at the bench workload (4096 matrices) from the committed ncu --set full capture
-# (profiles/r1_jacobi_ncu.md), keyed by n; algorithmic minimum = read H + write C + W = 16 n^2 + 8 n bytes per matrix.
-NCU_DRAM_BYTES = {100: 0.658889e9, 200: 3.122341e9}
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)
+# DRAM traffic per Jacobi launch comes from the committed ncu capture, keyed by (n, batch): profiles/jacobi_dram_traffic.csv
+# (command in profiles/jacobi_dram_traffic.md).  It is a static figure of that capture, reported only when (n, batch) match.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "jacobi_dram_traffic.csv")
+
+
+def ncu_traffic(n, batch):
+    """(bytes per launch or None, source/reason) from the committed profile table."""
+    try:
+        rows = [ln.strip().split(",") for ln in open(TRAFFIC_CSV) if ln.strip() and not ln.startswith("#")]
+    except OSError:
+        return None, "profiles/jacobi_dram_traffic.csv missing"
+    for r in rows[1:]:
+        if int(r[0]) == n and int(r[1]) == batch:
+            return float(r[2]), f"dram__bytes_read.sum + dram__bytes_write.sum of one launch, {r[3]} (static: from the committed capture, not this run)"
+    return None, f"no committed ncu capture for n={n}, batch={batch}"
+
+
+def measure_fp64_peak(h, torch):
+    """FP64 peak measured in this run with the library's register-only chain kernels (wpcd_probe_fp64): best of 3 launches
+    each of DFMA chains and DMMA (mma.sync.m8n8k4.f64) chains, CUDA events on the launching stream."""
+    out = {}
+    for kind, name in ((0, "dfma"), (1, "dmma")):
+        iters = 20000 if kind == 0 else 4000
+        best, sink = 0.0, None
+        for _ in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            flops, sink = h.probe_fp64(kind, iters, sink=sink)
+            e1.record()
+            torch.cuda.synchronize()
+            best = max(best, flops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        out[name] = best
+    return out
+
+
 METRIC = "channel-solves/s (fp64 H diag + on-shell T at all E)"
 CHANNELS = [(0, 0), (1, 1)]   # single 1S0 (n=N) and coupled 3S1-3D1 (n=2N)
 
@@ -117,7 +149,7 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     val = solves / dt
     sample = f"{n_each} samples x (1S0 + 3S1-3D1) per step, threads over solves; same inputs as the GPU arm"
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "channel-solves/s", "n_gpus": args.gpus,
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "channel-solves/s", "n_gpus": 1,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.N, args.samples, args.nE), "bounded_sample": sample},
@@ -166,11 +198,18 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     N, S, nE = args.N, args.samples, args.nE
+    if args.workload == "config3":          # BASELINE.json config 3: the Bayesian-sampling batch, all 14 channels J <= 4
+        N, S = 100, (1024 if args.samples == 4096 else args.samples)
+        channels = [(c, l) for _, c, l in inp.CHANNELS_J4]
+        wname = f"config3: {S} samples x 14 channels J<=4 (10 of {N}x{N}, 4 of {2 * N}x{2 * N}), {nE} energies"
+    else:
+        channels = CHANNELS
+        wname = workload_name(N, S, nE)
     tl, Ecm = inp.energies(nE)
     # every replica gets its own seeded batch (replicas only: the path does not shard)
     scales = inp.sample_scales(S, seed=rank)
     pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
-    pipe = Pipeline(inp.grid_edges(N), CHANNELS, Ecm, S, pot, device=local)
+    pipe = Pipeline(inp.grid_edges(N), channels, Ecm, S, pot, device=local)
     pipe.scales.copy_(torch.as_tensor(scales))
     names = pipe.stage_names()
 
@@ -237,8 +276,33 @@ def run_ours(args):
                        "rows_of_C_needed": rows_fraction(pipe, k2),
                        "tflops_algorithmic": f / (stage_ms[nm] * 1e-3) / 1e12,
                        "frac_fp64_peak": f / (stage_ms[nm] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
+        peak_meas = measure_fp64_peak(pipe.h, torch)
+        traffic, traffic_src = ncu_traffic(n, pipe.kind[kind]["batch"])
+        # secondary (HBM) rooflines: assembly stage and on-shell stage, algorithmic bytes over the stage's event time
+        hbm_peak = None
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        except Exception:
+            pass
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs" if hbm_peak else "fallback 6551.7 GB/s (this pool's measured copy bandwidth, B200_PROFILING.md)"
+        hbm_peak = hbm_peak or 6551.7
+        secondary = []
+        bytes_H = sum(8.0 * b["n"] ** 2 * b["batch"] for b in pipe.kind.values())
+        secondary.append({"bound": "hbm", "kernel": "assembly stage (k_grid + k_basis + k_combine): write H", "achieved": bytes_H / (stage_ms["build"] * 1e-3) / 1e9,
+                          "peak": hbm_peak, "unit": "GB/s", "frac": bytes_H / (stage_ms["build"] * 1e-3) / 1e9 / hbm_peak,
+                          "bytes_model": "8 n^2 per channel-solve (H written once)", "peak_source": hbm_src})
+        for k2, b in pipe.kind.items():
+            nm = "onshell_cpl" if k2 else "onshell_unc"
+            f2 = rows_fraction(pipe, k2) if b["n"] <= 200 else 1.0
+            by = (8.0 * b["n"] ** 2 * f2 + 8.0 * b["n"] + 16.0 * nE * (4 if k2 else 1) + 8.0 * nE * (3 if k2 else 1)) * b["batch"]
+            if b["n"] > 200:
+                by += 8.0 * b["n"] ** 2 * rows_fraction(pipe, k2) * b["batch"]       # the on-shell rows of H for V C
+            secondary.append({"bound": "hbm", "kernel": f"on-shell stage ({nm}: k_onshell + k_phase, n={b['n']})",
+                              "achieved": by / (stage_ms[nm] * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                              "frac": by / (stage_ms[nm] * 1e-3) / 1e9 / hbm_peak,
+                              "bytes_model": "rows of C the contraction reads + W + T and delta out", "peak_source": hbm_src})
         cpu = None
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and args.workload == "bench":
             cores = os.cpu_count() or 1
             n_each = 64 * max(cores, 8)          # about 10-20 s of CPU work on the box's cores
             k, dt = oracle_sample(N, nE, n_each, cores)
@@ -247,19 +311,21 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": "channel-solves/s", "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload_name(N, S, nE), "l2": "inputs_exceed_L2 (H batch >> 126 MB)",
+                "config": {"workload": wname, "l2": "inputs_exceed_L2 (H batch >> 126 MB)",
                            "replicas": world, "jacobi_tol": "2^-52 relative pivot test", "n_gl": 8},
                 "clocks": sampler.summary() if sampler else None,
                 "e2e": {"value": e2e, "unit": "channel-solves/s", "h2d_bytes_per_step": pipe.h2d_bytes(),
                         "d2h_bytes_per_step": pipe.d2h_bytes(), "ms_per_step": ms_e2e / args.steps},
                 "gpu_launches": pipe.launches_per_step * args.steps,
                 "roofline": {"bound": "alu", "kernel": f"k_jacobi ({dom}, n={n})", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
-                             "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(n),
-                             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_jacobi_ncu.md",
-                             "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DMMA microbenchmark measured 37.1)",
+                             "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_src,
+                             "algorithmic_bytes": (16.0 * n * n + 8.0 * n) * pipe.kind[kind]["batch"],
+                             "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md section 6); MEASURED_PEAKS.json has no fp64 entry",
+                             "peak_measured": peak_meas, "peak_measured_source": "wpcd_probe_fp64 in this run: register-only DFMA / DMMA chains on all SMs, best of 4, CUDA events",
+                             "frac_of_measured": ach / max(peak_meas.values()),
                              "flops_model": "(3 + 3 f) n^3 x rotating sweeps x batch: 3 n^3 for A (symmetric), 3 n^3 for the eigenvectors "
                                             "(SURVEY 8(d): 6 n^3), the latter scaled by the fraction f of rows of C that the on-shell step needs"},
-                "stages_ms": stage_ms, "jacobi": jac, "cpu_baseline": cpu}
+                "roofline_secondary": secondary, "stages_ms": stage_ms, "jacobi": jac, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -327,6 +393,83 @@ def run_table1(args):
                       "paper": {"hardware": "Tesla V100, one sample, pre-computed V", "ms": {"16": 0.5, "24": 2.5, "32": 6, "96": 35}}}))
 
 
+def run_config5_sweep(args):
+    """BASELINE.json config 5 in full: N in {32 ... 400} x 4096 seeded samples x {1S0 N x N, 3S1-3D1 2N x 2N}, 350 energies,
+    on the GPU (channel-solves/s, Jacobi fraction of the FP64 peak per launch), "plus the MI solver on the CPU oracle at
+    the same N for method-error and wall-time comparison" (SURVEY 8(d) "Oracle timing": N_Q = N, one sample, the same
+    energies; Eq. 37, 435-449 Table 1).  Prints ONE JSON object with all N."""
+    import torch
+    from concurrent.futures import ThreadPoolExecutor
+    from paper_2106_00454_b200.pipeline import Pipeline
+    from oracle import oracle as o
+    cores = os.cpu_count() or 1
+    nE, S = args.nE, args.samples
+    tl, Ecm = inp.energies(nE)
+    scales = inp.sample_scales(S, seed=0)
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    d180 = lambda a, b: np.abs((a - b + 90.0) % 180.0 - 90.0)
+    rows = {}
+    peak = None
+    for N in [int(x) for x in args.sweep_N.split(",")]:
+        pipe = Pipeline(inp.grid_edges(N), CHANNELS, Ecm, S, pot, device=0)
+        if peak is None:
+            peak = measure_fp64_peak(pipe.h, torch)
+        pipe.scales.copy_(torch.as_tensor(scales))
+        names = pipe.stage_names()
+        for _ in range(max(args.warmup, 3) if N <= 200 else 1):
+            pipe.solve_device()
+        torch.cuda.synchronize()
+        steps = args.steps if N <= 200 else max(1, min(args.steps, 2))
+        ev = [{nm: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for nm in names} for _ in range(steps)]
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for k in range(steps):
+            pipe.solve_device(events=ev[k])
+        t1.record()
+        torch.cuda.synchronize()
+        ms = t0.elapsed_time(t1) / steps
+        stage_ms = {nm: float(np.mean([e[nm][0].elapsed_time(e[nm][1]) for e in ev])) for nm in names}
+        info = {k: b["info"].cpu().numpy() for k, b in pipe.kind.items()}
+        assert all((v >= 1).all() for v in info.values()), "Jacobi did not converge"
+        jac = {}
+        for k2, b in pipe.kind.items():
+            nm = "diag_cpl" if k2 else "diag_unc"
+            f = jacobi_flops(b["n"], rows_fraction(pipe, k2)) * float(np.mean(info[k2] - 1)) * b["batch"]
+            jac[nm] = {"n": b["n"], "ms": stage_ms[nm], "rotating_sweeps": float(np.mean(info[k2] - 1)),
+                       "frac_fp64_peak": f / (stage_ms[nm] * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
+        d_unc = pipe.kind[0]["delta"][0].cpu().numpy()            # sample 0 (scales of seed 0, row 0)
+        d_cpl = pipe.kind[1]["delta"][0].cpu().numpy()
+        del pipe
+        torch.cuda.empty_cache()
+        # ---- MI on the CPU oracle: N_Q = N, sample 0, the same energies (a stride subsample above N = 200, stated)
+        n_mi = args.mi_energies or (nE if N <= 200 else 35)
+        idx = np.unique(np.linspace(0, nE - 1, n_mi).round().astype(int))
+        V0 = inp.MT_V0 * scales[0, :2]
+
+        def mi_one(e):
+            Su, _ = o.mi_solve(tl[e], V0=V0, mu=inp.MT_MU, l_or_J=0, NQ=N)
+            Sc, _ = o.mi_solve(tl[e], coupled=True, V0=V0, mu=inp.MT_MU, l_or_J=1, VT=inp.TENSOR_V * scales[0, 2], muT=inp.TENSOR_MU, NQ=N)
+            return Su, Sc
+        w0 = time.perf_counter()
+        with ThreadPoolExecutor(max_workers=cores) as ex:
+            res = list(ex.map(mi_one, idx))
+        mi_s = time.perf_counter() - w0
+        du = np.array([0.5 * np.degrees(np.angle(r[0])) for r in res])
+        dc = np.array([[0.5 * np.degrees(np.angle(r[1][0, 0])), 0.5 * np.degrees(np.angle(r[1][1, 1]))] for r in res])
+        eu = d180(d_unc[idx], du)
+        ec = d180(d_cpl[idx][:, :2], dc)
+        rows[str(N)] = {"ms_per_step": ms, "channel_solves_per_s": 2 * S / (ms * 1e-3), "stages_ms": stage_ms, "jacobi": jac,
+                        "mi_cpu_oracle": {"N_Q": N, "energies_solved": int(len(idx)), "wall_s": mi_s,
+                                          "wall_s_per_sample_350_energies": mi_s * nE / len(idx), "cores": cores,
+                                          "systems": "1S0 (N_Q+1 complex) + 3S1-3D1 (2 N_Q + 2 complex) per energy"},
+                        "wpcd_gpu_ms_per_sample_in_batch": ms / S,
+                        "method_error_deg": {"1S0_median": float(np.median(eu)), "1S0_max": float(eu.max()),
+                                             "3S1_3D1_delta_median": float(np.median(ec)), "3S1_3D1_delta_max": float(ec.max())}}
+    print(json.dumps({"workload": "config5_sweep: N x 4096 samples x {1S0, 3S1-3D1}, 350 energies; MI on the CPU oracle at N_Q = N",
+                      "metric": METRIC, "unit": "channel-solves/s", "samples": S, "energies": nE, "dtype": "f64",
+                      "fp64_peak": {"derived_tflops": FP64_PEAK_TFLOPS, "measured_tflops": peak}, "results": rows}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -337,10 +480,14 @@ def main():
     ap.add_argument("--N", type=int, default=100)
     ap.add_argument("--nE", type=int, default=350)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="bench", choices=["bench", "paper_table1"])
+    ap.add_argument("--workload", default="bench", choices=["bench", "config3", "config5_sweep", "paper_table1"])
+    ap.add_argument("--sweep-N", default="32,48,64,100,150,200,300,400", help="config5_sweep: the N values")
+    ap.add_argument("--mi-energies", type=int, default=0, help="config5_sweep: energies the CPU MI leg solves per N (0 = all for N <= 200, 35 above)")
     args = ap.parse_args()
     if args.workload == "paper_table1":
         return run_table1(args)
+    if args.workload == "config5_sweep":
+        return run_config5_sweep(args)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -66,6 +66,9 @@ class Pipeline:
         self.h_scales = torch.empty((self.S, n_scale_cols), dtype=f64).pin_memory()
         self.h_delta = {k: torch.empty(v["delta"].shape, dtype=f64).pin_memory() for k, v in self.kind.items()}
         self.h_info = {k: torch.empty(v["info"].shape, dtype=torch.int32).pin_memory() for k, v in self.kind.items()}
+        # the device->host copies of one kind's results run on a side stream while the next kind is diagonalised
+        self.copy_stream = torch.cuda.Stream(device=self.dev)
+        self.done = {k: torch.cuda.Event() for k in self.kind}
 
     @property
     def channel_solves(self):
@@ -76,9 +79,10 @@ class Pipeline:
         # k_grid, k_basis, k_combine per kind; k_schedule, k_jacobi, k_bins, k_onshell, k_phase per kind
         return 2 + len(self.kind) * 6 + (1 if self.J is not None else 0)
 
-    def solve_device(self, events=None):
+    def solve_device(self, events=None, to_host=False):
         """One pass of the whole hot path with inputs resident in HBM.  events: optional dict name -> (start, end)
-        torch.cuda.Event pairs recorded on the current stream around each stage."""
+        torch.cuda.Event pairs recorded on the current stream around each stage.  to_host: as soon as a kind's phase
+        shifts are complete they are copied to the pinned host buffers on the side stream (overlapping the next kind)."""
         def rec(name, which):
             if events is not None:
                 events[name][which].record()
@@ -98,6 +102,12 @@ class Pipeline:
                              T=b["T"], bins=b["bins"], work=b["owork"], mode=self.mode)
             self.h.phase_shifts(kind, b["T"], b["bins"], self.geo["dE"], want_S=False, delta=b["delta"])
             rec("onshell_" + tag, 1)
+            if to_host:
+                self.done[kind].record()
+                with torch.cuda.stream(self.copy_stream):
+                    self.copy_stream.wait_event(self.done[kind])
+                    self.h_delta[kind].copy_(b["delta"], non_blocking=True)
+                    self.h_info[kind].copy_(b["info"], non_blocking=True)
         if self.J is not None:
             any_kind = next(iter(self.kind.values()))
             self.h.sigma_tot(self.J[0], self.kind[0]["T"] if 0 in self.kind else None, self.J[1],
@@ -115,11 +125,9 @@ class Pipeline:
         """End-to-end user call: host scales [S][P] -> host phase shifts (pinned buffers), copies included."""
         self.h_scales.copy_(torch.as_tensor(scales_host))
         self.scales.copy_(self.h_scales, non_blocking=True)
-        self.solve_device()
-        for k, b in self.kind.items():
-            self.h_delta[k].copy_(b["delta"], non_blocking=True)
-            self.h_info[k].copy_(b["info"], non_blocking=True)
-        torch.cuda.current_stream().synchronize()
+        self.solve_device(to_host=True)
+        self.copy_stream.synchronize()
+        torch.cuda.current_stream(self.dev).synchronize()
         return self.h_delta, self.h_info
 
     def h2d_bytes(self):
