@@ -26,6 +26,7 @@
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
 #include <math.h>
 #include <type_traits>
+#include "jacobi_rotation.cuh"
 #include "jacobi_schedule.cuh"
 #include "wpcd_internal.cuh"
 
@@ -111,32 +112,6 @@ __device__ __forceinline__ int kPi(int x) {
   if (x == 1) return 2;
   if (x == 14) return 15;
   return (x & 1) ? x - 2 : x + 2;
-}
-
-// 1/sqrt(x) for normal x > 0 without the library routine's special-case branch: MUFU.RSQ64H seed (2^-22) and one
-// third-order correction y (1 + e/2 + 3e^2/8), e = 1 - x y^2, i.e. full double precision.  x = 0 gives inf.
-__device__ __forceinline__ double rsqrt_nr(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double e = fma(x, -(y * y), 1.0);
-  return fma(fma(e, 0.375, 0.5), y * e, y);
-}
-
-// Jacobi rotation annihilating a_pq (classical choice |angle| <= pi/4, "Jacobi method"), written with two
-// reciprocal square roots and no division:  with d = a_qq - a_pp, b = 2 a_pq, h = sqrt(d^2 + b^2):
-//   cos 2phi = |d|/h,  c = sqrt((1 + cos 2phi)/2),  s = sgn(d) (b/h)/(2c),  t = s/c.
-// Pivot test |a_pq| > tol sqrt(|a_pp a_qq|) (squared); below it the identity is returned.
-__device__ __forceinline__ bool rotation(double app, double aqq, double apq, double tol2, double& c, double& s, double& t) {
-  const bool doit = apq * apq > tol2 * fabs(app * aqq);
-  const double d = aqq - app, b = apq + apq;
-  const double rh = rsqrt_nr(fma(d, d, b * b));
-  const double c2 = fma(0.5 * fabs(d), rh, 0.5);
-  const double rc = rsqrt_nr(c2);
-  const double bh = copysign(0.5, d) * b * rh;
-  c = doit ? c2 * rc : 1.0;
-  s = doit ? bh * rc : 0.0;
-  t = doit ? bh * rc * rc : 0.0;
-  return doit;
 }
 
 // Cross-only tournament: the even positions (block I) stay, the odd ones (block J) move on by one pair, so that 8
@@ -802,6 +777,7 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
 }  // namespace
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
+  if (n <= WPCD_SMALL_N_MAX) return wpcd_jacobi_small_workspace();
   Geometry g = geometry(h, n);
   return g.tab_bytes + (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
@@ -809,6 +785,9 @@ size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                        double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
                        cudaStream_t st) {
+  // the paper's own size regime: element-wise parallel Jacobi, one small CTA per matrix (jacobi_small.cu)
+  if (n <= WPCD_SMALL_N_MAX)
+    return wpcd_jacobi_small_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, h_rows, n_ranges, d_work, work_bytes, st);
   Geometry g = geometry(h, n);
   if (g.smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   JacobiParams P;
