@@ -80,22 +80,51 @@ __device__ __forceinline__ bool cta_any(bool x) {
   return __syncthreads_or(x) != 0;
 }
 
-// Off-diagonal block number t (0 <= t < P(P-1)/2), enumerated along the super-diagonals d = b - a = 1, 2, ...: (a, a + d).
-__device__ __forceinline__ void unrank_block(int P, int t, int& a, int& b) {
-  int d = 1;
-  while (t >= P - d) { t -= P - d; ++d; }
-  a = t; b = t + d;
+// Deal of the off-diagonal blocks (a < b) of a round to the threads.  The first element of block (a, b) sits (16-byte
+// units modulo 8, row stride NP + 2) at bank group (2a + b + const) mod 8 =: its class.  Thread tid only takes blocks of
+// class tid & 7, so that the eight threads of a quarter warp (128-bit accesses of the even rounds) always hit eight
+// different bank groups; in the odd rounds (64-bit accesses, 16 threads per wavefront) the upper eight threads of a half
+// warp start with the block's second column, which moves them to the other eight 8-byte banks.  Within a class the
+// blocks go round-robin to the T/8 threads of that class; slots needed: ceil(largest class / (T/8)).
+__host__ __device__ constexpr int class_slots(int pairs, int threads) {
+  int cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int a = 0; a < pairs; ++a)
+    for (int b = a + 1; b < pairs; ++b) ++cnt[(2 * a + b) & 7];
+  int mx = 0;
+  for (int c = 0; c < 8; ++c) mx = cnt[c] > mx ? cnt[c] : mx;
+  const int ranks = threads / 8;
+  return (mx + ranks - 1) / ranks;
+}
+
+// blocks of thread tid: out[k] = first-element offset | a << 16 | b << 24, 0xFFFFFFFF = none; odd: pairs (2j+1, 2j+2)
+template <int K>
+__device__ __forceinline__ void deal_blocks(int pairs, int threads, int tid, int LD, int odd, unsigned (&out)[K]) {
+  const int cls = tid & 7, rank = tid >> 3, ranks = threads >> 3;
+#pragma unroll
+  for (int k = 0; k < K; ++k) out[k] = 0xFFFFFFFFu;
+  int i = 0;
+  for (int a = 0; a < pairs; ++a)
+    for (int b = a + 1; b < pairs; ++b) {
+      if (((2 * a + b) & 7) != cls) continue;
+      if (i % ranks == rank) {
+        const int slot = i / ranks;
+        const unsigned w = (unsigned)((2 * a + odd) * LD + 2 * b + odd) | (a << 16) | (b << 24);
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+          if (k == slot) out[k] = w;
+      }
+      ++i;
+    }
 }
 
 // NP: padded size (16, 32, 48, 64); one thread per row.
 template <int NP>
-__global__ void __launch_bounds__(NP <= 32 ? 32 : 64) k_jacobi_small(SmallParams prm) {
+__global__ void __launch_bounds__(NP <= 32 ? 32 : 64, NP == 32 ? 12 : 1) k_jacobi_small(SmallParams prm) {
   constexpr int T = NP <= 32 ? 32 : 64;       // threads of the CTA (rows >= NP idle in the V phase, work in the A phase)
   constexpr int P = NP / 2;                   // pairs of an even round
   constexpr int LD = NP + 2;                  // row stride of A (doubles): rows are 16 bytes apart modulo 128
-  constexpr int NB0 = P * (P - 1) / 2;        // off-diagonal blocks, even rounds
-  constexpr int NB1 = (P - 1) * (P - 2) / 2;  // odd rounds: P - 1 real pairs (the blocks of the end pair are handled apart)
-  constexpr int K0 = (NB0 + T - 1) / T, K1 = (NB1 + T - 1) / T;
+  // off-diagonal blocks: P (P - 1) / 2 in even rounds; odd rounds have P - 1 real pairs (the end pair is handled apart)
+  constexpr int K0 = class_slots(P, T), K1 = class_slots(P - 1, T);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* A = reinterpret_cast<double*>(smem_raw);       // [NP][LD], upper triangle
   double* cs = A + NP * LD;                              // [P] (c, s)
@@ -111,20 +140,12 @@ __global__ void __launch_bounds__(NP <= 32 ? 32 : 64) k_jacobi_small(SmallParams
   // static work lists: blocks of the even and odd rounds as byte offsets of the block's first element and of the two
   // (c, s) entries: off | a << 16 | b << 24
   unsigned blk0[K0], blk1[K1];
-#pragma unroll
-  for (int k = 0; k < K0; ++k) {
-    const int t = tid + k * T;
-    int a = 0, b = 0;
-    if (t < NB0) unrank_block(P, t, a, b);
-    blk0[k] = t < NB0 ? (unsigned)((2 * a) * LD + 2 * b) | (a << 16) | (b << 24) : 0xFFFFFFFFu;
-  }
-#pragma unroll
-  for (int k = 0; k < K1; ++k) {
-    const int t = tid + k * T;
-    int a = 0, b = 0;
-    if (t < NB1) unrank_block(P - 1, t, a, b);
-    blk1[k] = t < NB1 ? (unsigned)((2 * a + 1) * LD + 2 * b + 1) | (a << 16) | (b << 24) : 0xFFFFFFFFu;
-  }
+  deal_blocks<K0>(P, T, tid, LD, 0, blk0);
+  deal_blocks<K1>(P - 1, T, tid, LD, 1, blk1);
+  // odd rounds: the upper eight threads of every half warp work on the column-swapped block (see deal_blocks):
+  // [x1 x0] R(c, s) = [y1 y0] with R(c, -s)
+  const int swp = (tid >> 3) & 1;
+  const double sgn = swp ? -1.0 : 1.0;
 
   // bulk copies need 16-byte sizes and addresses: n even; odd n (never a config size) reads H with plain loads
   const bool bulk = (n & 1) == 0;
@@ -234,11 +255,14 @@ __global__ void __launch_bounds__(NP <= 32 ? 32 : 64) k_jacobi_small(SmallParams
                 double* x = A + (w & 0xFFFFu);
                 const double2 ga = *reinterpret_cast<const double2*>(cs + 2 * ((w >> 16) & 0xFFu));
                 const double2 gb = *reinterpret_cast<const double2*>(cs + 2 * (w >> 24));
-                const double x00 = x[0], x01 = x[1], x10 = x[LD], x11 = x[LD + 1];
-                const double y00 = gb.y * x00 + gb.x * x01, y01 = gb.x * x00 - gb.y * x01;
-                const double y10 = gb.y * x10 + gb.x * x11, y11 = gb.x * x10 - gb.y * x11;
-                x[0] = ga.y * y00 + ga.x * y10; x[1] = ga.y * y01 + ga.x * y11;
-                x[LD] = ga.x * y00 - ga.y * y10; x[LD + 1] = ga.x * y01 - ga.y * y11;
+                double* xa = x + swp;        // first-loaded column of the block (the second one for the swapped threads)
+                double* xb = x + 1 - swp;
+                const double sb = sgn * gb.y;
+                const double x00 = xa[0], x01 = xb[0], x10 = xa[LD], x11 = xb[LD];
+                const double y00 = sb * x00 + gb.x * x01, y01 = gb.x * x00 - sb * x01;
+                const double y10 = sb * x10 + gb.x * x11, y11 = gb.x * x10 - sb * x11;
+                xa[0] = ga.y * y00 + ga.x * y10; xb[0] = ga.y * y01 + ga.x * y11;
+                xa[LD] = ga.x * y00 - ga.y * y10; xb[LD] = ga.x * y01 - ga.y * y11;
               }
             }
             // the idle ends: row 0 gets the column rotations, column NP-1 the row rotations of the P-1 real pairs; the

@@ -23,7 +23,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
                        double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
                        cudaStream_t st);
 // jacobi_small.cu (n <= WPCD_SMALL_N_MAX)
-#define WPCD_SMALL_N_MAX 64
+#define WPCD_SMALL_N_MAX 32
 size_t wpcd_jacobi_small_workspace();
 int wpcd_jacobi_small_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                              double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
