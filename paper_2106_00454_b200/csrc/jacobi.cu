@@ -501,7 +501,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
     __syncwarp();
     // full sweep of the pivot every full_every-th step (every block then sits in a pivot at >= 1 full step per sweep,
     // so every pair is still met in every sweep); always for small matrices, where padding leaves few real pivots
-    const bool full = (tn % P.full_every) == 0 || P.nb < 8;
+    const bool full = (tn % P.full_every) == 0 || P.nb < 6;  // nb >= 6: every block sits in >= 1 full real pivot per sweep
     rotated = inner_solve(A, Qn, I, J, P.tol, full, lane);
   }
   if (lane == 0) {

@@ -117,9 +117,9 @@ __device__ __forceinline__ void deal_blocks(int pairs, int threads, int tid, int
     }
 }
 
-// NP: padded size (16, 32, 48, 64); one thread per row.
+// NP: padded size (16, 24, 32; 48 and 64 compile too but the block kernel of jacobi.cu is faster there); one thread per row.
 template <int NP>
-__global__ void __launch_bounds__(NP <= 32 ? 32 : 64, NP == 32 ? 12 : 1) k_jacobi_small(SmallParams prm) {
+__global__ void __launch_bounds__(NP <= 32 ? 32 : 64, NP <= 16 ? 16 : (NP <= 32 ? 12 : 1)) k_jacobi_small(SmallParams prm) {
   constexpr int T = NP <= 32 ? 32 : 64;       // threads of the CTA (rows >= NP idle in the V phase, work in the A phase)
   constexpr int P = NP / 2;                   // pairs of an even round
   constexpr int LD = NP + 2;                  // row stride of A (doubles): rows are 16 bytes apart modulo 128
@@ -215,8 +215,10 @@ __global__ void __launch_bounds__(NP <= 32 ? 32 : 64, NP == 32 ? 12 : 1) k_jacob
               A[q * LD + q] = app - t * apq;
               if (doit) A[p * LD + q] = 0.0;
               *reinterpret_cast<double2*>(cs + 2 * tid) = make_double2(c, s);
-              const int rp = real[p], rq = real[q];
-              real[p] = rq; real[q] = rp;
+              if (n < NP) {  // padding travels with the positions
+                const int rp = real[p], rq = real[q];
+                real[p] = rq; real[q] = rp;
+              }
             }
           }
           cta_sync<T>();
@@ -367,7 +369,6 @@ int wpcd_jacobi_small_launch(WpcdHandle* h, int n, int batch, const double* d_A,
   prm.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   // CTAs per SM: bounded by registers (one row of V per thread) and by the 32-CTA limit
   if (n <= 16) return launch_small<16>(h, prm, 16, st);
-  if (n <= 32) return launch_small<32>(h, prm, 12, st);
-  if (n <= 48) return launch_small<48>(h, prm, 4, st);
-  return launch_small<64>(h, prm, 4, st);
+  if (n <= 24) return launch_small<24>(h, prm, 12, st);
+  return launch_small<32>(h, prm, 12, st);
 }
