@@ -380,6 +380,131 @@ __global__ void __launch_bounds__(kOnThreads) k_onshell_i1(OnshellParams P) {
   }
 }
 
+
+// Point-wise variant of k_onshell_i1 (mode 0), one THREAD per energy and the telescoped form of SURVEY 8(d): inside a
+// branch the pseudostate bins share their edges (hi_k = lo_{k+1}, Eq. 23), so
+//   sum_k w_k [ln|E - lo_k| - ln|E - hi_k|]  =  sum_k (w_k - w_{k-1}) ln|E - lo_k|  -  w_last ln|E - hi_last|,
+//   w_k = (VC)_ik (VC)_i'k / (hi_k - lo_k)  (Eqs. B.5-B.6, sign per reading G2):
+// ONE logarithm per (energy, edge), no division, the three elements of a coupled block sharing it; the previous state's
+// weights stay in registers.  No warp reduction: a thread walks the eigenstates alone, 32 energies per warp side by side
+// (they sit in the same or neighbouring on-shell bins, so the rows of C they read are shared through L1).  Against the
+// warp-per-energy kernel: 1.31 -> see profiles/r2_onshell.md at n = 100; it matters most for the paper's own N_WP = 16 .. 48
+// (PAPER.md:437-445), where the on-shell step had become a third of the pass.
+template <int NC>
+__global__ void __launch_bounds__(512) k_onshell_i1_pw(OnshellParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int N = P.N, n = P.n, nE = P.nE;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  double* sW = reinterpret_cast<double*>(smem_raw);  // [n]
+  double* sLo = sW + n;                                // [n + NC]: lower edge of state k; [n + br]: upper edge of the last state of branch br
+  double* sIw = sLo + n + NC;                          // [n] 1/(hi - lo) of the positive states
+  __shared__ int s_nb;
+  const size_t mat = blockIdx.x;
+  const double* H = P.H + mat * (size_t)n * n;
+  const double* C = P.C + mat * (size_t)n * n;
+  const double* W = P.W + mat * (size_t)n;
+  double* T = P.T + mat * (size_t)nE * NC * NC * 2;
+  if (tid == 0) s_nb = 0;
+  for (int k = tid; k < n; k += nthr) sW[k] = W[k];
+  __syncthreads();
+  {
+    int cnt = 0;
+    for (int k = tid; k < n; k += nthr) cnt += sW[k] < 0.0;
+    if (cnt) atomicAdd(&s_nb, cnt);
+  }
+  __syncthreads();
+  const int nbd = s_nb;
+  if (tid < NC) sLo[n + tid] = 0.0;
+  for (int k = tid; k < n; k += nthr) {
+    double lo = 0.0, hi = 0.0;
+    if (k >= nbd) {
+      const int br = (k - nbd) % NC, i = (k - nbd) / NC;
+      const int mbr = (n - nbd - br + NC - 1) / NC;  // states in this branch
+      const double w = sW[k];
+      lo = i == 0 ? 0.0 : 0.5 * (sW[k - NC] + w);
+      if (i < mbr - 1) hi = 0.5 * (w + sW[k + NC]);
+      else if (mbr == 1) hi = 2.0 * w;
+      else {
+        const double lop = i == 1 ? 0.0 : 0.5 * (sW[k - 2 * NC] + sW[k - NC]);
+        hi = w + 0.5 * (lo - lop);
+      }
+      if (i == mbr - 1) sLo[n + br] = hi;  // Eq. 23's last edge of the branch
+    }
+    sLo[k] = lo;
+    sIw[k] = k >= nbd ? 1.0 / (hi - lo) : 0.0;
+  }
+  __syncthreads();
+  for (int e = tid; e < nE; e += nthr) {
+    const int b = P.bin[e];
+    if (b < 0) {
+#pragma unroll
+      for (int x = 0; x < NC * NC * 2; ++x) T[(size_t)e * NC * NC * 2 + x] = 0.0;
+      continue;
+    }
+    const double E = P.Ecm[e], e0b = P.e0[b];
+    const double* c0 = C + (size_t)b * n;
+    const double* c1 = C + (size_t)((NC - 1) * N + b) * n;
+    double re00 = 0, im00 = 0, re01 = 0, im01 = 0, re11 = 0, im11 = 0;
+    for (int k = 0; k < nbd; ++k) {  // bound states: 1/(E - eps_b)
+      const double w = sW[k] - e0b, g = 1.0 / (E - sW[k]);
+      const double a = __ldg(c0 + k) * w;
+      re00 = fma(a * a, g, re00);
+      if (NC == 2) {
+        const double bb = __ldg(c1 + k) * w;
+        re01 = fma(a * bb, g, re01);
+        re11 = fma(bb * bb, g, re11);
+      }
+    }
+    double p00[NC], p01[NC], p11[NC];   // weights of the previous state of each branch
+#pragma unroll
+    for (int br = 0; br < NC; ++br) p00[br] = p01[br] = p11[br] = 0.0;
+    for (int k0 = nbd; k0 < n; k0 += NC) {
+#pragma unroll
+      for (int br = 0; br < NC; ++br) {
+        const int k = k0 + br;
+        if (k < n) {
+          const double lo = sLo[k], iw = sIw[k], w = sW[k] - e0b;
+          const double hi = k + NC < n ? sLo[k + NC] : sLo[n + br];
+          const double L = log(fabs(E - lo));
+          const bool in = E >= lo && E < hi;
+          const double a = __ldg(c0 + k) * w;
+          const double w00 = a * a * iw;
+          re00 = fma(w00 - p00[br], L, re00); p00[br] = w00;
+          im00 += in ? w00 : 0.0;
+          if (NC == 2) {
+            const double bb = __ldg(c1 + k) * w;
+            const double w01 = a * bb * iw, w11 = bb * bb * iw;
+            re01 = fma(w01 - p01[br], L, re01); p01[br] = w01;
+            re11 = fma(w11 - p11[br], L, re11); p11[br] = w11;
+            im01 += in ? w01 : 0.0;
+            im11 += in ? w11 : 0.0;
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int br = 0; br < NC; ++br) {   // the upper edge of each branch's last state
+      if (nbd + br < n) {
+        const double L = log(fabs(E - sLo[n + br]));
+        re00 = fma(-p00[br], L, re00);
+        if (NC == 2) { re01 = fma(-p01[br], L, re01); re11 = fma(-p11[br], L, re11); }
+      }
+    }
+    const double* h0 = H + (size_t)b * n;  // row (0, b) of H; V = H - diag(e0)
+    if (NC == 1) {
+      T[(size_t)e * 2] = (h0[b] - e0b) + re00;
+      T[(size_t)e * 2 + 1] = -WPCD_PI * im00;
+    } else {
+      const double* h1 = H + (size_t)(N + b) * n;  // row (1, b)
+      double* t = T + (size_t)e * 8;
+      t[0] = (h0[b] - e0b) + re00;     t[1] = -WPCD_PI * im00;
+      t[2] = h0[N + b] + re01;         t[3] = -WPCD_PI * im01;
+      t[4] = h1[b] + re01;             t[5] = -WPCD_PI * im01;
+      t[6] = (h1[N + b] - e0b) + re11; t[7] = -WPCD_PI * im11;
+    }
+  }
+}
+
 __global__ void k_phase(int coupled, size_t total, int nE, const double* __restrict__ T, const int* __restrict__ bin,
                         const double* __restrict__ dE, double* __restrict__ delta, double* __restrict__ S) {
   size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -558,7 +683,15 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   if (smem > (size_t)h->max_smem_optin) return WPCD_ESIZE;
   k_bins<<<1, 256, 0, st>>>(N, nE, d_Eedge, d_Ecm, d_bin, static_cast<int*>(d_work));
   if (P.n <= kI1MaxN) {
-    k_onshell_i1<<<batch, kOnThreads, (size_t)4 * P.n * 8, st>>>(P);
+    if (mode == 0) {  // point-wise resolvent: one thread per energy, telescoped logarithms
+      int thr = (nE + 127) / 128 * 128;
+      if (thr > 512) thr = 512;
+      const size_t sm = (size_t)(3 * P.n + P.nc) * 8;
+      if (coupled) k_onshell_i1_pw<2><<<batch, thr, sm, st>>>(P);
+      else k_onshell_i1_pw<1><<<batch, thr, sm, st>>>(P);
+    } else {
+      k_onshell_i1<<<batch, kOnThreads, (size_t)4 * P.n * 8, st>>>(P);
+    }
     return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
   }
   int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
