@@ -115,6 +115,7 @@ def _compare_channel(res, kind, s, c, N, lJ, Ecm, scale=(1.0, 1.0, 1.0), yamaguc
         ARBITRATED.append((label, "phase", N, n, edges is not None))
         assert _arbitration_allowed(N, n, edges is not None), (label, "phase arbitration outside DESIGN.md's list", dphi, dS)
         assert dphi_o > dphi or dS_o > dS, (label, "arbitration: the fp64 oracle must be the less accurate side")
+    print("PARITY", label, "n", n, "eig", errW, "phase", dphi, "S", dS)
     assert dphi <= hp.TOL_PHASE_DEG, (label, "phase", dphi)
     assert dS <= hp.TOL_S_ABS, (label, "S", dS)
     return errH, errW, dphi, dS
