@@ -142,6 +142,7 @@ struct OnshellParams {
   double* T;
   int N, n, nc, nE, R;  // R = bins per chunk
   int ldv, gemm;        // k_onshell: row stride of the V rows in shared memory; 1 = tensor-core product
+  int nsplit;           // k_onshell: CTAs that share one matrix (they take the chunks of on-shell rows in turn)
   int mode;             // 0 point-wise resolvent (B.5-B.6), 1 energy-averaged (Eq. 28, B.7-B.8)
 };
 
@@ -156,7 +157,11 @@ __global__ void __launch_bounds__(kOnGemmThreads) k_onshell(OnshellParams P) {
   double* sV = sHi + n;                                // [max(R*nc, 8)][ldv]
   double* sVC = sV + (size_t)vrows * ldv;              // [R*nc][n]
   __shared__ int s_nb;
-  const size_t mat = blockIdx.x;
+  // nsplit consecutive CTAs work on the same matrix and take its chunks in turn: every chunk is a pass over all of C,
+  // and with one matrix per SM the 148 C's in flight (n = 300: 106 MB) fall out of L2 between the passes (round 1: C read
+  // ~12 times from DRAM); sharing a matrix between CTAs that run at the same time keeps the set of live C's inside L2.
+  const size_t mat = blockIdx.x / P.nsplit;
+  const int part = blockIdx.x % P.nsplit;
   const double* H = P.H + mat * (size_t)n * n;
   const double* C = P.C + mat * (size_t)n * n;
   const double* W = P.W + mat * (size_t)n;
@@ -189,11 +194,11 @@ __global__ void __launch_bounds__(kOnGemmThreads) k_onshell(OnshellParams P) {
     sLo[k] = lo; sHi[k] = hi;
   }
   // energies outside the grid: T = 0
-  for (int e = tid; e < nE; e += kOnGemmThreads)
+  for (int e = tid; e < nE && part == 0; e += kOnGemmThreads)
     if (P.bin[e] < 0 || (P.mode == 1 && nbd + nc * P.bin[e] + nc - 1 >= n))
       for (int x = 0; x < nc * nc * 2; ++x) T[(size_t)e * nc * nc * 2 + x] = 0.0;
   const int bmin = P.range[0], bmax = P.range[1];
-  for (int b0 = bmin; b0 <= bmax; b0 += R) {
+  for (int b0 = bmin + part * R; b0 <= bmax; b0 += R * P.nsplit) {
     const int nbins = min(R, bmax - b0 + 1), nrows = nbins * nc;
     __syncthreads();
     // V rows of this chunk: chunk row rr = (b - b0)*nc + alpha  <->  matrix row alpha*N + b
@@ -666,7 +671,7 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
                         int mode, double* d_T, int* d_bin, void* d_work, size_t, cudaStream_t st) {
   OnshellParams P;
   P.e0 = d_e0; P.H = d_H; P.W = d_W; P.C = d_C; P.Ecm = d_Ecm; P.bin = d_bin; P.range = static_cast<int*>(d_work);
-  P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE; P.mode = mode;
+  P.T = d_T; P.N = N; P.nc = coupled ? 2 : 1; P.n = P.nc * N; P.nE = nE; P.mode = mode; P.nsplit = 1;
   // chunk of 32 (else 16, else 8) rows of VC per pass over C on the tensor-core path; beyond that (n > ~1500) the plain loop
   // with as many bins per chunk as fit
   const size_t cap = (size_t)h->max_smem_optin - 1024;
@@ -696,7 +701,16 @@ int wpcd_onshell_launch(WpcdHandle* h, int N, int coupled, int batch, const doub
   }
   int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_onshell, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "onshell attr");
   if (rc) return rc;
-  k_onshell<<<batch, kOnGemmThreads, smem, st>>>(P);
+  {  // CTAs per matrix so that the C's of the matrices in flight (one CTA per SM) stay within ~40 MB of L2
+    const double live = (double)h->num_sms * P.n * P.n * 8.0;
+    int ns = (int)(live / (40.0 * 1048576.0)) + 1;
+    const int nchunks_max = (N + P.R - 1) / P.R;
+    if (ns > nchunks_max) ns = nchunks_max;
+    if (ns > 16) ns = 16;
+    if (ns < 1 || (size_t)batch * ns > 0x7fffffffu) ns = 1;
+    P.nsplit = ns;
+  }
+  k_onshell<<<batch * P.nsplit, kOnGemmThreads, smem, st>>>(P);
   return wpcd_check_cuda(h, cudaGetLastError(), "onshell_T launch");
 }
 
