@@ -442,7 +442,7 @@ def run_config5_sweep(args):
         del pipe
         torch.cuda.empty_cache()
         # ---- MI on the CPU oracle: N_Q = N, sample 0, the same energies (a stride subsample above N = 200, stated)
-        n_mi = args.mi_energies or (nE if N <= 200 else 35)
+        n_mi = args.mi_energies or nE
         idx = np.unique(np.linspace(0, nE - 1, n_mi).round().astype(int))
         V0 = inp.MT_V0 * scales[0, :2]
 
@@ -482,7 +482,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="bench", choices=["bench", "config3", "config5_sweep", "paper_table1"])
     ap.add_argument("--sweep-N", default="32,48,64,100,150,200,300,400", help="config5_sweep: the N values")
-    ap.add_argument("--mi-energies", type=int, default=0, help="config5_sweep: energies the CPU MI leg solves per N (0 = all for N <= 200, 35 above)")
+    ap.add_argument("--mi-energies", type=int, default=0, help="config5_sweep: energies the CPU MI leg solves per N (0 = all)")
     args = ap.parse_args()
     if args.workload == "paper_table1":
         return run_table1(args)

@@ -34,7 +34,8 @@ namespace {
 
 // Optional cycle counters (only in profiling builds, -DWPCD_PROFILE), accumulated by CTA 0:
 //   [0] whole steps (thread 0), [1] critical tile + pivot solve of warp 1, [2] number of steps,
-//   [3] queue part of warp 15, [4] queue part of warp 1
+//   [3] queue part of warp 15, [4] queue part of warp 1, [5] whole matrices (load, ordering, sweeps, write-back; thread 0),
+//   [6] load + ordering + V = 1 part, [7] sort + write-back part
 #ifdef WPCD_PROFILE
 __device__ long long wpcd_prof[8];
 #define WPCD_PROF_ADD(k, v) atomicAdd((unsigned long long*)&wpcd_prof[k], (unsigned long long)(v))
@@ -567,6 +568,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
   for (int mat = blockIdx.x; mat < P.batch;) {
     const double* H = P.H + (size_t)mat * n * n;
     __syncthreads();
+#ifdef WPCD_PROFILE
+    const long long tm0 = clock64();
+#endif
     // Ordering (de Rijk): the rows/columns are taken in the order of DESCENDING diagonal entries.  On these graded
     // Hamiltonians (kinetic energies from 1e-3 to 1e5 MeV along the diagonal) the cyclic sweeps then converge in one to
     // two sweeps fewer than in the natural ascending order (oracle: 7 -> 5-6 sweeps at N = 100).  Pure relabelling:
@@ -614,6 +618,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     }
     if (tid < 4) sm.ctr[tid] = 0;
     __syncthreads();
+#ifdef WPCD_PROFILE
+    if (blockIdx.x == 0 && tid == 0) WPCD_PROF_ADD(6, clock64() - tm0);
+#endif
     // prologue: pivots of (sweep 0, step 0) into Q buffer 0
     if (widx >= 0)
       for (int sn = widx; sn < nslots; sn += kPivotWarps) prepare_slot<kMode>(sm, P, 0, sn, 0, false, 0, 0, 0, lane, widx);
@@ -694,6 +701,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     }
     // eigenvalues = diagonal; rank sort ascending (ties by index); gather columns
     __syncthreads();
+#ifdef WPCD_PROFILE
+    const long long tm1 = clock64();
+#endif
     for (int k = tid; k < n; k += kThreads) sm.wsort[k] = Av.get(k, k);
     __syncthreads();
     for (int k = tid; k < n; k += kThreads) {
@@ -720,6 +730,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
       s_next = atomicAdd(P.next, 1);
     }
     __syncthreads();
+#ifdef WPCD_PROFILE
+    if (blockIdx.x == 0 && tid == 0) { WPCD_PROF_ADD(5, clock64() - tm0); WPCD_PROF_ADD(7, clock64() - tm1); }
+#endif
     mat = s_next;
   }
 }
