@@ -5,8 +5,8 @@
 //   on-shell momentum p = sqrt(E_cm/cE)                                                    (Eq. 4)
 //   D_j = (2/pi) w_j k_j^2 f/(p^2-k_j^2),  D_{NQ+1} = -(2/pi) f p^2 sum_j w_j/(p^2-k_j^2) - i f p,  f = 2 mu/hbarc^2
 //   (derived from Eqs. 2-4, reading C3: the printed Eq. 5 is inconsistent)
-//   F = 1 - V diag(D) (Eq. 7), F T = V (Eq. 6) by complex Gauss elimination with partial pivoting in shared memory,
-//   S = 1 - 2 i f p T_onshell (convention A, reading C2).
+//   F = 1 - V diag(D) (Eq. 7), F T = V (Eq. 6), solved as the real K-matrix system plus the on-shell rank-nc correction
+//   (Eq. 38; see k_mi_solve), S = 1 - 2 i f p T_onshell (convention A, reading C2).
 // Potential in convention A: v_l(k',k) = sum_t V0_t Q_l(z_t)/(2k'k); coupled channels: blocks l = J-1, J+1 and the
 // off-diagonal Yukawa V_T Q_J(z_T)/(2k'k) (reading C8); Yamaguchi -lambda_A g(k')g(k).
 #include <math.h>
@@ -92,18 +92,28 @@ __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
   return make_double2((a.x * b.x + a.y * b.y) / d, (a.y * b.x - a.x * b.y) / d);
 }
 
-// grid (nE, nch, S); dynamic shared memory: F [n][ld] complex (ld = n + nc: the right-hand sides ride along), q [M],
-// D [M] complex.
+// grid (nE, nch, S); dynamic shared memory: F [n][ld] (ld = n + nc: the right-hand sides ride along), q [M], D [M], row flags.
+//
+// K-matrix form ("it is numerically more stable to first introduce the K-matrix as the principal value part of the
+// LS equation ... a set of purely real matrix-equations", Eq. 38: a quarter of the complex flops).  The only
+// complex entry of D is the on-shell one, D_{NQ+1} = D_r - i f p (reading C3), so F = F_r + i f p u e^T with F_r = 1 - V diag(D_r)
+// real and u the on-shell column(s) of V: solve F_r K = u in real arithmetic (Gauss elimination with partial pivoting, the
+// pivoting implicit through row flags: no row swaps, two barriers per column), then T_on = K_on (1 + i f p K_on)^-1
+// (Sherman-Morrison for the rank-nc term) and S = 1 - 2 i f p T_on.  Same S as the complex elimination of Eqs. 6-7, which the
+// oracle performs, up to rounding.  The unknowns are ordered grid points first (block by block), on-shell points last, so that
+// K_on falls out of the last nc pivots without a back substitution over the grid.
 __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int tid = threadIdx.x;
-  const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = n + nc;
-  double2* F = reinterpret_cast<double2*>(smem_raw);
-  double* q = reinterpret_cast<double*>(F + (size_t)n * ld);
-  double2* D = reinterpret_cast<double2*>(q + M + (M & 1));
-  __shared__ double s_red[kMiThreads];
-  __shared__ int s_idx[kMiThreads];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kMiThreads / 32;
+  const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = n + nc, ng = nc * NQ;
+  double* F = reinterpret_cast<double*>(smem_raw);       // [n][ld]
+  double* q = F + (size_t)n * ld;                         // [M]
+  double* D = q + M;                                      // [M] real parts (principal value)
+  int* prow = reinterpret_cast<int*>(D + M);              // [n] pivot row of column c
+  int* lst = prow + n;                                    // [2][n] rows not yet used as a pivot (double buffered)
   __shared__ double sV0[WPCD_MAX_TERMS], sVT;
+  __shared__ double cval[2 * (kMiThreads / 32)];         // pivot candidates per warp (double buffered)
+  __shared__ int cpos[2 * (kMiThreads / 32)];
   const int e = blockIdx.x, ch = blockIdx.y;
   const size_t smp = blockIdx.z;
   const double cE = P.hbarc * P.hbarc / (2.0 * P.mured), f = 2.0 * P.mured / (P.hbarc * P.hbarc);
@@ -123,19 +133,21 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   for (int j = tid; j < NQ; j += kMiThreads) {
     const double k = P.kq[j];
     q[j] = k;
-    D[j] = make_double2((2.0 / WPCD_PI) * P.wq[j] * k * k * f / (p * p - k * k), 0.0);
+    D[j] = (2.0 / WPCD_PI) * P.wq[j] * k * k * f / (p * p - k * k);
   }
   __syncthreads();
   if (tid == 0) {
     double ssum = 0.0;
     for (int j = 0; j < NQ; ++j) ssum += P.wq[j] / (p * p - q[j] * q[j]);
-    D[NQ] = make_double2(-(2.0 / WPCD_PI) * f * p * p * ssum, -f * p);
+    D[NQ] = -(2.0 / WPCD_PI) * f * p * p * ssum;   // the principal-value part; the -i f p part enters after the solve
   }
   __syncthreads();
-  // V on the basis, F = 1 - V diag(D), right-hand sides = on-shell columns of V
+  // V on the basis, F_r = 1 - V diag(D_r), right-hand sides = on-shell columns of V.  Index r < ng: grid point r % NQ of
+  // block r / NQ; r >= ng: on-shell point of block r - ng.
   for (int idx = tid; idx < n * n; idx += kMiThreads) {
     const int r = idx / n, c = idx - r * n;
-    const int a = r / M, i = r - a * M, b = c / M, j = c - b * M;
+    const int a = r < ng ? r / NQ : r - ng, i = r < ng ? r - a * NQ : NQ;
+    const int b = c < ng ? c / NQ : c - ng, j = c < ng ? c - b * NQ : NQ;
     double v;
     if (P.kind == 1) {
       v = -P.lambdaA / ((q[i] * q[i] + P.beta * P.beta) * (q[j] * q[j] + P.beta * P.beta));
@@ -152,89 +164,125 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
     } else if (!P.coupled) v = yukawa_A(lJ, P.nterms, sV0, P.mu, q[i], q[j]);
     else if (a == b) v = yukawa_A(a == 0 ? lJ - 1 : lJ + 1, P.nterms, sV0, P.mu, q[i], q[j]);
     else v = yukawa_A(lJ, 1, &sVT, &P.muT, q[i], q[j]);
-    const double2 d = D[j];
-    F[(size_t)r * ld + c] = make_double2((r == c ? 1.0 : 0.0) - v * d.x, -v * d.y);
-    if (j == NQ) F[(size_t)r * ld + n + b] = make_double2(v, 0.0);
+    F[(size_t)r * ld + c] = (r == c ? 1.0 : 0.0) - v * D[j];
+    if (j == NQ) F[(size_t)r * ld + n + b] = v;
   }
   __syncthreads();
-  // Gauss elimination with partial pivoting
-  for (int c = 0; c < n; ++c) {
+  // Gauss elimination with partial pivoting, ONE barrier per column.  The rows still to be eliminated are kept as a
+  // compact list (double buffered: a column reads list b and writes the list without its pivot row into b^1); the
+  // pivot of column c+1 is found while column c is being eliminated (the lanes that update the entries of column c+1
+  // keep the largest one per warp; double buffered candidates), so there is no separate search phase; a warp updates
+  // four rows at a time with the pivot row's entries loaded once.
+  {
     double best = -1.0;
-    int bi = c;
-    for (int r = c + tid; r < n; r += kMiThreads) {
-      const double2 x = F[(size_t)r * ld + c];
-      const double v = hypot(x.x, x.y);
-      if (v > best) { best = v; bi = r; }
+    int bpos = 0;
+    for (int j = tid; j < n; j += kMiThreads) {
+      lst[j] = j;
+      const double v = fabs(F[(size_t)j * ld]);
+      if (v > best) { best = v; bpos = j; }
     }
-    // arg-max over the CTA: shuffles inside a warp, one round through shared memory across the warps
     for (int o = 16; o > 0; o >>= 1) {
       const double ob = __shfl_xor_sync(0xffffffffu, best, o);
-      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+      const int oi = __shfl_xor_sync(0xffffffffu, bpos, o);
+      if (ob > best || (ob == best && oi < bpos)) { best = ob; bpos = oi; }
     }
-    if ((tid & 31) == 0) { s_red[tid >> 5] = best; s_idx[tid >> 5] = bi; }
-    __syncthreads();
-    if (tid < 32) {
-      best = tid < kMiThreads / 32 ? s_red[tid] : -1.0;
-      bi = tid < kMiThreads / 32 ? s_idx[tid] : n;
-      for (int o = 16; o > 0; o >>= 1) {
-        const double ob = __shfl_xor_sync(0xffffffffu, best, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-      }
-      if (tid == 0) s_idx[kMiThreads / 32] = bi;
-    }
-    __syncthreads();
-    const int piv = s_idx[kMiThreads / 32];
-    if (piv != c)
-      for (int k = c + tid; k < ld; k += kMiThreads) {
-        const double2 t = F[(size_t)c * ld + k];
-        F[(size_t)c * ld + k] = F[(size_t)piv * ld + k];
-        F[(size_t)piv * ld + k] = t;
-      }
-    __syncthreads();
-    const double2 dcc = F[(size_t)c * ld + c];
-    for (int r = c + 1 + tid; r < n; r += kMiThreads) F[(size_t)r * ld + c] = cdiv(F[(size_t)r * ld + c], dcc);  // multiplier
-    __syncthreads();
-    // rank-one update of the trailing block: a warp walks along a row (conflict-free 16-byte accesses), 8 rows at a time
-    for (int k = c + 1 + (tid & 31); k < ld; k += 32) {
-      const double2 pk = F[(size_t)c * ld + k];
-      for (int r = c + 1 + (tid >> 5); r < n; r += kMiThreads / 32) {
-        const double2 x = cmul(F[(size_t)r * ld + c], pk);
-        double2 y = F[(size_t)r * ld + k];
-        y.x -= x.x; y.y -= x.y;
-        F[(size_t)r * ld + k] = y;
-      }
-    }
-    __syncthreads();
+    if (lane == 0) { cval[warp] = best; cpos[warp] = bpos; }
   }
-  // back substitution, column oriented: x_r = b_r / F_rr, then b_r' -= F_r'r x_r for the rows above
-  for (int r = n - 1; r >= 0; --r) {
-    if (tid < nc) F[(size_t)r * ld + n + tid] = cdiv(F[(size_t)r * ld + n + tid], F[(size_t)r * ld + r]);
+  for (int c = 0; c < n; ++c) {
     __syncthreads();
-    for (int idx = tid; idx < r * nc; idx += kMiThreads) {
-      const int rr = idx / nc, b = idx - rr * nc;
-      const double2 x = cmul(F[(size_t)rr * ld + r], F[(size_t)r * ld + n + b]);
-      double2 y = F[(size_t)rr * ld + n + b];
-      y.x -= x.x; y.y -= x.y;
-      F[(size_t)rr * ld + n + b] = y;
+    const int b = c & 1, nact = n - c;
+    const int* lb = lst + b * n;
+    int* ln = lst + (b ^ 1) * n;
+    double best = cval[b * nwarps];
+    int pos = cpos[b * nwarps];
+    for (int w = 1; w < nwarps; ++w) {
+      const double ob = cval[b * nwarps + w];
+      const int oi = cpos[b * nwarps + w];
+      if (ob > best || (ob == best && oi < pos)) { best = ob; pos = oi; }
     }
-    __syncthreads();
+    const int piv = lb[pos], lastr = lb[nact - 1];
+    if (tid == 0) prow[c] = piv;
+    for (int j = tid; j < nact - 1; j += kMiThreads) ln[j] = j == pos ? lastr : lb[j];
+    const double* prw = F + (size_t)piv * ld;
+    const double rp = 1.0 / prw[c];
+    double wbest = -1.0;
+    int wpos = 0;
+    for (int j0 = 4 * warp; j0 < nact - 1; j0 += 4 * nwarps) {
+      double* row[4];
+      double mlt[4];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        const int j = j0 + x < nact - 1 ? j0 + x : j0;   // (a short tail repeats row j0: same values written twice)
+        row[x] = F + (size_t)(j == pos ? lastr : lb[j]) * ld;
+        mlt[x] = row[x][c] * rp;
+      }
+      for (int k = c + 1 + lane; k < ld; k += 32) {
+        const double pk = prw[k];
+        double v[4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v[x] = fma(-mlt[x], pk, row[x][k]);
+#pragma unroll
+        for (int x = 0; x < 4; ++x) row[x][k] = v[x];
+        if (k == c + 1) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x)
+            if (j0 + x < nact - 1 && fabs(v[x]) > wbest) { wbest = fabs(v[x]); wpos = j0 + x; }
+        }
+      }
+    }
+    // lane 0 of a warp saw column c+1 of all its rows
+    wbest = __shfl_sync(0xffffffffu, wbest, 0);
+    wpos = __shfl_sync(0xffffffffu, wpos, 0);
+    if (lane == 0) { cval[(b ^ 1) * nwarps + warp] = wbest; cpos[(b ^ 1) * nwarps + warp] = wpos; }
   }
-  // S = 1 - 2 i f p T_onshell
-  if (tid < nc * nc) {
-    const int a = tid / nc, b = tid - a * nc;
-    const double2 t = F[(size_t)(a * M + NQ) * ld + n + b];
-    const double g = 2.0 * f * p;  // -i g t = (g t.y, -g t.x)
-    double* o = P.Sout + (((smp * P.nch + ch) * P.nE + e) * nc * nc + tid) * 2;
-    o[0] = (a == b ? 1.0 : 0.0) + g * t.y;
-    o[1] = -g * t.x;
+  __syncthreads();
+  // the on-shell unknowns are the last nc columns: K_on from the last nc pivot rows (upper triangular in pivot order)
+  if (tid == 0) {
+    double K[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+    const double* r1 = F + (size_t)prow[n - 1] * ld;
+    if (nc == 1) {
+      K[0][0] = r1[n] / r1[n - 1];
+    } else {
+      const double* r0 = F + (size_t)prow[n - 2] * ld;
+      for (int b = 0; b < 2; ++b) {
+        K[1][b] = r1[n + b] / r1[n - 1];
+        K[0][b] = (r0[n + b] - r0[n - 1] * K[1][b]) / r0[n - 2];
+      }
+    }
+    // T_on = K_on (1 + i g K_on)^-1, S = 1 - 2 i g T_on, g = f p
+    const double g = f * p;
+    double* o = P.Sout + ((smp * P.nch + ch) * P.nE + e) * (size_t)(nc * nc * 2);
+    if (nc == 1) {
+      const double x = g * K[0][0], den = 1.0 + x * x;
+      o[0] = (1.0 - x * x) / den;
+      o[1] = -2.0 * x / den;
+    } else {
+      // M = 1 + i g K;  M^-1 = adj(M)/det(M)
+      const double2 m00 = make_double2(1.0, g * K[0][0]), m01 = make_double2(0.0, g * K[0][1]);
+      const double2 m10 = make_double2(0.0, g * K[1][0]), m11 = make_double2(1.0, g * K[1][1]);
+      const double2 d1 = cmul(m00, m11), d2 = cmul(m01, m10);
+      const double2 det = make_double2(d1.x - d2.x, d1.y - d2.y);
+      const double2 one = make_double2(1.0, 0.0);
+      const double2 idet = cdiv(one, det);
+      const double2 i00 = cmul(m11, idet), i11 = cmul(m00, idet);
+      const double2 i01 = cmul(make_double2(-m01.x, -m01.y), idet), i10 = cmul(make_double2(-m10.x, -m10.y), idet);
+      const double2 inv[2][2] = {{i00, i01}, {i10, i11}};
+      for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) {
+          // T_ab = sum_c K_ac inv_cb (K real)
+          const double tr = K[a][0] * inv[0][b].x + K[a][1] * inv[1][b].x;
+          const double ti = K[a][0] * inv[0][b].y + K[a][1] * inv[1][b].y;
+          // -2 i g (tr + i ti) = 2 g ti - 2 i g tr
+          o[(a * 2 + b) * 2] = (a == b ? 1.0 : 0.0) + 2.0 * g * ti;
+          o[(a * 2 + b) * 2 + 1] = -2.0 * g * tr;
+        }
+    }
   }
 }
 
 size_t mi_smem(int NQ, int coupled) {
   const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = n + nc;
-  return (size_t)n * ld * 16 + (size_t)(M + (M & 1)) * 8 + (size_t)M * 16;
+  return (size_t)n * ld * 8 + (size_t)2 * M * 8 + (size_t)3 * n * 4 + 16;
 }
 
 }  // namespace
