@@ -149,7 +149,8 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     val = solves / dt
     sample = f"{n_each} samples x (1S0 + 3S1-3D1) per step, threads over solves; same inputs as the GPU arm"
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "channel-solves/s", "n_gpus": 1,
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "channel-solves/s", "n_gpus": args.gpus,
+            "ranks_working": 1,   # the oracle runs on rank 0's host cores only, whatever N the driver launched
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.N, args.samples, args.nE), "bounded_sample": sample},
