@@ -19,7 +19,7 @@ class Pipeline:
                  onshell_rows_only=True, channel_J=None, mode=0, n_gl=8, energy_packets=False):
         self.h = wpcd.Handle(device)
         self.dev = self.h.device
-        self.edges = np.asarray(edges, dtype=np.float64)
+        self.edges = np.ascontiguousarray(edges, dtype=np.float64)
         self.N = len(self.edges) - 1
         self.channels = list(channels)
         self.S = int(S)
@@ -113,6 +113,19 @@ class Pipeline:
             self.h.sigma_tot(self.J[0], self.kind[0]["T"] if 0 in self.kind else None, self.J[1],
                              self.kind[1]["T"] if 1 in self.kind else None, any_kind["bins"], self.geo["dE"], self.Ecm,
                              out=self.sigma)
+
+    def capture(self):
+        """Captures one pass (solve_device) into a CUDA graph: the pass is a fixed sequence of 14-15 small launches on
+        preallocated buffers, so for ONE potential sample (the paper's Table-1 use, latency bound) replaying the graph removes
+        the launch overhead.  Returns a callable that replays it on the current stream."""
+        for _ in range(2):
+            self.solve_device()          # warm-up outside the capture (function attributes, lazy module loading)
+        torch.cuda.synchronize(self.dev)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            self.solve_device()
+        self.graph = graph
+        return graph.replay
 
     def stage_names(self):
         names = ["build"]

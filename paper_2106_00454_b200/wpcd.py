@@ -134,7 +134,12 @@ class Handle:
         """edges: host sequence [N+1]; channels: list of (coupled, lJ); scales: device tensor [S][P] or None.
         Returns dict(H_unc, H_cpl, e0, dE, Eedge) of device tensors."""
         N = len(edges) - 1
-        h_edges = (C.c_double * (N + 1))(*[float(x) for x in edges])
+        if hasattr(edges, "ctypes") and edges.dtype.name == "float64" and edges.flags["C_CONTIGUOUS"]:
+            # the caller's array is used in place: the library copies it to the device asynchronously (a captured CUDA graph
+            # replays that copy, so the array has to outlive the graph -- Pipeline keeps it)
+            h_edges = edges.ctypes.data_as(C.POINTER(C.c_double))
+        else:
+            h_edges = (C.c_double * (N + 1))(*[float(x) for x in edges])
         grid = Grid(N, h_edges, hbarc, mured, n_gl, 1 if energy_packets else 0)
         pot = Potential()
         keep = []
