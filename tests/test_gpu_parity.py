@@ -742,6 +742,29 @@ def test_large_n_batch_exceeds_grid(ctx, N, S, picks):
         _compare_channel(res, 1, Sc - 1, 0, N, 1, Ecm, scale=tuple(scales[Sc - 1]), label=f"batch>grid N={N} coupled s={Sc - 1}")
 
 
+def test_pipeline_cuda_graph_replay_and_fp64_probe(ctx):
+    """Pipeline.capture(): the pass replayed as a CUDA graph gives bit-identical phase shifts for new inputs written into the
+    pipeline's buffers; wpcd_probe_fp64 (the in-run FP64 peak measurement of bench.py) launches and reports its flop count."""
+    torch = ctx["torch"]
+    from paper_2106_00454_b200.pipeline import Pipeline
+    tl, Ecm = inp.energies(50)
+    pot = dict(V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
+    pipe = Pipeline(inp.grid_edges(24), [(0, 0), (1, 1)], Ecm, 3, pot, device=0)
+    replay = pipe.capture()
+    sc = torch.as_tensor(inp.sample_scales(3, seed=5), device=ctx["dev"])
+    pipe.scales.copy_(sc)
+    pipe.solve_device(); torch.cuda.synchronize()
+    ref = {k: b["delta"].clone() for k, b in pipe.kind.items()}
+    for b in pipe.kind.values():
+        b["delta"].zero_()
+    replay(); torch.cuda.synchronize()
+    for k, b in pipe.kind.items():
+        assert torch.equal(b["delta"], ref[k]) and bool((b["info"] >= 1).all())
+    flops, sink = ctx["h"].probe_fp64(1, 200)
+    torch.cuda.synchronize()
+    assert flops == sink.numel() / 32 * 200 * 8 * 512 and bool(torch.isfinite(sink).all())
+
+
 def test_zz_arbitration_only_where_design_allows():
     """Runs last in this module: every case that needed the 80-bit arbiter is on DESIGN.md section 3's list (n >= 600 or
     N >= 400 on the config grid, or the Chebyshev grid); the assertion at the point of use already failed otherwise -- this prints the
