@@ -16,6 +16,7 @@
 namespace {
 
 constexpr int kMiThreads = 256;
+constexpr int kMiWarps = kMiThreads / 32;   // one thread per row in the panel factorisation: n <= 166 < 256
 
 struct MiParams {
   const double* kq;      // [NQ] grid momenta
@@ -33,6 +34,8 @@ struct MiParams {
   double lambdaA, beta;
   double hbarc, mured;
   const double* basis;                                   // [nbasis][NQ][NQ]: Q_l(z(k_i,k_j))/(2 k_i k_j) per distinct (l, mu)
+  const double* onb;                                     // [chunk energies][nbasis][NQ+1]: the same for (p, k_j), j = NQ: (p, p)
+  int nbasis, e_first;                                   // this launch covers energies e_first .. e_first + gridDim.x - 1
   int id_mm[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // basis matrix of term t in the block l = lJ (uncoupled) / J-1
   int id_pp[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // ... in the block l = J+1
   int id_mp[WPCD_MAX_CHANNELS];                           // ... of the off-diagonal Yukawa
@@ -49,7 +52,19 @@ __global__ void k_mi_basis(int NQ, MiBasisTable tab, const double* __restrict__ 
   const double kp = kq[i], k = kq[j], mu = tab.mu[blockIdx.y];
   const double diff = kp - k;
   const double zm1 = fma(diff, diff, mu * mu) / (2.0 * kp * k);
-  basis[(size_t)blockIdx.y * NQ * NQ + idx] = legendre_q(tab.l[blockIdx.y], zm1);
+  basis[(size_t)blockIdx.y * NQ * NQ + idx] = legendre_q(tab.l[blockIdx.y], zm1) / (2.0 * kp * k);
+}
+
+// The on-shell row/column of V depends on the energy but not on the sample or the channel beyond (l, mu): one table per
+// (energy of the chunk, distinct (l, mu)), entries j < NQ for (p, k_j), entry NQ for (p, p).  grid (chunk, nbasis).
+__global__ void k_mi_onbasis(int NQ, MiBasisTable tab, const double* __restrict__ kq, const double* __restrict__ Ecm, int e_first,
+                             double cE, double* __restrict__ onb) {
+  const int j = threadIdx.x, b = blockIdx.y;
+  if (j > NQ) return;
+  const double p = sqrt(Ecm[e_first + blockIdx.x] / cE), k = j < NQ ? kq[j] : p, mu = tab.mu[b];
+  const double diff = p - k;
+  const double zm1 = fma(diff, diff, mu * mu) / (2.0 * p * k);
+  onb[((size_t)blockIdx.x * gridDim.y + b) * (NQ + 1) + j] = legendre_q(tab.l[b], zm1) / (2.0 * p * k);
 }
 
 // k_j, w_j of the MI grid: root a of P_NQ by Newton, mapped with c tan(pi(1+x)/4)
@@ -76,14 +91,10 @@ __global__ void k_mi_grid(int NQ, double cmap, double* __restrict__ kq, double* 
   wq[a] = cmap * (WPCD_PI / 4.0) * w / (c * c);
 }
 
-__device__ __forceinline__ double yukawa_A(int l, int nterms, const double* V0, const double* mu, double kp, double k) {
-  double s = 0.0;
-  for (int t = 0; t < nterms; ++t) {
-    const double diff = kp - k;
-    const double zm1 = fma(diff, diff, mu[t] * mu[t]) / (2.0 * kp * k);
-    s += V0[t] * legendre_q(l, zm1);
-  }
-  return s / (2.0 * kp * k);
+__device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {  // D (8x8) += A (8x4, row) B (4x8, col), fp64 tensor core
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d[0]), "+d"(d[1])
+               : "d"(a), "d"(b));
 }
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -105,20 +116,21 @@ __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
 __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kMiThreads / 32;
-  const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = n + nc, ng = nc * NQ;
+  const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1, ng = nc * NQ;  // ld even: 16-byte row pairs
   double* F = reinterpret_cast<double*>(smem_raw);       // [n][ld]
   double* q = F + (size_t)n * ld;                         // [M]
   double* D = q + M;                                      // [M] real parts (principal value)
   int* prow = reinterpret_cast<int*>(D + M);              // [n] pivot row of column c
   int* lst = prow + n;                                    // [2][n] rows not yet used as a pivot (double buffered)
   __shared__ double sV0[WPCD_MAX_TERMS], sVT;
-  __shared__ double cval[2 * (kMiThreads / 32)];         // pivot candidates per warp (double buffered)
-  __shared__ int cpos[2 * (kMiThreads / 32)];
-  const int e = blockIdx.x, ch = blockIdx.y;
+  __shared__ double cval[2 * kMiWarps];                   // pivot candidate of every warp (double buffered over the columns)
+  __shared__ int cpos[2 * kMiWarps];
+  __shared__ double pb[2 * kMiWarps * 8];                 // ... and the panel entries of that row
+  __shared__ int pivpos[8];                               // list positions of the panel's pivot rows
+  const int e = P.e_first + blockIdx.x, ch = blockIdx.y;
   const size_t smp = blockIdx.z;
   const double cE = P.hbarc * P.hbarc / (2.0 * P.mured), f = 2.0 * P.mured / (P.hbarc * P.hbarc);
   const double p = sqrt(P.Ecm[e] / cE);
-  const int lJ = P.lJ[ch];
   if (tid < P.nterms) {
     double v = P.V0[tid];
     if (P.scales && P.sidx[tid] >= 0) v *= P.scales[smp * P.P + P.sidx[tid]];
@@ -144,98 +156,171 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   __syncthreads();
   // V on the basis, F_r = 1 - V diag(D_r), right-hand sides = on-shell columns of V.  Index r < ng: grid point r % NQ of
   // block r / NQ; r >= ng: on-shell point of block r - ng.
-  for (int idx = tid; idx < n * n; idx += kMiThreads) {
-    const int r = idx / n, c = idx - r * n;
+  // A warp per row, lanes along the columns; every Yukawa element comes from the tables (grid x grid: basis, per call;
+  // row/column of the on-shell point: onb, per energy), scaled by this sample's strengths.
+  const double* onb = P.onb + (size_t)blockIdx.x * P.nbasis * M;
+  const size_t nn = (size_t)NQ * NQ;
+  for (int r = warp; r < n; r += nwarps) {
     const int a = r < ng ? r / NQ : r - ng, i = r < ng ? r - a * NQ : NQ;
-    const int b = c < ng ? c / NQ : c - ng, j = c < ng ? c - b * NQ : NQ;
-    double v;
-    if (P.kind == 1) {
-      v = -P.lambdaA / ((q[i] * q[i] + P.beta * P.beta) * (q[j] * q[j] + P.beta * P.beta));
-    } else if (i < NQ && j < NQ) {  // grid x grid: tabulated Q_l, same arithmetic as yukawa_A
-      const size_t o = (size_t)i * NQ + j, nn = (size_t)NQ * NQ;
-      double sacc = 0.0;
-      if (a == b) {
-        const int* id = (P.coupled && a == 1) ? P.id_pp[ch] : P.id_mm[ch];
-        for (int t = 0; t < P.nterms; ++t) sacc += sV0[t] * P.basis[id[t] * nn + o];
+    double* Fr = F + (size_t)r * ld;
+    for (int c = lane; c < n; c += 32) {
+      const int b = c < ng ? c / NQ : c - ng, j = c < ng ? c - b * NQ : NQ;
+      double v;
+      if (P.kind == 1) {
+        v = -P.lambdaA / ((q[i] * q[i] + P.beta * P.beta) * (q[j] * q[j] + P.beta * P.beta));
       } else {
-        sacc += sVT * P.basis[P.id_mp[ch] * nn + o];
-      }
-      v = sacc / (2.0 * q[i] * q[j]);
-    } else if (!P.coupled) v = yukawa_A(lJ, P.nterms, sV0, P.mu, q[i], q[j]);
-    else if (a == b) v = yukawa_A(a == 0 ? lJ - 1 : lJ + 1, P.nterms, sV0, P.mu, q[i], q[j]);
-    else v = yukawa_A(lJ, 1, &sVT, &P.muT, q[i], q[j]);
-    F[(size_t)r * ld + c] = (r == c ? 1.0 : 0.0) - v * D[j];
-    if (j == NQ) F[(size_t)r * ld + n + b] = v;
-  }
-  __syncthreads();
-  // Gauss elimination with partial pivoting, ONE barrier per column.  The rows still to be eliminated are kept as a
-  // compact list (double buffered: a column reads list b and writes the list without its pivot row into b^1); the
-  // pivot of column c+1 is found while column c is being eliminated (the lanes that update the entries of column c+1
-  // keep the largest one per warp; double buffered candidates), so there is no separate search phase; a warp updates
-  // four rows at a time with the pivot row's entries loaded once.
-  {
-    double best = -1.0;
-    int bpos = 0;
-    for (int j = tid; j < n; j += kMiThreads) {
-      lst[j] = j;
-      const double v = fabs(F[(size_t)j * ld]);
-      if (v > best) { best = v; bpos = j; }
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-      const double ob = __shfl_xor_sync(0xffffffffu, best, o);
-      const int oi = __shfl_xor_sync(0xffffffffu, bpos, o);
-      if (ob > best || (ob == best && oi < bpos)) { best = ob; bpos = oi; }
-    }
-    if (lane == 0) { cval[warp] = best; cpos[warp] = bpos; }
-  }
-  for (int c = 0; c < n; ++c) {
-    __syncthreads();
-    const int b = c & 1, nact = n - c;
-    const int* lb = lst + b * n;
-    int* ln = lst + (b ^ 1) * n;
-    double best = cval[b * nwarps];
-    int pos = cpos[b * nwarps];
-    for (int w = 1; w < nwarps; ++w) {
-      const double ob = cval[b * nwarps + w];
-      const int oi = cpos[b * nwarps + w];
-      if (ob > best || (ob == best && oi < pos)) { best = ob; pos = oi; }
-    }
-    const int piv = lb[pos], lastr = lb[nact - 1];
-    if (tid == 0) prow[c] = piv;
-    for (int j = tid; j < nact - 1; j += kMiThreads) ln[j] = j == pos ? lastr : lb[j];
-    const double* prw = F + (size_t)piv * ld;
-    const double rp = 1.0 / prw[c];
-    double wbest = -1.0;
-    int wpos = 0;
-    for (int j0 = 4 * warp; j0 < nact - 1; j0 += 4 * nwarps) {
-      double* row[4];
-      double mlt[4];
-#pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        const int j = j0 + x < nact - 1 ? j0 + x : j0;   // (a short tail repeats row j0: same values written twice)
-        row[x] = F + (size_t)(j == pos ? lastr : lb[j]) * ld;
-        mlt[x] = row[x][c] * rp;
-      }
-      for (int k = c + 1 + lane; k < ld; k += 32) {
-        const double pk = prw[k];
-        double v[4];
-#pragma unroll
-        for (int x = 0; x < 4; ++x) v[x] = fma(-mlt[x], pk, row[x][k]);
-#pragma unroll
-        for (int x = 0; x < 4; ++x) row[x][k] = v[x];
-        if (k == c + 1) {
-#pragma unroll
-          for (int x = 0; x < 4; ++x)
-            if (j0 + x < nact - 1 && fabs(v[x]) > wbest) { wbest = fabs(v[x]); wpos = j0 + x; }
+        const bool gg = i < NQ && j < NQ;
+        const size_t o = gg ? (size_t)i * NQ + j : (size_t)(i < j ? i : j);   // on-shell tables: index of the grid point (NQ: p itself)
+        v = 0.0;
+        if (a == b) {
+          const int* id = (P.coupled && a == 1) ? P.id_pp[ch] : P.id_mm[ch];
+          for (int t = 0; t < P.nterms; ++t) v += sV0[t] * (gg ? P.basis[id[t] * nn + o] : onb[id[t] * M + o]);
+        } else {
+          v = sVT * (gg ? P.basis[P.id_mp[ch] * nn + o] : onb[P.id_mp[ch] * M + o]);
         }
       }
+      Fr[c] = (r == c ? 1.0 : 0.0) - v * D[j];
+      if (j == NQ) Fr[n + b] = v;
     }
-    // lane 0 of a warp saw column c+1 of all its rows
-    wbest = __shfl_sync(0xffffffffu, wbest, 0);
-    wpos = __shfl_sync(0xffffffffu, wpos, 0);
-    if (lane == 0) { cval[(b ^ 1) * nwarps + warp] = wbest; cpos[(b ^ 1) * nwarps + warp] = wpos; }
+    if (lane == 0 && ld > n + nc) Fr[ld - 1] = 0.0;   // padding column
   }
   __syncthreads();
+  // Blocked Gauss elimination with partial pivoting (right-looking, panels of 8 columns):
+  //   (1) the panel is factorised in registers, one thread per row still to be eliminated, one barrier per column (the
+  //       arg-max candidates of the warps travel with their rows' panel entries); multipliers stored in place -- the same
+  //       pivot sequence as column-by-column partial pivoting;
+  //   (2) the pivot rows' entries right of the panel get the panel's unit-lower-triangular solve (one thread per column),
+  //       while another warp removes the pivot rows from the compact list of active rows;
+  //   (3) trailing update A22 -= L21 U12 as fp64 tensor-core products (mma.sync m8n8k4, two per 8x8 tile).
+  for (int j = tid; j < n; j += kMiThreads) lst[j] = j;
+  __syncthreads();
+  for (int c0 = 0, m = n, lb = 0; c0 < n; c0 += 8, lb ^= 1) {
+    const int w = n - c0 < 8 ? n - c0 : 8;   // panel width
+    const int* la = lst + lb * n;            // active rows before this panel (m of them)
+    int* ln = lst + (lb ^ 1) * n;            // ... after it (m - w)
+    {
+      // (1) panel factorisation: thread j < m holds the 8 panel entries of active row j.  Per column ONE barrier: every
+      // warp publishes its best candidate TOGETHER with that row's panel entries, after the barrier all threads pick the
+      // winner among the warps and eliminate their own row.
+      const bool mine = tid < m;
+      double a[8];
+      {
+        const double* src = F + (size_t)(mine ? la[tid] : 0) * ld + c0;
+#pragma unroll
+        for (int x = 0; x < 8; ++x) a[x] = (mine && x < w) ? src[x] : 0.0;
+      }
+      bool used = !mine;
+      const int nrw = (m + 31) >> 5;   // warps that hold rows
+#pragma unroll
+      for (int x = 0; x < 8; ++x) {
+        if (x < w) {
+          const int cb = x & 1;
+          double best = used ? -1.0 : fabs(a[x]);
+          int bj = tid;
+          for (int o = 16; o > 0; o >>= 1) {
+            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
+            if (ob > best || (ob == best && oj < bj)) { best = ob; bj = oj; }
+          }
+          if (warp < nrw && bj == tid) {
+            cval[cb * kMiWarps + warp] = best;
+            cpos[cb * kMiWarps + warp] = tid;
+#pragma unroll
+            for (int x2 = 0; x2 < 8; ++x2) pb[(cb * kMiWarps + warp) * 8 + x2] = a[x2];
+          }
+          __syncthreads();
+          double gbest = cval[cb * kMiWarps];
+          int gw = 0;
+          for (int ww = 1; ww < nrw; ++ww) {
+            const double ob = cval[cb * kMiWarps + ww];
+            if (ob > gbest) { gbest = ob; gw = ww; }
+          }
+          const int gpos = cpos[cb * kMiWarps + gw];
+          double pr[8];
+#pragma unroll
+          for (int x2 = 0; x2 < 8; ++x2) pr[x2] = pb[(cb * kMiWarps + gw) * 8 + x2];
+          if (tid == gpos) {
+            used = true;
+            prow[c0 + x] = la[tid];
+            pivpos[x] = tid;
+          }
+          if (!used) {
+            const double mlt = a[x] / pr[x];
+            a[x] = mlt;
+#pragma unroll
+            for (int x2 = x + 1; x2 < 8; ++x2) a[x2] = fma(-mlt, pr[x2], a[x2]);
+          }
+        }
+      }
+      if (mine) {
+        double* dst = F + (size_t)la[tid] * ld + c0;
+#pragma unroll
+        for (int x = 0; x < 8; ++x)
+          if (x < w) dst[x] = a[x];
+      }
+    }
+    __syncthreads();
+    // (2) U12 = L11^-1 A12 on the pivot rows (thread per column right of the panel), and the new list of active rows
+    if (tid < ld - c0 - w) {
+      const int k = c0 + w + tid;
+      double u[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) u[i] = i < w ? F[(size_t)prow[c0 + i] * ld + k] : 0.0;
+#pragma unroll
+      for (int i = 1; i < 8; ++i)
+        if (i < w) {
+          const double* li = F + (size_t)prow[c0 + i] * ld + c0;   // multipliers of pivot row i (columns c0 .. c0+i-1)
+          double acc = u[i];
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            if (j < i) acc = fma(-li[j], u[j], acc);
+          u[i] = acc;
+        }
+#pragma unroll
+      for (int i = 1; i < 8; ++i)
+        if (i < w) F[(size_t)prow[c0 + i] * ld + k] = u[i];
+    }
+    if (warp == nwarps - 1) {
+      int base = 0;
+      for (int j0 = 0; j0 < m; j0 += 32) {
+        const int j = j0 + lane;
+        bool keep = j < m;
+#pragma unroll
+        for (int x = 0; x < 8; ++x) keep = keep && !(x < w && pivpos[x] == j);
+        const unsigned bal = __ballot_sync(0xffffffffu, keep);
+        if (keep) ln[base + __popc(bal & ((1u << lane) - 1u))] = la[j];
+        base += __popc(bal);
+      }
+    }
+    __syncthreads();
+    // (3) trailing update of the remaining rows, columns right of the panel (right-hand sides included)
+    const int mr = m - w, ncol = ld - c0 - w;
+    if (mr > 0 && ncol > 0) {
+      const int g = lane >> 2, t = lane & 3;
+      const int rt_n = (mr + 7) >> 3, ct_n = (ncol + 7) >> 3;
+      for (int tile = warp; tile < rt_n * ct_n; tile += nwarps) {
+        const int rt = tile / ct_n, ct = tile - rt * ct_n;
+        const int jr = 8 * rt + g < mr ? 8 * rt + g : mr - 1;        // (a short tail repeats the last row: same values twice)
+        double* rowp = F + (size_t)ln[jr] * ld;
+        const int k0 = c0 + w + 8 * ct;
+        const int kb = k0 + g < ld ? k0 + g : ld - 1;
+        double cfr[2];
+        const bool cin = k0 + 2 * t < ld;                            // ld and k0 are even: both columns of the pair or none
+        const double2 cc = cin ? *reinterpret_cast<const double2*>(rowp + k0 + 2 * t) : make_double2(0.0, 0.0);
+        cfr[0] = cc.x; cfr[1] = cc.y;
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int x = 4 * hh + t;
+          const double av = x < w ? -rowp[c0 + x] : 0.0;
+          const double bv = x < w ? F[(size_t)prow[c0 + x] * ld + kb] : 0.0;
+          dmma(cfr, av, bv);
+        }
+        if (cin && 8 * rt + g < mr) *reinterpret_cast<double2*>(rowp + k0 + 2 * t) = make_double2(cfr[0], cfr[1]);
+      }
+    }
+    m = mr;
+    __syncthreads();
+  }
   // the on-shell unknowns are the last nc columns: K_on from the last nc pivot rows (upper triangular in pivot order)
   if (tid == 0) {
     double K[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
@@ -281,14 +366,17 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
 }
 
 size_t mi_smem(int NQ, int coupled) {
-  const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = n + nc;
+  const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1;
   return (size_t)n * ld * 8 + (size_t)2 * M * 8 + (size_t)3 * n * 4 + 16;
 }
 
 }  // namespace
 
 constexpr int kMiMaxBasis = WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1);
-size_t wpcd_mi_workspace(int NQ) { return (size_t)2 * ((NQ * 8 + 255) & ~255) + (size_t)kMiMaxBasis * NQ * NQ * 8; }
+constexpr int kMiEChunk = 128;   // energies per launch: the on-shell tables of one chunk live in the workspace
+size_t wpcd_mi_workspace(int NQ) {
+  return (size_t)2 * ((NQ * 8 + 255) & ~255) + (size_t)kMiMaxBasis * NQ * NQ * 8 + (size_t)kMiEChunk * kMiMaxBasis * (NQ + 1) * 8;
+}
 
 // does the system of this kind fit one CTA's shared memory?
 bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled) { return mi_smem(NQ, coupled) + 4096 <= (size_t)h->max_smem_optin; }
@@ -299,6 +387,8 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
   double* kq = static_cast<double*>(d_work);
   double* wq = reinterpret_cast<double*>(static_cast<char*>(d_work) + ((NQ * 8 + 255) & ~255));
   double* basis = reinterpret_cast<double*>(static_cast<char*>(d_work) + 2 * ((NQ * 8 + 255) & ~255));
+  double* onb = basis + (size_t)kMiMaxBasis * NQ * NQ;
+  const double cE = hbarc * hbarc / (2.0 * mu);
   k_mi_grid<<<(NQ + 127) / 128, 128, 0, st>>>(NQ, cmap, kq, wq);
   // distinct (l, mu) of all channel blocks
   MiBasisTable bt; bt.n = 0;
@@ -317,10 +407,13 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
     for (int c = 0; c < n_chan; ++c) if (chan[c].coupled) ids_mp[c] = find_or_add(chan[c].lJ, pot->muT);
     k_mi_basis<<<dim3((NQ * NQ + 255) / 256, bt.n), 256, 0, st>>>(NQ, bt, kq, basis);
   }
+  for (int e_first = 0; e_first < nE; e_first += kMiEChunk) {
+  const int ne = nE - e_first < kMiEChunk ? nE - e_first : kMiEChunk;
+  if (pot->kind == 0) k_mi_onbasis<<<dim3(ne, bt.n), (NQ + 1 + 31) / 32 * 32, 0, st>>>(NQ, bt, kq, d_Ecm, e_first, cE, onb);
   for (int coupled = 0; coupled < 2; ++coupled) {
     MiParams Q;
     Q.kq = kq; Q.wq = wq; Q.Ecm = d_Ecm; Q.scales = d_scales; Q.Sout = coupled ? d_S_cpl : d_S_unc;
-    Q.NQ = NQ; Q.nE = nE; Q.P = P; Q.coupled = coupled; Q.nch = 0; Q.basis = basis;
+    Q.NQ = NQ; Q.nE = nE; Q.P = P; Q.coupled = coupled; Q.nch = 0; Q.basis = basis; Q.onb = onb; Q.nbasis = bt.n; Q.e_first = e_first;
     for (int c = 0; c < n_chan; ++c)
       if ((chan[c].coupled ? 1 : 0) == coupled) {
         for (int t = 0; t < WPCD_MAX_TERMS; ++t) { Q.id_mm[Q.nch][t] = ids_mm[c][t]; Q.id_pp[Q.nch][t] = ids_pp[c][t]; }
@@ -340,7 +433,8 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
     const size_t smem = mi_smem(NQ, coupled);
     int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_mi_solve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "mi attr");
     if (rc) return rc;
-    k_mi_solve<<<dim3(nE, Q.nch, S), kMiThreads, smem, st>>>(Q);
+    k_mi_solve<<<dim3(ne, Q.nch, S), kMiThreads, smem, st>>>(Q);
+  }
   }
   return wpcd_check_cuda(h, cudaGetLastError(), "mi_solve launch");
 }
