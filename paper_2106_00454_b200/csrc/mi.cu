@@ -115,7 +115,7 @@ __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
 // K_on falls out of the last nc pivots without a back substitution over the grid.
 __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = kMiThreads / 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x, nwarps = nthr >> 5;  // nthr >= n (mi_threads)
   const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1, ng = nc * NQ;  // ld even: 16-byte row pairs
   double* F = reinterpret_cast<double*>(smem_raw);       // [n][ld]
   double* q = F + (size_t)n * ld;                         // [M]
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
     sVT = v;
     q[NQ] = p;
   }
-  for (int j = tid; j < NQ; j += kMiThreads) {
+  for (int j = tid; j < NQ; j += nthr) {
     const double k = P.kq[j];
     q[j] = k;
     D[j] = (2.0 / WPCD_PI) * P.wq[j] * k * k * f / (p * p - k * k);
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   //   (2) the pivot rows' entries right of the panel get the panel's unit-lower-triangular solve (one thread per column),
   //       while another warp removes the pivot rows from the compact list of active rows;
   //   (3) trailing update A22 -= L21 U12 as fp64 tensor-core products (mma.sync m8n8k4, two per 8x8 tile).
-  for (int j = tid; j < n; j += kMiThreads) lst[j] = j;
+  for (int j = tid; j < n; j += nthr) lst[j] = j;
   __syncthreads();
   for (int c0 = 0, m = n, lb = 0; c0 < n; c0 += 8, lb ^= 1) {
     const int w = n - c0 < 8 ? n - c0 : 8;   // panel width
@@ -365,6 +365,13 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   }
 }
 
+// threads of a CTA (>= one per row of the system): two warps for n <= 64 (many CTAs per SM; measured N_Q = 24: 0.42 -> 0.23 ms
+// per sample), the full 256 above, where the assembly and the trailing updates use them (N_Q = 96: 1.61 ms against 1.91 with 128)
+int mi_threads(int NQ, int coupled) {
+  const int n = (coupled ? 2 : 1) * (NQ + 1);
+  return n <= 64 ? 64 : kMiThreads;
+}
+
 size_t mi_smem(int NQ, int coupled) {
   const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1;
   return (size_t)n * ld * 8 + (size_t)2 * M * 8 + (size_t)3 * n * 4 + 16;
@@ -433,7 +440,7 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
     const size_t smem = mi_smem(NQ, coupled);
     int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_mi_solve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "mi attr");
     if (rc) return rc;
-    k_mi_solve<<<dim3(ne, Q.nch, S), kMiThreads, smem, st>>>(Q);
+    k_mi_solve<<<dim3(ne, Q.nch, S), mi_threads(NQ, coupled), smem, st>>>(Q);
   }
   }
   return wpcd_check_cuda(h, cudaGetLastError(), "mi_solve launch");
