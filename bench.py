@@ -468,6 +468,27 @@ def run_config5_sweep(args):
         with ThreadPoolExecutor(max_workers=cores) as ex:
             res = list(ex.map(mi_one, idx))
         mi_s = time.perf_counter() - w0
+        # ---- the same MI systems on the GPU (wpcd_mi_solve: K-matrix form), where they fit one CTA's shared memory
+        mi_gpu = None
+        try:
+            from paper_2106_00454_b200 import wpcd as _w
+            hg = _w.Handle(0)
+            dEc = torch.as_tensor(np.ascontiguousarray(Ecm), device="cuda:0")
+            sc0 = torch.as_tensor(scales[:1].copy(), device="cuda:0")
+            chans = [(0, 0), (1, 1)] if N <= 81 else [(0, 0)] if N <= 164 else []
+            if chans:
+                for _ in range(2):
+                    hg.mi_solve(chans, dEc, NQ=N, scales=sc0, S=1, **pot)
+                torch.cuda.synchronize()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(); Sg_u, Sg_c = hg.mi_solve(chans, dEc, NQ=N, scales=sc0, S=1, **pot); g1.record(); torch.cuda.synchronize()
+                Su = Sg_u.cpu().numpy()[0, 0]; Su = Su[..., 0] + 1j * Su[..., 1]
+                mi_gpu = {"channels": "1S0 + 3S1-3D1" if len(chans) == 2 else "1S0 only (coupled system too large for one CTA)",
+                          "ms_per_sample_350_energies": g0.elapsed_time(g1),
+                          "max_abs_dS_vs_cpu_oracle_1S0": float(np.abs(Su[idx] - np.array([r[0] for r in res])).max())}
+            hg.close()
+        except Exception as ex:  # context leg only: never fails the sweep
+            mi_gpu = {"error": str(ex)[:200]}
         du = np.array([0.5 * np.degrees(np.angle(r[0])) for r in res])
         dc = np.array([[0.5 * np.degrees(np.angle(r[1][0, 0])), 0.5 * np.degrees(np.angle(r[1][1, 1]))] for r in res])
         eu = d180(d_unc[idx], du)
@@ -476,6 +497,7 @@ def run_config5_sweep(args):
                         "mi_cpu_oracle": {"N_Q": N, "energies_solved": int(len(idx)), "wall_s": mi_s,
                                           "wall_s_per_sample_350_energies": mi_s * nE / len(idx), "cores": cores,
                                           "systems": "1S0 (N_Q+1 complex) + 3S1-3D1 (2 N_Q + 2 complex) per energy"},
+                        "mi_gpu": mi_gpu,
                         "wpcd_gpu_ms_per_sample_in_batch": ms / S,
                         "method_error_deg": {"1S0_median": float(np.median(eu)), "1S0_max": float(eu.max()),
                                              "3S1_3D1_delta_median": float(np.median(ec)), "3S1_3D1_delta_max": float(ec.max())}}
