@@ -129,6 +129,23 @@ int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double*
                       double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
                       void* stream);
 
+/* wpcd_diag_batched for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same kernels on the same arguments, Eq. 21, with the workspace taken from a
+ * file-scope device array of WPCD_STATIC_WORK_BYTES inside the library instead of d_work.  The call allocates nothing
+ * (no cudaMalloc / cudaFree / allocating library routine; the array's device address is looked up once per device, at
+ * the first call on that device).  Every GPU that loads the library holds the array until the process exits.
+ *   - sizes: wpcd_diag_workspace_bytes(handle, n, batch) must be <= WPCD_STATIC_WORK_BYTES, else WPCD_ESIZE before any
+ *     launch (wpcd_last_cuda_error then holds the sizes).  16 MiB cover n <= 32 at any batch, n = 100 up to batch 193,
+ *     n = 200 up to batch 52 -- one potential sample of the paper's channel list -- not the production batches.
+ *   - ALL calls on a device share the one array: two calls that overlap on the GPU (different streams, or graphs replayed
+ *     concurrently) race and give wrong results; calls in one stream are ordered and safe.  The array keeps the previous
+ *     call's contents; nothing in it needs clearing by the caller: the schedule tables and the work counter are rewritten
+ *     by the first kernel of every call and each CTA initialises its own eigenvector workspace per matrix.
+ *   - results are those of wpcd_diag_batched (same grid, same kernels); all other arguments as there. */
+#define WPCD_STATIC_WORK_BYTES (16u << 20)
+int wpcd_diag_batched_static(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                             double tol, int max_sweeps, const int* h_rows, int n_ranges, void* stream);
+
 /* Steps (iii)-(v).  For every matrix b and energy e: FWP bin i(e) with Eedge_i <= E_e < Eedge_{i+1}, then
  *   uncoupled: T_ii(E) = V_ii + sum_b (VC)_ib^2/(E - eps_b) + sum_k (VC)_ik^2 g_k(E)
  *   coupled  : T^{ab}(E) = V_{(a i)(b i)} + sum_k (VC)_{(a i)k} g_k(E) (VC)_{(b i)k},  a,b in {0,1}

@@ -143,6 +143,20 @@ int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double*
                             static_cast<cudaStream_t>(stream));
 }
 
+int wpcd_diag_batched_static(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                             double tol, int max_sweeps, const int* h_rows, int n_ranges, void* stream) {
+  WpcdHandle* h = static_cast<WpcdHandle*>(handle);
+  if (!h || !d_A || !d_W || !d_C || !d_info || batch < 1 || max_sweeps < 1) return WPCD_EINVAL;
+  if (n_ranges < 0 || n_ranges > 4 || (n_ranges > 0 && !h_rows)) return WPCD_EINVAL;
+  for (int r = 0; r < n_ranges; ++r)
+    if (h_rows[2 * r] < 0 || h_rows[2 * r + 1] > n || h_rows[2 * r] >= h_rows[2 * r + 1]) return WPCD_EINVAL;
+  if (n < 2 || n > 4096) return WPCD_ESIZE;
+  if (!aligned16(d_A) || !aligned16(d_C)) return WPCD_EINVAL;
+  if (!on_handle_device(h)) return WPCD_EINVAL;
+  return wpcd_jacobi_static_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, h_rows, n_ranges,
+                                   static_cast<cudaStream_t>(stream));
+}
+
 int wpcd_onshell_T(void* handle, int N, int coupled, int batch, const double* d_e0, const double* d_Eedge,
                    const double* d_H, const double* d_W, const double* d_C, const double* d_Ecm, int nE, int mode,
                    double* d_T, int* d_bin, void* d_work, size_t work_bytes, void* stream) {

@@ -25,6 +25,8 @@
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
 #include <math.h>
+#include <cstdio>
+#include <mutex>
 #include <type_traits>
 #include "jacobi_rotation.cuh"
 #include "jacobi_schedule.cuh"
@@ -838,6 +840,46 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   }
   if (rc) return rc;
   return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch");
+}
+
+// ------------------------------------------------------------------------- wpcd_diag_batched_static (include/wpcd.h)
+// The workspace of the launch above -- schedule tables, work counter, per-CTA eigenvector blocks -- in a file-scope
+// device array, for callers that must not allocate.  Every device that loads the library holds the array until exit.
+// In host code the NAME of the array is a host-side stand-in, not a device address: the address the kernels get is
+// looked up with cudaGetSymbolAddress, once per device, with that device current (the entry point has checked that the
+// current device is the handle's).  All calls on a device share the array: overlapping calls race (see the header).
+static __device__ __align__(256) unsigned char wpcd_static_work[WPCD_STATIC_WORK_BYTES];
+
+namespace {
+constexpr int kMaxStaticDevices = 64;
+std::mutex s_static_mutex;
+void* s_static_ptr[kMaxStaticDevices];  // device address of wpcd_static_work per CUDA ordinal, nullptr = not looked up yet
+}  // namespace
+
+int wpcd_jacobi_static_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                              double tol, int max_sweeps, const int* h_rows, int n_ranges, cudaStream_t st) {
+  if (h->device < 0 || h->device >= kMaxStaticDevices) return WPCD_EINVAL;
+  const size_t need = wpcd_jacobi_workspace(h, n, batch);
+  if (need > (size_t)WPCD_STATIC_WORK_BYTES) {
+    snprintf(h->cuda_err, sizeof(h->cuda_err),
+             "wpcd_diag_batched_static: n = %d, batch = %d needs %zu bytes of workspace, the static array holds %zu "
+             "(use wpcd_diag_batched with a caller-allocated workspace)",
+             n, batch, need, (size_t)WPCD_STATIC_WORK_BYTES);
+    return WPCD_ESIZE;
+  }
+  void* ptr = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(s_static_mutex);
+    ptr = s_static_ptr[h->device];
+    if (!ptr) {
+      if (int rc = wpcd_check_cuda(h, cudaGetSymbolAddress(&ptr, wpcd_static_work), "cudaGetSymbolAddress(wpcd_static_work)")) return rc;
+      if (!ptr) return WPCD_ECUDA;
+      s_static_ptr[h->device] = ptr;
+    }
+  }
+  // nothing to clear: k_schedule / k_small_counter rewrite the tables and the counter, the CTAs initialise their V blocks
+  return wpcd_jacobi_launch(h, n, batch, d_A, d_W, d_C, d_info, tol, max_sweeps, h_rows, n_ranges, ptr,
+                            (size_t)WPCD_STATIC_WORK_BYTES, st);
 }
 
 // Test hooks (host only): the block tournament of jacobi_schedule.cuh, see include/wpcd.h.

@@ -22,6 +22,9 @@ size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch);
 int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                        double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
                        cudaStream_t st);
+// wpcd_diag_batched_static: the same launch with the workspace in jacobi.cu's file-scope device array
+int wpcd_jacobi_static_launch(WpcdHandle* h, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
+                              double tol, int max_sweeps, const int* h_rows, int n_ranges, cudaStream_t st);
 // jacobi_small.cu (n <= WPCD_SMALL_N_MAX)
 #define WPCD_SMALL_N_MAX 32
 size_t wpcd_jacobi_small_workspace();

@@ -52,6 +52,8 @@ _lib.wpcd_build_channels.argtypes = [_vp, C.POINTER(Grid), C.POINTER(Potential),
 _lib.wpcd_build_channels.restype = _i
 _lib.wpcd_diag_batched.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _d, _i, C.POINTER(_i), _i, _vp, _sz, _vp]
 _lib.wpcd_diag_batched.restype = _i
+_lib.wpcd_diag_batched_static.argtypes = [_vp, _i, _i, _vp, _vp, _vp, _vp, _d, _i, C.POINTER(_i), _i, _vp]
+_lib.wpcd_diag_batched_static.restype = _i
 _lib.wpcd_onshell_T.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp, _vp, _vp, _sz, _vp]
 _lib.wpcd_onshell_T.restype = _i
 _lib.wpcd_phase_shifts.argtypes = [_vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -73,7 +75,7 @@ _lib.wpcd_probe_fp64.argtypes = [_vp, _i, _i, _vp, C.POINTER(_d), _vp]; _lib.wpc
 # every symbol include/wpcd.h declares (tests/test_abi_cpu.py compares this list with the header and the library)
 EXPORTS = ["wpcd_create", "wpcd_destroy", "wpcd_strerror", "wpcd_last_cuda_error", "wpcd_num_sms",
            "wpcd_build_workspace_bytes", "wpcd_diag_workspace_bytes", "wpcd_onshell_workspace_bytes",
-           "wpcd_build_channels", "wpcd_diag_batched", "wpcd_onshell_T", "wpcd_phase_shifts", "wpcd_onshell_rows",
+           "wpcd_build_channels", "wpcd_diag_batched", "wpcd_diag_batched_static", "wpcd_onshell_T", "wpcd_phase_shifts", "wpcd_onshell_rows",
            "wpcd_interp_phases", "wpcd_sigma_tot", "wpcd_mi_workspace_bytes", "wpcd_mi_solve",
            "wpcd_probe_sink_elems", "wpcd_probe_fp64", "wpcd_jacobi_schedule", "wpcd_jacobi_critical_slot"]
 
@@ -226,6 +228,20 @@ class Handle:
         rc = _lib.wpcd_diag_batched(self._h, n, batch, _ptr(A), _ptr(W), _ptr(Cm), _ptr(info), float(tol), int(max_sweeps),
                                     h_rows, nr, _ptr(work), work.numel(), _stream(stream, self.device))
         self._check(rc, "wpcd_diag_batched")
+        return W, Cm, info
+
+    STATIC_WORK_BYTES = 16 << 20   # WPCD_STATIC_WORK_BYTES of include/wpcd.h
+
+    def diag_batched_static(self, A, W, Cm, info, tol=0.0, max_sweeps=30, stream=None, rows=None):
+        """wpcd_diag_batched_static: diag_batched with the workspace in the library's static device array -- the call
+        allocates nothing, so the outputs W [batch][n], Cm [batch][n][n], info [batch] (int32) are the caller's.  Sizes with
+        diag_workspace_bytes(n, batch) > STATIC_WORK_BYTES raise WpcdError; calls that overlap on the GPU race."""
+        batch, n = A.shape[0], A.shape[-1]
+        nr = 0 if rows is None else len(rows)
+        h_rows = (_i * (2 * nr))(*[int(x) for r in rows for x in r]) if nr else None
+        rc = _lib.wpcd_diag_batched_static(self._h, n, batch, _ptr(A), _ptr(W), _ptr(Cm), _ptr(info), float(tol),
+                                           int(max_sweeps), h_rows, nr, _stream(stream, self.device))
+        self._check(rc, "wpcd_diag_batched_static")
         return W, Cm, info
 
     # ------------------------------------------------------------------ wpcd_onshell_T
