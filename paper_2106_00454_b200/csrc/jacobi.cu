@@ -26,6 +26,7 @@
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
 #include <math.h>
 #include <cstdio>
+#include <cstdlib>
 #include <mutex>
 #include <type_traits>
 #include "jacobi_rotation.cuh"
@@ -104,6 +105,10 @@ struct Smem {
   int* act;      // [nb] active row blocks of V (those that hold wanted rows of C)
   int* perm;     // [np] internal row/column i holds original index perm[i] & 0xFFFF; bit 16: row i of C is wanted
   const int* tab; // slot and feed tables [2][m-1][nslots]: shared-memory copy (modes 0, 1) or k_schedule's global ones
+  // log mode: the log region of the matrix being solved (ctr[4] = entries so far, ctr[5] = overflow)
+  double* logq;   // [log_cap][256] rotation products in the layout of a slot's Q
+  int* logtag;    // [log_cap] I | J << 16
+  int logcap;
 };
 
 // ---------------------------------------------------------------------------------------------- pivot solve
@@ -365,7 +370,7 @@ __device__ __forceinline__ size_t vidx(int nb, int r, int c) {
 // Items of 4 row blocks (half the queue traffic and Q loads of items of 2: n=200 6 % faster; with A's upper-block layout
 // in the workspace modes too: n=300 3 % faster, together with the interleaved queue order 11 %; items of 8: slower).
 
-template <int nbk>
+template <int nbk, bool kQcg = false>
 __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, const double* __restrict__ Q, int I, int J,
                                              const int* __restrict__ rb, int nrb, int lane, bool kStream) {
   const int g = lane >> 2, t = lane & 3;
@@ -374,7 +379,10 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, con
 #pragma unroll
   for (int c = 0; c < nbk; ++c)
 #pragma unroll
-    for (int r = 0; r < 2; ++r) bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
+    for (int r = 0; r < 2; ++r) {
+      if (kQcg) bq[c][r] = __ldcg(reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g)));  // written by another CTA: L2 only
+      else bq[c][r] = *reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g));
+    }
 #pragma unroll 1
   for (int k = 0; k < nrb; k += 2) {
     const bool two = k + 1 < nrb;
@@ -430,7 +438,27 @@ struct JacobiParams {
   int stream_v;    // workspace modes: 1 = V accesses carry the evict-first hint (see wpcd_jacobi_launch)
   int full_every;  // a full 16x16 pivot sweep every full_every-th step of the tournament, cross-only sweeps between
   double tol;
+  // fallback launches (matrices whose log overflowed): the matrices are list[0 .. *nlist) instead of 0 .. batch-1
+  const int* list;
+  const int* nlist;
+  // log mode (kMode 4, see k_jacobi): scheduler block, log regions (two per CTA) and their geometry
+  int* sched;
+  char* logbase;
+  size_t region_bytes;
+  int log_cap, log_steps;  // capacity of a region in entries (rotating slots) and in tournament steps
+  int rbp, npanels;        // row blocks of C per replay unit, replay units per matrix
+  int ready_off, fb_off;   // offsets (ints) of the ready list and of the fallback list inside the scheduler block
 };
+
+// Scheduler block of the log mode (ints): [0] next matrix, [1] matrices published for replay, [2] replay units claimed,
+// [3] replay units done, [4] matrices solved (published or sent to the fallback list), [5] length of the fallback list,
+// [6] watchdog flag, [kSchedDone + r] replay units done of log region r; then the ready list (region of the k-th published
+// matrix, -1 = not written yet) and the fallback list.
+constexpr int kSchedDone = 16;
+__global__ void k_sched_init(int* __restrict__ sched, int nzero, int nneg) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nzero + nneg; i += gridDim.x * blockDim.x) sched[i] = i < nzero ? 0 : -1;
+}
+__global__ void k_set_counter(int* p, int v) { *p = v; }
 
 
 // Schedule tables (one copy per launch, read through the L1): the tournament needs integer divisions that would
@@ -506,10 +534,94 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
     // so every pair is still met in every sweep); always for small matrices, where padding leaves few real pivots
     const bool full = (tn % P.full_every) == 0 || P.nb < 6;  // nb >= 6: every block sits in >= 1 full real pivot per sweep
     rotated = inner_solve(A, Qn, I, J, P.tol, full, lane);
+    if (kMode == 4 && rotated) {  // log mode: the eigenvectors are accumulated later, by a replay of these products
+      int idx = 0;
+      if (lane == 0) idx = atomicAdd(&sm.ctr[4], 1);
+      idx = __shfl_sync(0xffffffffu, idx, 0);
+      __syncwarp();
+      if (idx < sm.logcap) {
+        double2* dst = reinterpret_cast<double2*>(sm.logq + (size_t)idx * kQSlot);
+        const double2* src = reinterpret_cast<const double2*>(Qn);
+#pragma unroll
+        for (int u = 0; u < kQSlot / 64; ++u) dst[lane + 32 * u] = src[lane + 32 * u];
+        if (lane == 0) sm.logtag[idx] = (I & 0xFFFF) | ((J & 0xFFFF) << 16);
+      } else if (lane == 0) {
+        sm.ctr[5] = 1;
+      }
+    }
   }
   if (lane == 0) {
     sm.rot[bn * nslots + sn] = rotated ? 1 : 0;
     if (rotated) atomicAdd(&sm.ctr[2 + parity], 1);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- log mode
+// Layout of a log region (ints, then the products): [0] entries, [1] steps, [2] overflow, [3] matrix, [8 ..) perm[np],
+// src[np], step_start[log_steps + 2], tags[log_cap]; the products [log_cap][256] doubles follow, 256-byte aligned.
+__host__ __device__ inline int log_perm_off() { return 8; }
+__host__ __device__ inline int log_src_off(int np) { return 8 + np; }
+__host__ __device__ inline int log_step_off(int np) { return 8 + 2 * np; }
+__host__ __device__ inline int log_tag_off(int np, int steps) { return 8 + 2 * np + steps + 2; }
+__host__ __device__ inline size_t log_q_off(int np, int steps, int cap) {
+  return (((size_t)(log_tag_off(np, steps) + cap) * 4) + 255) & ~(size_t)255;
+}
+constexpr int kJobWait = 0, kJobSolve = 1, kJobReplay = 2, kJobExit = 3;
+
+// Replay unit: rows [8 rbp panel, 8 rbp (panel + 1)) (internal order) of the eigenvector matrix of the matrix logged in
+// `region`.  The panel starts as rows of the identity in shared memory (blocked like V: vidx with local row blocks), takes
+// V <- V Q for every logged product in order -- the products of one tournament step touch disjoint column blocks, so the
+// warps share them out and meet at one barrier per step -- and is written to its rows of C.  Same arithmetic, in the
+// same order, as the V items of the workspace modes (apply_V_item), but V never leaves the SM and the products are read
+// once per panel from L2: the DRAM traffic of the large-n path drops from ~200x to ~10x the algorithmic bytes.
+template <int kThreads>
+__device__ __forceinline__ void replay_panel(const JacobiParams& P, int region, int panel, double* Vp) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n = P.n, np = P.np, nb = P.nb;
+  const int* hdr = reinterpret_cast<const int*>(P.logbase + (size_t)region * P.region_bytes);
+  const int* perm = hdr + log_perm_off();
+  const int* src = hdr + log_src_off(np);
+  const int* step_start = hdr + log_step_off(np);
+  const int* tags = hdr + log_tag_off(np, P.log_steps);
+  const double* logq = reinterpret_cast<const double*>(reinterpret_cast<const char*>(hdr) + log_q_off(np, P.log_steps, P.log_cap));
+  const int nsteps = __ldcg(hdr + 1), mat = __ldcg(hdr + 3);
+  const int rb0 = panel * P.rbp;
+  const int nrbp = nb - rb0 < P.rbp ? nb - rb0 : P.rbp;
+  int* srcs = reinterpret_cast<int*>(Vp + (size_t)P.rbp * nb * 64);  // [np] sort permutation, [rbp] local row blocks
+  int* rbl = srcs + np;
+  for (int e = tid; e < nrbp * nb * 64; e += kThreads) {
+    const int blk = e >> 6, r = (e >> 3) & 7, c = e & 7;
+    const int lr = blk / nb, cb = blk - lr * nb;
+    Vp[e] = (8 * (rb0 + lr) + r == 8 * cb + c) ? 1.0 : 0.0;
+  }
+  for (int k = tid; k < n; k += kThreads) srcs[k] = __ldcg(src + k);
+  if (tid < P.rbp) rbl[tid] = tid;
+  __syncthreads();
+  const int nper = (nrbp + 1) >> 1;  // items of two row blocks
+  for (int gs = 0; gs < nsteps; ++gs) {
+    const int e0 = __ldcg(step_start + gs), e1 = __ldcg(step_start + gs + 1);
+    if (e1 <= e0) continue;
+    for (int itm = warp; itm < (e1 - e0) * nper; itm += kThreads / 32) {
+      const int e = e0 + itm / nper, pr = itm - (itm / nper) * nper;
+      const int tag = __ldcg(tags + e);
+      const int I = tag & 0xFFFF, J = (tag >> 16) == 0xFFFF ? -1 : (tag >> 16);
+      const int nrb = nrbp - 2 * pr < 2 ? nrbp - 2 * pr : 2;
+      if (J >= 0) apply_V_item<2, true>(Vp, nb, logq + (size_t)e * kQSlot, I, J, rbl + 2 * pr, nrb, lane, false);
+      else apply_V_item<1, true>(Vp, nb, logq + (size_t)e * kQSlot, I, J, rbl + 2 * pr, nrb, lane, false);
+    }
+    __syncthreads();
+  }
+  double* Co = P.C + (size_t)mat * n * n;
+  for (int lr = 0; lr < 8 * nrbp; ++lr) {
+    const int i = 8 * rb0 + lr;
+    if (i >= n) break;
+    const int pi = __ldcg(perm + i);
+    double* row = Co + (size_t)(pi & 0xFFFF) * n;
+    const double* vrow = Vp + ((size_t)((lr >> 3) * nb) << 6) + ((lr & 7) << 3);
+    for (int k = tid; k < n; k += kThreads) {
+      const int c = srcs[k];
+      row[k] = (pi >> 16) ? vrow[((size_t)(c >> 3) << 6) + (c & 7)] : 0.0;
+    }
   }
 }
 
@@ -536,6 +648,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     if (kMode == 1) {
       sm.A = d; d += (size_t)(nb * (nb + 1) / 2) * 64;
       sm.V = g; g += (size_t)np * np;
+    } else if (kMode == 4) {
+      sm.A = g; g += (size_t)(nb * (nb + 1) / 2) * 64;
+      sm.V = nullptr;
     } else {
       sm.A = g; g += (size_t)(nb * (nb + 1) / 2) * 64;
       sm.V = g; g += (size_t)np * np;
@@ -546,7 +661,7 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     int* ip = reinterpret_cast<int*>(d);
     sm.rot = ip; ip += 2 * nslots;
     sm.src = ip; ip += np;
-    sm.ctr = ip; ip += 4;
+    sm.ctr = ip; ip += 8;
     sm.act = ip; ip += 2 * nb;  // list of active row blocks, then a flag per row block
     sm.perm = ip; ip += np;
     if (kMode == 1) {  // small tables: keep the slot and feed tables of all steps in shared memory
@@ -567,7 +682,80 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
   // matrices are handed out dynamically (they need 6-8 sweeps each): the first one is the CTA's own index, the next ones
   // come from a global counter that k_schedule set to gridDim.x
   __shared__ int s_next;
-  for (int mat = blockIdx.x; mat < P.batch;) {
+  __shared__ int s_job[4];
+  const int nmat = (kMode != 4 && P.nlist) ? *P.nlist : P.batch;
+  bool busy0 = false, busy1 = false;  // log mode, thread 0: own log regions that wait for their replay
+  int waits = 0;
+  for (int it = blockIdx.x;;) {
+    int mat, region = 0;
+    if (kMode == 4) {
+      // Log mode: one persistent loop over three kinds of work, decided by thread 0.  (a) A replay unit (a panel of rows
+      // of the eigenvector matrix of a solved matrix, see replay_panel) if one is published and unclaimed -- first, so
+      // that the log regions drain; (b) else the next matrix, if one of this CTA's two log regions is free; (c) else wait.
+      __syncthreads();
+      if (tid == 0) {
+        volatile int* sc = P.sched;
+        int kind = kJobWait, a = 0, b = 0;
+        int c = sc[2];
+        for (;;) {
+          const int pub = sc[1];
+          if (c >= pub * P.npanels) break;
+          const int old = atomicCAS(P.sched + 2, c, c + 1);
+          if (old == c) { kind = kJobReplay; a = c / P.npanels; b = c - a * P.npanels; break; }
+          c = old;
+        }
+        if (kind == kJobReplay) {  // the publisher's ticket may precede its list entry by a few cycles
+          volatile int* rl = P.sched + P.ready_off;
+          int spins = 0, r;
+          while ((r = rl[a]) < 0 && ++spins < (1 << 24)) __nanosleep(64);
+          if (r < 0) { P.sched[6] = 1; kind = kJobExit; }
+          a = r;
+        } else {
+          int* done = P.sched + kSchedDone + 2 * blockIdx.x;
+          if (busy0 && sc[kSchedDone + 2 * blockIdx.x] >= P.npanels) { done[0] = 0; busy0 = false; }
+          if (busy1 && sc[kSchedDone + 2 * blockIdx.x + 1] >= P.npanels) { done[1] = 0; busy1 = false; }
+          if (!(busy0 && busy1) && sc[0] < P.batch) {
+            const int mnew = atomicAdd(P.sched, 1);
+            if (mnew < P.batch) {
+              kind = kJobSolve; a = mnew; b = busy0 ? 1 : 0;
+              if (b) busy1 = true; else busy0 = true;
+            }
+          }
+          if (kind == kJobWait && sc[0] >= P.batch && sc[4] >= P.batch) {
+            __threadfence();
+            if (sc[3] >= sc[1] * P.npanels) kind = kJobExit;
+          }
+          if (kind == kJobWait && ++waits > (1 << 23)) { P.sched[6] = 1; kind = kJobExit; }  // watchdog: never hang the GPU
+        }
+        if (kind != kJobWait) waits = 0;
+        s_job[0] = kind; s_job[1] = a; s_job[2] = b;
+      }
+      __syncthreads();
+      const int kind = s_job[0];
+      if (kind == kJobExit) break;
+      if (kind == kJobWait) { __nanosleep(256); continue; }
+      if (kind == kJobReplay) {
+        replay_panel<kThreads>(P, s_job[1], s_job[2], reinterpret_cast<double*>(smem_raw));
+        __syncthreads();
+        if (tid == 0) {  // all reads of the region and all writes of C are done
+          __threadfence();
+          atomicAdd(P.sched + kSchedDone + s_job[1], 1);
+          atomicAdd(P.sched + 3, 1);
+        }
+        continue;
+      }
+      mat = s_job[1];
+      region = 2 * blockIdx.x + s_job[2];
+    } else {
+      if (it >= nmat) break;
+      mat = P.list ? P.list[it] : it;
+    }
+    int* const lhdr = kMode == 4 ? reinterpret_cast<int*>(P.logbase + (size_t)region * P.region_bytes) : nullptr;
+    if (kMode == 4) {
+      sm.logtag = lhdr + log_tag_off(np, P.log_steps);
+      sm.logq = reinterpret_cast<double*>(reinterpret_cast<char*>(lhdr) + log_q_off(np, P.log_steps, P.log_cap));
+      sm.logcap = P.log_cap;
+    }
     const double* H = P.H + (size_t)mat * n * n;
     __syncthreads();
 #ifdef WPCD_PROFILE
@@ -609,16 +797,16 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     __syncthreads();
     const int nact = sm.ctr[0];
     const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
-    const int nitems = ntiles + nslots * nvgrp;
+    const int nitems = kMode == 4 ? ntiles : ntiles + nslots * nvgrp;  // log mode: no eigenvector items
     const float rnvgrp = 1.0f / (float)(nvgrp > 0 ? nvgrp : 1);
     __syncthreads();
     for (int e = tid; e < np * np; e += kThreads) {
       int r = e / np, c = e - r * np;
       double a = (r < n && c < n) ? H[(size_t)(sm.perm[r] & 0xFFFF) * n + (sm.perm[c] & 0xFFFF)] : 0.0;
       Av.put(r, c, a);
-      sm.V[vidx(nb, r, c)] = (r == c) ? 1.0 : 0.0;
+      if (kMode != 4) sm.V[vidx(nb, r, c)] = (r == c) ? 1.0 : 0.0;
     }
-    if (tid < 4) sm.ctr[tid] = 0;
+    if (tid < 8) sm.ctr[tid] = 0;
     __syncthreads();
 #ifdef WPCD_PROFILE
     if (blockIdx.x == 0 && tid == 0) WPCD_PROF_ADD(6, clock64() - tm0);
@@ -629,6 +817,9 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     __syncthreads();
     int sweeps = 0, buf = 0, gstep = 0;
     bool converged = false;
+    // log mode: entries [step_start[k], step_start[k+1]) are the products applied at global step k; nprep steps prepared
+    int nprep = 1;
+    if (kMode == 4 && tid == 0) { lhdr[log_step_off(np)] = 0; lhdr[log_step_off(np) + 1] = sm.ctr[4]; }
     for (;;) {
       const int par = sweeps & 1;
       for (int step = 0; step < m - 1; ++step, ++gstep) {
@@ -696,6 +887,13 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
 #ifdef WPCD_PROFILE
         if (blockIdx.x == 0 && tid == 0) { WPCD_PROF_ADD(0, clock64() - tk0); WPCD_PROF_ADD(2, 1); }
 #endif
+        if (kMode == 4 && do_next) {
+          nprep = gstep + 2;
+          if (tid == 0) {
+            if (nprep <= P.log_steps) lhdr[log_step_off(np) + nprep] = sm.ctr[4];
+            else sm.ctr[5] = 1;
+          }
+        }
         buf ^= 1;
       }
       ++sweeps;
@@ -721,21 +919,46 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     double* Wo = P.W + (size_t)mat * n;
     double* Co = P.C + (size_t)mat * n * n;
     for (int k = tid; k < n; k += kThreads) Wo[k] = sm.wsort[sm.src[k]];
-    for (int e = tid; e < n * n; e += kThreads) {  // internal row i goes back to row perm[i]; unwanted rows: zeros
-      int i = e / n, k = e - i * n;
-      int c = sm.src[k];
-      const int pi = sm.perm[i];
-      Co[(size_t)(pi & 0xFFFF) * n + k] = (pi >> 16) ? sm.V[vidx(nb, i, c)] : 0.0;
-    }
-    if (tid == 0) {
-      P.info[mat] = converged ? sweeps : -1;
-      s_next = atomicAdd(P.next, 1);
+    if (kMode != 4) {
+      for (int e = tid; e < n * n; e += kThreads) {  // internal row i goes back to row perm[i]; unwanted rows: zeros
+        int i = e / n, k = e - i * n;
+        int c = sm.src[k];
+        const int pi = sm.perm[i];
+        Co[(size_t)(pi & 0xFFFF) * n + k] = (pi >> 16) ? sm.V[vidx(nb, i, c)] : 0.0;
+      }
+      if (tid == 0) {
+        P.info[mat] = converged ? sweeps : -1;
+        s_next = atomicAdd(P.next, 1);
+      }
+    } else {
+      // log mode: what the replay needs besides the products -- the ordering, the sort, the step table -- then publish
+      for (int k = tid; k < np; k += kThreads) {
+        lhdr[log_perm_off() + k] = sm.perm[k];
+        lhdr[log_src_off(np) + k] = k < n ? sm.src[k] : 0;
+      }
+      __threadfence();  // every thread's log and header writes, before thread 0 publishes the region
+      __syncthreads();
+      if (tid == 0) {
+        const bool ovf = sm.ctr[5] != 0 || sm.ctr[4] > P.log_cap;
+        P.info[mat] = converged ? sweeps : -1;
+        lhdr[0] = sm.ctr[4]; lhdr[1] = nprep; lhdr[2] = ovf ? 1 : 0; lhdr[3] = mat;
+        __threadfence();
+        if (!ovf) {
+          const int ticket = atomicAdd(P.sched + 1, 1);
+          P.sched[P.ready_off + ticket] = region;
+        } else {  // too many rotations for the log region: the matrix is redone by the fallback launch (workspace mode)
+          P.sched[P.fb_off + atomicAdd(P.sched + 5, 1)] = mat;
+          if (region & 1) busy1 = false; else busy0 = false;
+        }
+        __threadfence();
+        atomicAdd(P.sched + 4, 1);
+      }
     }
     __syncthreads();
 #ifdef WPCD_PROFILE
     if (blockIdx.x == 0 && tid == 0) { WPCD_PROF_ADD(5, clock64() - tm0); WPCD_PROF_ADD(7, clock64() - tm1); }
 #endif
-    mat = s_next;
+    it = s_next;
   }
 }
 
@@ -757,7 +980,7 @@ Geometry geometry(const WpcdHandle* h, int n) {
   if (g.m < 6) g.m = 6;  // the pipeline needs >= 3 slots (distinct critical tiles)
   g.nslots = g.m / 2;
   g.tab_bytes = ((((size_t)(g.m - 1) * (2 * g.nslots + g.nslots * (g.nslots - 1) / 2) * 4) + 255) & ~(size_t)255) + 256;  // + counter
-  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + 2 * g.np + 4 + 2 * g.nb) * 4 + 64;
+  const size_t misc = (size_t)g.np * 8 + (size_t)(2 * g.nslots + 2 * g.np + 8 + 2 * g.nb) * 4 + 64;
   const size_t tabs = (size_t)2 * (g.m - 1) * g.nslots * 4;  // shared-memory copy of the slot and feed tables (modes 0, 1)
   const size_t q = (size_t)2 * g.nslots * kQSlot * 8;
   const size_t a_half = (size_t)(g.nb * (g.nb + 1) / 2) * 512, v = (size_t)g.np * g.np * 8;
@@ -789,11 +1012,56 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
   return WPCD_OK;
 }
 
+// Log mode (k_jacobi<4>): used where the workspace mode 2 would run (A does not fit shared memory, Q does: 200 < n <~ 880).
+// Capacity of a log region: kLogSweeps sweeps' worth of rotating slots (measured need: 5-6; more goes to the fallback
+// launch) and 16 sweeps' worth of steps.  WPCD_JACOBI_LOG_SWEEPS in the environment overrides kLogSweeps (a test hook:
+// 0 disables the log mode, 1 forces matrices into the fallback launch).
+constexpr int kLogSweeps = 7;
+struct LogGeometry {
+  bool use;
+  int grid, cap, steps, rbp, npanels, ready_off, fb_off;
+  size_t region_bytes, smem, sched_bytes, a_bytes, off_sched, off_a, off_log, off_fb, total;
+};
+
+LogGeometry log_geometry(const WpcdHandle* h, const Geometry& g, int batch) {
+  LogGeometry L{};
+  int sweeps = kLogSweeps;
+  if (const char* e = getenv("WPCD_JACOBI_LOG_SWEEPS")) sweeps = atoi(e);
+  const size_t cap_smem = (size_t)h->max_smem_optin;
+  const size_t per_rb = (size_t)g.nb * 512;
+  size_t avail = cap_smem > 2048 + 4 * (size_t)g.np ? cap_smem - 2048 - 4 * (size_t)g.np : 0;
+  int rbp = (int)(avail / per_rb);
+  if (rbp > 8) rbp = 8;
+  if (rbp > 2) rbp &= ~1;
+  L.use = g.mode == 2 && sweeps > 0 && rbp >= 1;
+  if (!L.use) return L;
+  L.grid = batch < h->num_sms ? batch : h->num_sms;
+  L.cap = sweeps * (g.m - 1) * g.nslots;
+  L.steps = 16 * (g.m - 1);
+  L.rbp = rbp;
+  L.npanels = (g.nb + rbp - 1) / rbp;
+  L.region_bytes = (log_q_off(g.np, L.steps, L.cap) + (size_t)L.cap * kQSlot * 8 + 255) & ~(size_t)255;
+  const size_t smem_b = (size_t)rbp * per_rb + 4 * (size_t)(g.np + 8);
+  L.smem = g.smem > smem_b ? g.smem : smem_b;
+  L.ready_off = kSchedDone + 2 * L.grid;
+  L.fb_off = L.ready_off + batch;
+  L.sched_bytes = (((size_t)(L.fb_off + batch) * 4) + 255) & ~(size_t)255;
+  L.a_bytes = (size_t)(g.nb * (g.nb + 1) / 2) * 512;
+  L.off_sched = g.tab_bytes;
+  L.off_a = L.off_sched + L.sched_bytes;
+  L.off_log = L.off_a + (size_t)L.grid * L.a_bytes;
+  L.off_fb = L.off_log + (size_t)2 * L.grid * L.region_bytes;
+  L.total = L.off_fb + 256 + (size_t)L.grid * g.gstride * 8;  // fallback: its own counter and mode-2 workspaces
+  return L;
+}
+
 }  // namespace
 
 size_t wpcd_jacobi_workspace(const WpcdHandle* h, int n, int batch) {
   if (n <= WPCD_SMALL_N_MAX) return wpcd_jacobi_small_workspace();
   Geometry g = geometry(h, n);
+  const LogGeometry L = log_geometry(h, g, batch);
+  if (L.use) return L.total;
   return g.tab_bytes + (size_t)global_grid(h, g, batch) * g.gstride * 8;
 }
 
@@ -819,6 +1087,40 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   if (g.mode == 1) P.full_every = (g.m - 1 + 2) / 3 > 5 ? (g.m - 1 + 2) / 3 : 5;
   else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
+  P.list = nullptr; P.nlist = nullptr; P.sched = nullptr; P.logbase = nullptr;
+  P.region_bytes = 0; P.log_cap = P.log_steps = P.rbp = P.npanels = P.ready_off = P.fb_off = 0;
+  const LogGeometry L = log_geometry(h, g, batch);
+  if (L.use) {
+    // Log mode: one persistent launch solves the matrices without their eigenvectors (A through L2, as in mode 2),
+    // logs the rotation products and replays them panel by panel into C (k_jacobi<4>, replay_panel); a second launch
+    // of the workspace mode redoes the matrices whose log overflowed (normally none: its CTAs exit at once).
+    if (work_bytes < L.total) return WPCD_EWORK;
+    char* w = static_cast<char*>(d_work);
+    P.next = reinterpret_cast<int*>(w + g.tab_bytes - 256);
+    k_schedule<<<g.m - 1, 128, 0, st>>>(g.m, g.nb, static_cast<int*>(d_work), P.next, L.grid);
+    JacobiParams P4 = P;
+    P4.sched = reinterpret_cast<int*>(w + L.off_sched);
+    P4.gwork = reinterpret_cast<double*>(w + L.off_a);
+    P4.gstride = L.a_bytes / 8;
+    P4.logbase = w + L.off_log;
+    P4.region_bytes = L.region_bytes;
+    P4.log_cap = L.cap; P4.log_steps = L.steps; P4.rbp = L.rbp; P4.npanels = L.npanels;
+    P4.ready_off = L.ready_off; P4.fb_off = L.fb_off;
+    P4.stream_v = 0;
+    k_sched_init<<<64, 256, 0, st>>>(P4.sched, L.ready_off, 2 * batch);
+    int rc = launch_mode<4, 640>(h, P4, L.grid, L.smem, st);
+    if (rc) return rc;
+    JacobiParams P2 = P;
+    P2.list = P4.sched + L.fb_off;
+    P2.nlist = P4.sched + 5;
+    P2.next = reinterpret_cast<int*>(w + L.off_fb);
+    P2.gwork = reinterpret_cast<double*>(w + L.off_fb + 256);
+    P2.stream_v = (size_t)L.grid * L.a_bytes <= ((size_t)96 << 20);
+    k_set_counter<<<1, 1, 0, st>>>(P2.next, L.grid);
+    rc = launch_mode<2, 640>(h, P2, L.grid, g.smem, st);
+    if (rc) return rc;
+    return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch (log mode)");
+  }
   const int grid = global_grid(h, g, batch);
   // Workspace modes: while the A blocks of all CTAs together fit L2 (n <= ~390 with 148 CTAs) V is streamed through it
   // with the evict-first hint and A stays resident: a third less DRAM traffic (n=300: 320 -> 280 ms per 4096 matrices;

@@ -742,6 +742,47 @@ def test_large_n_batch_exceeds_grid(ctx, N, S, picks):
         _compare_channel(res, 1, Sc - 1, 0, N, 1, Ecm, scale=tuple(scales[Sc - 1]), label=f"batch>grid N={N} coupled s={Sc - 1}")
 
 
+def test_log_mode_fallback_and_workspace_mode_are_bit_identical(ctx):
+    """The three ways the large-n eigensolver can run give the same bits: the log mode (k_jacobi<4>: solve without
+    eigenvectors, log the rotation products, replay them panel by panel into C), its fallback (a log region too small for
+    the matrix: the matrix is redone by the workspace kernel) and the workspace mode alone.  Same rotations, same products,
+    same order of the DMMA accumulations per column of C -- so W, C and info must agree exactly, with and without row
+    ranges (rows outside the ranges: zeros).  WPCD_JACOBI_LOG_SWEEPS is the test hook of csrc/jacobi.cu."""
+    import os
+    torch, h = ctx["torch"], ctx["h"]
+    N, S = 150, 40
+    scales = torch.as_tensor(inp.sample_scales(S, seed=11), device=ctx["dev"])
+    out = h.build_channels(inp.grid_edges(N), [(0, 0), (1, 1)], V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V,
+                           muT=inp.TENSOR_MU, VT_scale_idx=2, scales=scales, S=S)
+    H = out["H_cpl"].reshape(-1, 2 * N, 2 * N).contiguous()       # n = 300
+    runs = {}
+    old = os.environ.get("WPCD_JACOBI_LOG_SWEEPS")
+    try:
+        for name, val in (("log", None), ("fallback", "1"), ("workspace", "0")):
+            if val is None:
+                os.environ.pop("WPCD_JACOBI_LOG_SWEEPS", None)
+            else:
+                os.environ["WPCD_JACOBI_LOG_SWEEPS"] = val
+            for rows in (None, [(10, 95), (160, 245)]):
+                W, C, info = h.diag_batched(H, rows=rows)
+                torch.cuda.synchronize()
+                runs[(name, rows is None)] = (W.cpu().numpy(), C.cpu().numpy(), info.cpu().numpy())
+    finally:
+        if old is None:
+            os.environ.pop("WPCD_JACOBI_LOG_SWEEPS", None)
+        else:
+            os.environ["WPCD_JACOBI_LOG_SWEEPS"] = old
+    W0, C0, i0 = runs[("workspace", True)]
+    assert (i0 >= 1).all() and np.abs(np.einsum("bik,bil->bkl", C0[:3], C0[:3]) - np.eye(2 * N)).max() < 1e-12
+    for key, (W, C, info) in runs.items():
+        assert np.array_equal(W, W0) and np.array_equal(info, i0), key
+        if key[1]:
+            assert np.array_equal(C, C0), key
+        else:
+            assert np.array_equal(C[:, 10:95], C0[:, 10:95]) and np.array_equal(C[:, 160:245], C0[:, 160:245]), key
+            assert not C[:, :10].any() and not C[:, 95:160].any() and not C[:, 245:].any(), key
+
+
 def test_pipeline_cuda_graph_replay_and_fp64_probe(ctx):
     """Pipeline.capture(): the pass replayed as a CUDA graph gives bit-identical phase shifts for new inputs written into the
     pipeline's buffers; wpcd_probe_fp64 (the in-run FP64 peak measurement of bench.py) launches and reports its flop count."""
