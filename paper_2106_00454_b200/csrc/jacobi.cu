@@ -20,7 +20,15 @@
 //   * Rows/columns are relabelled in the order of descending diagonal entries (de Rijk): on the graded WPCD Hamiltonians
 //     the sweeps converge faster than in the natural ascending order (n=200: 7.0 -> 6.3 sweeps).
 // n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
-// n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.  Larger n: A and V in the workspace.
+// n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.
+// 200 < n <~ 880 (A does not fit shared memory, the Q buffers do): LOG MODE.  V <- V Q never feeds back into the sweeps, and
+// with A and V both streaming through L2/DRAM every step the launch was DRAM-bound (174 GB per 592 matrices at n = 300).
+// So the sweeps run on A alone (through L2), every rotating slot appends its 16x16 product to a log region, and the same
+// persistent launch later REPLAYS the log: a CTA takes a panel of <= 64 rows of the identity into shared memory, applies
+// the logged products in order (one barrier per tournament step) and writes the rows of C.  Solve jobs and replay units
+// are handed out by a small scheduler in global memory (replay first, so that the two log regions of every CTA drain).
+// Same products in the same order: bit-identical to the accumulation in place; a tenth of the DRAM traffic.
+// Larger n (the Q buffers do not fit either): A, V and Q in the workspace.
 //
 // The rotation arithmetic follows the classical Jacobi method the paper names for this step ("parallel cyclic-order
 // Jacobi"); blocking, tensor-core application, pipelining and the schedule are this library's.
@@ -543,7 +551,7 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
         double2* dst = reinterpret_cast<double2*>(sm.logq + (size_t)idx * kQSlot);
         const double2* src = reinterpret_cast<const double2*>(Qn);
 #pragma unroll
-        for (int u = 0; u < kQSlot / 64; ++u) dst[lane + 32 * u] = src[lane + 32 * u];
+        for (int u = 0; u < kQSlot / 64; ++u) __stcs(dst + lane + 32 * u, src[lane + 32 * u]);  // streaming: A stays in L2
         if (lane == 0) sm.logtag[idx] = (I & 0xFFFF) | ((J & 0xFFFF) << 16);
       } else if (lane == 0) {
         sm.ctr[5] = 1;
@@ -600,6 +608,13 @@ __device__ __forceinline__ void replay_panel(const JacobiParams& P, int region, 
   const int nper = (nrbp + 1) >> 1;  // items of two row blocks
   for (int gs = 0; gs < nsteps; ++gs) {
     const int e0 = __ldcg(step_start + gs), e1 = __ldcg(step_start + gs + 1);
+#ifndef WPCD_NO_REPLAY_PREFETCH
+    if (gs + 1 < nsteps) {  // the next step's products on their way from DRAM to L2 while this step computes
+      const int e2 = __ldcg(step_start + gs + 2);
+      const char* q = reinterpret_cast<const char*>(logq + (size_t)e1 * kQSlot);
+      for (int x = tid; x < (e2 - e1) * (kQSlot * 8 / 128); x += kThreads) asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)x * 128));
+    }
+#endif
     if (e1 <= e0) continue;
     for (int itm = warp; itm < (e1 - e0) * nper; itm += kThreads / 32) {
       const int e = e0 + itm / nper, pr = itm - (itm / nper) * nper;
