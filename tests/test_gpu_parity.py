@@ -758,7 +758,8 @@ def test_log_mode_fallback_and_workspace_mode_are_bit_identical(ctx):
     runs = {}
     old = os.environ.get("WPCD_JACOBI_LOG_SWEEPS")
     try:
-        for name, val in (("log", None), ("fallback", "1"), ("workspace", "0")):
+        # capacities of 5 and 6 sweeps' worth sit at these matrices' need (5-6): some are replayed, the others fall back
+        for name, val in (("log", None), ("fallback", "1"), ("mixed5", "5"), ("mixed6", "6"), ("workspace", "0")):
             if val is None:
                 os.environ.pop("WPCD_JACOBI_LOG_SWEEPS", None)
             else:
@@ -781,6 +782,55 @@ def test_log_mode_fallback_and_workspace_mode_are_bit_identical(ctx):
         else:
             assert np.array_equal(C[:, 10:95], C0[:, 10:95]) and np.array_equal(C[:, 160:245], C0[:, 160:245]), key
             assert not C[:, :10].any() and not C[:, 95:160].any() and not C[:, 245:].any(), key
+
+
+@pytest.mark.parametrize("n,batch,max_sweeps", [(201, 1, 30), (207, 3, 30), (333, 5, 30), (256, 2, 2), (505, 2, 30)])
+def test_log_mode_edge_cases_against_the_oracle_and_the_workspace_mode(ctx, n, batch, max_sweeps):
+    """Log mode at its edges: the smallest size it takes (n = 201), ragged sizes (padding rows in the last panel), batches
+    smaller than the grid (every CTA but a few only replays), a sweep limit that stops before convergence (info = -1, the
+    log is replayed all the same) and a log capacity of three sweeps' worth, where some matrices are replayed and the others
+    go through the fallback launch.  Dense random symmetric matrices (the slowest to converge): invariants against the
+    input and eigenvalues against the CPU oracle's Jacobi on the first matrix; every variant bit-identical to the workspace
+    mode."""
+    import os
+    torch, h = ctx["torch"], ctx["h"]
+    rng = np.random.default_rng(1000 + n)
+    A = rng.standard_normal((batch, n, n)); A = A + A.transpose(0, 2, 1)
+    d_A = _to_dev(ctx, A)
+    old = os.environ.get("WPCD_JACOBI_LOG_SWEEPS")
+    runs = {}
+    try:
+        for name, val in (("log", None), ("mixed", "3"), ("workspace", "0")):
+            if val is None:
+                os.environ.pop("WPCD_JACOBI_LOG_SWEEPS", None)
+            else:
+                os.environ["WPCD_JACOBI_LOG_SWEEPS"] = val
+            W, C, info = h.diag_batched(d_A, max_sweeps=max_sweeps)
+            torch.cuda.synchronize()
+            runs[name] = (W.cpu().numpy(), C.cpu().numpy(), info.cpu().numpy())
+    finally:
+        if old is None:
+            os.environ.pop("WPCD_JACOBI_LOG_SWEEPS", None)
+        else:
+            os.environ["WPCD_JACOBI_LOG_SWEEPS"] = old
+    W0, C0, i0 = runs["workspace"]
+    for name in ("log", "mixed"):
+        W, C, info = runs[name]
+        assert np.array_equal(W, W0) and np.array_equal(C, C0) and np.array_equal(info, i0), name
+    W, C, info = runs["log"]
+    if max_sweeps < 5:
+        assert (info == -1).all()                       # stopped early: still an orthogonal similarity transform
+        for b in range(batch):
+            assert np.abs(C[b].T @ C[b] - np.eye(n)).max() < 1e-12
+        return
+    assert (info >= 1).all()
+    for b in range(batch):
+        nrm = np.abs(A[b]).max()
+        assert np.abs(C[b].T @ C[b] - np.eye(n)).max() < 1e-12
+        assert np.abs(A[b] @ C[b] - C[b] * W[b]).max() < 1e-13 * n * nrm
+    if n <= 340:
+        Wo = hp.o.jacobi(A[0])[0]
+        assert np.abs(W[0] - Wo).max() <= 1e-12 * n * np.abs(A[0]).max()
 
 
 def test_pipeline_cuda_graph_replay_and_fp64_probe(ctx):
