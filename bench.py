@@ -468,14 +468,15 @@ def run_config5_sweep(args):
         with ThreadPoolExecutor(max_workers=cores) as ex:
             res = list(ex.map(mi_one, idx))
         mi_s = time.perf_counter() - w0
-        # ---- the same MI systems on the GPU (wpcd_mi_solve: K-matrix form), where they fit one CTA's shared memory
+        # ---- the same MI systems on the GPU (wpcd_mi_solve: K-matrix form), where one CTA can take them
         mi_gpu = None
         try:
             from paper_2106_00454_b200 import wpcd as _w
             hg = _w.Handle(0)
             dEc = torch.as_tensor(np.ascontiguousarray(Ecm), device="cuda:0")
             sc0 = torch.as_tensor(scales[:1].copy(), device="cuda:0")
-            chans = [(0, 0), (1, 1)] if N <= 81 else [(0, 0)] if N <= 164 else []
+            # one thread per row: both channels up to N_Q = 127 (above 81 with the system in an L2 region), 1S0 alone up to 255
+            chans = [(0, 0), (1, 1)] if N <= 127 else [(0, 0)] if N <= 255 else []
             if chans:
                 for _ in range(2):
                     hg.mi_solve(chans, dEc, NQ=N, scales=sc0, S=1, **pot)
@@ -483,7 +484,7 @@ def run_config5_sweep(args):
                 g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 g0.record(); Sg_u, Sg_c = hg.mi_solve(chans, dEc, NQ=N, scales=sc0, S=1, **pot); g1.record(); torch.cuda.synchronize()
                 Su = Sg_u.cpu().numpy()[0, 0]; Su = Su[..., 0] + 1j * Su[..., 1]
-                mi_gpu = {"channels": "1S0 + 3S1-3D1" if len(chans) == 2 else "1S0 only (coupled system too large for one CTA)",
+                mi_gpu = {"channels": "1S0 + 3S1-3D1" if len(chans) == 2 else "1S0 only (coupled system: more rows than threads of a CTA)",
                           "ms_per_sample_350_energies": g0.elapsed_time(g1),
                           "max_abs_dS_vs_cpu_oracle_1S0": float(np.abs(Su[idx] - np.array([r[0] for r in res])).max())}
             hg.close()

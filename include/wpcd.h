@@ -221,8 +221,9 @@ int wpcd_sigma_tot(void* handle, int S, int nE, int n_unc, const int* h_J_unc, c
  * recommends (Eq. 38): the principal-value part F_r K = V in REAL arithmetic by Gauss elimination with partial
  * pivoting in shared memory, then T_on = K_on (1 + i f p K_on)^-1 and S = 1 - 2 i f p T, f = 2 mu/hbarc^2.  The potential is the same wpcd_potential as for
  * wpcd_build_channels, used in convention A: v_l = sum_t V0_t Q_l(z_t)/(2k'k) (Yamaguchi: lambda_A = (pi/2) lambda).
- *   NQ      : quadrature points; the system (NQ+1, coupled 2(NQ+1), real) must fit one CTA's shared memory:
- *             NQ <= 164 uncoupled, NQ <= 81 coupled, else WPCD_ESIZE
+ *   NQ      : quadrature points; the system has NQ+1 (coupled: 2(NQ+1)) real rows, one thread per row: NQ <= 255
+ *             uncoupled, NQ <= 127 coupled, else WPCD_ESIZE.  Up to NQ = 164 / 81 it lives in one CTA's shared memory,
+ *             above in an L2-resident region of the workspace per CTA (a fixed grid of CTAs loops over the systems)
  *   d_Ecm   : [nE] c.m. energies, MeV (p = sqrt(E_cm/cE))
  *   d_S_unc : [S][n_unc][nE][2]        S-matrix (re,im), list order of the uncoupled channels
  *   d_S_cpl : [S][n_cpl][nE][2][2][2]  S-matrix of the coupled channels

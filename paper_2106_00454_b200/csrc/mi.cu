@@ -39,6 +39,8 @@ struct MiParams {
   int id_mm[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // basis matrix of term t in the block l = lJ (uncoupled) / J-1
   int id_pp[WPCD_MAX_CHANNELS][WPCD_MAX_TERMS];           // ... in the block l = J+1
   int id_mp[WPCD_MAX_CHANNELS];                           // ... of the off-diagonal Yukawa
+  double* fwork;                                         // L2 variant: [gridDim.x][n][ld] systems of the CTAs (else unused)
+  int ne, S;                                             // energies of this launch, samples
 };
 
 struct MiBasisTable { int n; int l[WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1)]; double mu[WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1)]; };
@@ -113,12 +115,16 @@ __device__ __forceinline__ double2 cdiv(double2 a, double2 b) {
 // (Sherman-Morrison for the rank-nc term) and S = 1 - 2 i f p T_on.  Same S as the complex elimination of Eqs. 6-7, which the
 // oracle performs, up to rounding.  The unknowns are ordered grid points first (block by block), on-shell points last, so that
 // K_on falls out of the last nc pivots without a back substitution over the grid.
+// kGlob: systems too large for shared memory (coupled N_Q > 81, uncoupled N_Q > 164; n <= 256 rows: one thread per row)
+// keep F in a per-CTA region of the workspace that stays in L2; the grid is then a fixed number of CTAs that loop over the
+// systems.  Same code otherwise (the barriers of a CTA order its global accesses too).
+template <bool kGlob>
 __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x, nwarps = nthr >> 5;  // nthr >= n (mi_threads)
   const int NQ = P.NQ, M = NQ + 1, nc = P.coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1, ng = nc * NQ;  // ld even: 16-byte row pairs
-  double* F = reinterpret_cast<double*>(smem_raw);       // [n][ld]
-  double* q = F + (size_t)n * ld;                         // [M]
+  double* F = kGlob ? P.fwork + (size_t)blockIdx.x * n * ld : reinterpret_cast<double*>(smem_raw);       // [n][ld]
+  double* q = kGlob ? reinterpret_cast<double*>(smem_raw) : F + (size_t)n * ld;                         // [M]
   double* D = q + M;                                      // [M] real parts (principal value)
   int* prow = reinterpret_cast<int*>(D + M);              // [n] pivot row of column c
   int* lst = prow + n;                                    // [2][n] rows not yet used as a pivot (double buffered)
@@ -127,8 +133,12 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   __shared__ int cpos[2 * kMiWarps];
   __shared__ double pb[2 * kMiWarps * 8];                 // ... and the panel entries of that row
   __shared__ int pivpos[8];                               // list positions of the panel's pivot rows
-  const int e = P.e_first + blockIdx.x, ch = blockIdx.y;
-  const size_t smp = blockIdx.z;
+  const int nsys = kGlob ? P.ne * P.nch * P.S : 1;
+  for (int sys = kGlob ? blockIdx.x : 0; sys < nsys; sys += gridDim.x) {
+  const int el = kGlob ? sys % P.ne : blockIdx.x;                       // energy within the launch's chunk
+  const int ch = kGlob ? (sys / P.ne) % P.nch : blockIdx.y;
+  const size_t smp = kGlob ? sys / (P.ne * P.nch) : blockIdx.z;
+  const int e = P.e_first + el;
   const double cE = P.hbarc * P.hbarc / (2.0 * P.mured), f = 2.0 * P.mured / (P.hbarc * P.hbarc);
   const double p = sqrt(P.Ecm[e] / cE);
   if (tid < P.nterms) {
@@ -158,7 +168,7 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   // block r / NQ; r >= ng: on-shell point of block r - ng.
   // A warp per row, lanes along the columns; every Yukawa element comes from the tables (grid x grid: basis, per call;
   // row/column of the on-shell point: onb, per energy), scaled by this sample's strengths.
-  const double* onb = P.onb + (size_t)blockIdx.x * P.nbasis * M;
+  const double* onb = P.onb + (size_t)el * P.nbasis * M;
   const size_t nn = (size_t)NQ * NQ;
   for (int r = warp; r < n; r += nwarps) {
     const int a = r < ng ? r / NQ : r - ng, i = r < ng ? r - a * NQ : NQ;
@@ -363,6 +373,8 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
         }
     }
   }
+  __syncthreads();   // the next system of this CTA (kGlob) reuses q, D and the lists
+  }
 }
 
 // threads of a CTA (>= one per row of the system): two warps for n <= 64 (many CTAs per SM; measured N_Q = 24: 0.42 -> 0.23 ms
@@ -376,17 +388,41 @@ size_t mi_smem(int NQ, int coupled) {
   const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1;
   return (size_t)n * ld * 8 + (size_t)2 * M * 8 + (size_t)3 * n * 4 + 16;
 }
+// the L2 variant: F lives in the workspace, only the vectors and lists in shared memory
+size_t mi_smem_glob(int NQ, int coupled) {
+  const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M;
+  return (size_t)2 * M * 8 + (size_t)3 * n * 4 + 16;
+}
+size_t mi_fbytes(int NQ, int coupled) {
+  const int M = NQ + 1, nc = coupled ? 2 : 1, n = nc * M, ld = (n + nc + 1) & ~1;
+  return (((size_t)n * ld * 8) + 255) & ~(size_t)255;
+}
+constexpr int kMiGlobCtas = 320;   // CTAs of the L2 variant (2 per SM on 148 SMs, rounded up): each owns one F region
 
 }  // namespace
 
 constexpr int kMiMaxBasis = WPCD_MAX_CHANNELS * (2 * WPCD_MAX_TERMS + 1);
 constexpr int kMiEChunk = 128;   // energies per launch: the on-shell tables of one chunk live in the workspace
+static size_t mi_tables_bytes(int NQ) {
+  return (((size_t)2 * ((NQ * 8 + 255) & ~255) + (size_t)kMiMaxBasis * NQ * NQ * 8 + (size_t)kMiEChunk * kMiMaxBasis * (NQ + 1) * 8) + 255) & ~(size_t)255;
+}
+// does the system of this kind fit one CTA's shared memory?  (227 KB opt-in on sm_100a: N_Q <= 164 uncoupled, <= 81 coupled)
+static bool mi_in_smem(int NQ, int coupled) { return mi_smem(NQ, coupled) + 4096 <= (size_t)232448; }
 size_t wpcd_mi_workspace(int NQ) {
-  return (size_t)2 * ((NQ * 8 + 255) & ~255) + (size_t)kMiMaxBasis * NQ * NQ * 8 + (size_t)kMiEChunk * kMiMaxBasis * (NQ + 1) * 8;
+  size_t f = 0;   // F regions of the L2 variant, for the larger of the two kinds that needs them
+  for (int coupled = 0; coupled < 2; ++coupled)
+    if (!mi_in_smem(NQ, coupled) && (coupled ? 2 : 1) * (NQ + 1) <= kMiThreads) {
+      const size_t b = (size_t)kMiGlobCtas * mi_fbytes(NQ, coupled);
+      f = b > f ? b : f;
+    }
+  return mi_tables_bytes(NQ) + f;
 }
 
-// does the system of this kind fit one CTA's shared memory?
-bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled) { return mi_smem(NQ, coupled) + 4096 <= (size_t)h->max_smem_optin; }
+// is the system of this kind supported?  One thread per row: n <= 256 (N_Q <= 255 uncoupled, <= 127 coupled)
+bool wpcd_mi_fits(const WpcdHandle* h, int NQ, int coupled) {
+  if (mi_smem(NQ, coupled) + 4096 <= (size_t)h->max_smem_optin) return true;
+  return (coupled ? 2 : 1) * (NQ + 1) <= kMiThreads;
+}
 
 int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel* chan, int n_chan, const double* d_scales,
                    int S, int P, int NQ, double cmap, double hbarc, double mu, const double* d_Ecm, int nE, double* d_S_unc,
@@ -437,10 +473,20 @@ int wpcd_mi_launch(WpcdHandle* h, const wpcd_potential* pot, const wpcd_channel*
     Q.VT = pot->VT; Q.muT = pot->muT; Q.VT_sidx = pot->VT_scale_idx;
     Q.lambdaA = pot->lambda * (WPCD_PI / 2.0);  // wpcd_potential.lambda is convention B: lambda_B = (2/pi) lambda_A (reading C15)
     Q.beta = pot->beta; Q.hbarc = hbarc; Q.mured = mu;
-    const size_t smem = mi_smem(NQ, coupled);
-    int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_mi_solve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "mi attr");
-    if (rc) return rc;
-    k_mi_solve<<<dim3(ne, Q.nch, S), mi_threads(NQ, coupled), smem, st>>>(Q);
+    Q.ne = ne; Q.S = S; Q.fwork = nullptr;
+    if (mi_smem(NQ, coupled) + 4096 <= (size_t)h->max_smem_optin) {
+      const size_t smem = mi_smem(NQ, coupled);
+      int rc = wpcd_check_cuda(h, cudaFuncSetAttribute(k_mi_solve<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "mi attr");
+      if (rc) return rc;
+      k_mi_solve<false><<<dim3(ne, Q.nch, S), mi_threads(NQ, coupled), smem, st>>>(Q);
+    } else {
+      // L2 variant: a fixed grid of CTAs, each with its own F region behind the tables, loops over the systems
+      Q.fwork = reinterpret_cast<double*>(static_cast<char*>(d_work) + mi_tables_bytes(NQ));
+      const long long nsys = (long long)ne * Q.nch * S;
+      int grid = 2 * h->num_sms < kMiGlobCtas ? 2 * h->num_sms : kMiGlobCtas;
+      if (nsys < grid) grid = (int)nsys;
+      k_mi_solve<true><<<grid, kMiThreads, mi_smem_glob(NQ, coupled), st>>>(Q);
+    }
   }
   }
   return wpcd_check_cuda(h, cudaGetLastError(), "mi_solve launch");

@@ -689,9 +689,37 @@ def test_mi_solver_on_gpu(ctx):
         p = np.sqrt(inp.MU * t) / inp.HBARC
         Sx = 1 + 4j * lp * p / (p * p + beta * beta) ** 2 / (1 - lp / (beta * (beta - 1j * p) ** 2))
         assert abs(Su[e] - Sx) < 1e-11, (t, Su[e], Sx)
-    # sizes that do not fit one CTA's shared memory are refused
+    # systems that do not fit one CTA's shared memory (coupled N_Q > 81, uncoupled N_Q > 164) run with F in an L2-resident
+    # workspace region per CTA, a fixed grid looping over the systems: coupled N_Q = 96 and 120, uncoupled
+    # N_Q = 200, more systems than CTAs (2 samples x 3 channels x 5 energies here; the loop is also taken with few systems)
+    sc2 = inp.sample_scales(2, seed=6)
+    for NQ, chans in ((96, [(1, 1), (1, 2), (0, 0)]), (120, [(1, 1)]), (200, [(0, 0), (0, 2)])):
+        S_unc, S_cpl = h.mi_solve(chans, dE, NQ=NQ, V0=inp.MT_V0, mu=inp.MT_MU, scale_idx=[0, 1], VT=inp.TENSOR_V,
+                                  muT=inp.TENSOR_MU, VT_scale_idx=2, scales=_to_dev(ctx, sc2), S=2)
+        torch.cuda.synchronize()
+        worst, iu, ic = 0.0, 0, 0
+        for (kind, lJ) in chans:
+            for s in range(2):
+                V0 = inp.MT_V0 * sc2[s, :2]
+                for e, t in enumerate(tl):
+                    if kind:
+                        got = S_cpl[s, ic, e].cpu().numpy(); got = got[..., 0] + 1j * got[..., 1]
+                        ref, _ = hp.o.mi_solve(t, coupled=True, V0=V0, mu=inp.MT_MU, l_or_J=lJ, VT=inp.TENSOR_V * sc2[s, 2],
+                                               muT=inp.TENSOR_MU, NQ=NQ)
+                        worst = max(worst, np.abs(got - ref).max())
+                    else:
+                        got = S_unc[s, iu, e].cpu().numpy(); got = got[0] + 1j * got[1]
+                        ref, _ = hp.o.mi_solve(t, V0=V0, mu=inp.MT_MU, l_or_J=lJ, NQ=NQ)
+                        worst = max(worst, abs(got - ref))
+            if kind: ic += 1
+            else: iu += 1
+        print(f"MI on the GPU (L2 variant), NQ={NQ}: max |dS| vs oracle {worst:.2e}")
+        assert worst < 1e-10
+    # more than one thread per row would be needed: refused
     with pytest.raises(RuntimeError):
-        h.mi_solve([(1, 1)], dE, NQ=96, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+        h.mi_solve([(1, 1)], dE, NQ=128, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
+    with pytest.raises(RuntimeError):
+        h.mi_solve([(0, 0)], dE, NQ=256, V0=inp.MT_V0, mu=inp.MT_MU)
     # wpcd_sigma_tot on S-matrices (d_bin = d_dE = NULL) against the oracle's Clebsch-Gordan chain on the oracle's MI S
     names = [c[0] for c in inp.CHANNELS_J4]; sJ = [inp.channel_sJ(nm) for nm in names]
     S_unc, S_cpl = h.mi_solve(channels, dE, NQ=24, V0=inp.MT_V0, mu=inp.MT_MU, VT=inp.TENSOR_V, muT=inp.TENSOR_MU)
