@@ -112,7 +112,7 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
  * accumulated rotations are applied to H and C as fp64 tensor-core (DMMA) tile products; the pivots of the next step
  * are solved while the current step's updates run.  Rows and columns are taken in the order of descending diagonal
  * entries (a relabelling; one to two sweeps fewer on these graded matrices).  n <= 200: the matrix (upper 8x8 blocks) in shared memory, the
- * eigenvectors in an L2-resident workspace, 1-4 matrices in flight per SM; 200 < n <~ 880: the matrix through L2, the
+ * eigenvectors in an L2-resident workspace, 1-4 matrices in flight per SM; 200 < n <= 848: the matrix through L2, the
  * eigenvectors not accumulated during the sweeps at all -- the 16x16 rotation products are logged (workspace) and replayed
  * panel by panel in shared memory into d_C by the same persistent launch (bit-identical to the accumulation in place, a
  * tenth of its DRAM traffic; the workspace then holds two log regions per SM: ~3 GB at n = 300, ~20 GB at n = 800);

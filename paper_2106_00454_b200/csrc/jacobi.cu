@@ -21,7 +21,7 @@
 //     the sweeps converge faster than in the natural ascending order (n=200: 7.0 -> 6.3 sweeps).
 // n <= 200: A (upper 8x8 blocks) and Q in shared memory, V in a per-CTA global workspace that stays L2 resident; for
 // n <= 104 with 320 threads (n <= 56: 160) so that 2 (4) matrices share an SM.
-// 200 < n <~ 880 (A does not fit shared memory, the Q buffers do): LOG MODE.  V <- V Q never feeds back into the sweeps, and
+// 200 < n <= 848 (A does not fit shared memory, the Q buffers do): LOG MODE.  V <- V Q never feeds back into the sweeps, and
 // with A and V both streaming through L2/DRAM every step the launch was DRAM-bound (174 GB per 592 matrices at n = 300).
 // So the sweeps run on A alone (through L2), every rotating slot appends its 16x16 product to a log region, and the same
 // persistent launch later REPLAYS the log: a CTA takes a panel of <= 64 rows of the identity into shared memory, applies
@@ -1027,7 +1027,7 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
   return WPCD_OK;
 }
 
-// Log mode (k_jacobi<4>): used where the workspace mode 2 would run (A does not fit shared memory, Q does: 200 < n <~ 880).
+// Log mode (k_jacobi<4>): used where the workspace mode 2 would run (A does not fit shared memory, Q does: 200 < n <= 848).
 // Capacity of a log region: kLogSweeps sweeps' worth of rotating slots (measured need: 5-6; more goes to the fallback
 // launch) and 16 sweeps' worth of steps.  WPCD_JACOBI_LOG_SWEEPS in the environment overrides kLogSweeps (a test hook:
 // 0 disables the log mode, 1 forces matrices into the fallback launch).
