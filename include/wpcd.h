@@ -120,7 +120,8 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
  *   d_A    : [batch][n][n] input (only read; must be symmetric)
  *   d_W    : [batch][n] eigenvalues ascending
  *   d_C    : [batch][n][n] eigenvectors, column k belongs to d_W[k]  (C_ij = <x_i|z_j>)
- *   d_info : [batch] sweeps used (>= 1), or -1 if not converged in max_sweeps
+ *   d_info : [batch] sweeps used (>= 1), or -1 if not converged in max_sweeps (-2 for every matrix: the scheduler of the
+ *            200 < n <= 848 path gave up waiting -- a safety net that has never been seen to fire; the results are then invalid)
  *   tol    : a pivot is rotated iff |a_pq| > tol sqrt(|a_pp a_qq|); convergence = a full sweep without rotation.
  *            tol <= 0 selects the default 2^-52.
  *   h_rows : optional HOST array of n_ranges (<= 4) half-open row ranges [lo, hi) of C that the caller needs (NULL,

@@ -467,6 +467,11 @@ __global__ void k_sched_init(int* __restrict__ sched, int nzero, int nneg) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nzero + nneg; i += gridDim.x * blockDim.x) sched[i] = i < nzero ? 0 : -1;
 }
 __global__ void k_set_counter(int* p, int v) { *p = v; }
+// the watchdog of the log mode fired (a wait that should never be that long): no result of the launch can be trusted
+__global__ void k_log_watchdog(const int* __restrict__ sched, int* __restrict__ info, int batch) {
+  if (sched[6] == 0) return;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < batch; i += gridDim.x * blockDim.x) info[i] = -2;
+}
 
 
 // Schedule tables (one copy per launch, read through the L1): the tournament needs integer divisions that would
@@ -1134,6 +1139,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
     k_set_counter<<<1, 1, 0, st>>>(P2.next, L.grid);
     rc = launch_mode<2, 640>(h, P2, L.grid, g.smem, st);
     if (rc) return rc;
+    k_log_watchdog<<<8, 256, 0, st>>>(P4.sched, d_info, batch);
     return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch (log mode)");
   }
   const int grid = global_grid(h, g, batch);

@@ -77,8 +77,9 @@ class Pipeline:
     @property
     def launches_per_step(self):
         # k_grid, k_basis, k_combine per kind; k_schedule, k_jacobi, k_bins, k_onshell, k_phase per kind; the eigensolver's
-        # log mode (200 < n <= 848, csrc/jacobi.cu) adds k_sched_init, k_set_counter and the fallback launch of k_jacobi
-        extra = sum(3 for b in self.kind.values() if 200 < b["n"] <= 848)
+        # log mode (200 < n <= 848, csrc/jacobi.cu) adds k_sched_init, k_set_counter, the fallback launch of k_jacobi and
+        # k_log_watchdog
+        extra = sum(4 for b in self.kind.values() if 200 < b["n"] <= 848)
         return 2 + len(self.kind) * 6 + extra + (1 if self.J is not None else 0)
 
     def solve_device(self, events=None, to_host=False):
