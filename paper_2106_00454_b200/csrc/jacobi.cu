@@ -703,9 +703,10 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
   // come from a global counter that k_schedule set to gridDim.x
   __shared__ int s_next;
   __shared__ int s_job[4];
-  const int nmat = (kMode != 4 && P.nlist) ? *P.nlist : P.batch;
-  bool busy0 = false, busy1 = false;  // log mode, thread 0: own log regions that wait for their replay
-  int waits = 0;
+  constexpr bool kList = kMode == 2 || kMode == 3;  // only the workspace modes serve as the fallback launch of the log mode
+  // log mode, used by thread 0 only: [0], [1] own log regions that wait for their replay, [2] consecutive waits
+  __shared__ int s_state[4];
+  if (kMode == 4 && tid == 0) { s_state[0] = 0; s_state[1] = 0; s_state[2] = 0; }
   for (int it = blockIdx.x;;) {
     int mat, region = 0;
     if (kMode == 4) {
@@ -732,22 +733,22 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
           a = r;
         } else {
           int* done = P.sched + kSchedDone + 2 * blockIdx.x;
-          if (busy0 && sc[kSchedDone + 2 * blockIdx.x] >= P.npanels) { done[0] = 0; busy0 = false; }
-          if (busy1 && sc[kSchedDone + 2 * blockIdx.x + 1] >= P.npanels) { done[1] = 0; busy1 = false; }
-          if (!(busy0 && busy1) && sc[0] < P.batch) {
+          if (s_state[0] && sc[kSchedDone + 2 * blockIdx.x] >= P.npanels) { done[0] = 0; s_state[0] = 0; }
+          if (s_state[1] && sc[kSchedDone + 2 * blockIdx.x + 1] >= P.npanels) { done[1] = 0; s_state[1] = 0; }
+          if (!(s_state[0] && s_state[1]) && sc[0] < P.batch) {
             const int mnew = atomicAdd(P.sched, 1);
             if (mnew < P.batch) {
-              kind = kJobSolve; a = mnew; b = busy0 ? 1 : 0;
-              if (b) busy1 = true; else busy0 = true;
+              kind = kJobSolve; a = mnew; b = s_state[0] ? 1 : 0;
+              s_state[b] = 1;
             }
           }
           if (kind == kJobWait && sc[0] >= P.batch && sc[4] >= P.batch) {
             __threadfence();
             if (sc[3] >= sc[1] * P.npanels) kind = kJobExit;
           }
-          if (kind == kJobWait && ++waits > (1 << 23)) { P.sched[6] = 1; kind = kJobExit; }  // watchdog: never hang the GPU
+          if (kind == kJobWait && ++s_state[2] > (1 << 23)) { P.sched[6] = 1; kind = kJobExit; }  // watchdog: never hang the GPU
         }
-        if (kind != kJobWait) waits = 0;
+        if (kind != kJobWait) s_state[2] = 0;
         s_job[0] = kind; s_job[1] = a; s_job[2] = b;
       }
       __syncthreads();
@@ -767,8 +768,8 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
       mat = s_job[1];
       region = 2 * blockIdx.x + s_job[2];
     } else {
-      if (it >= nmat) break;
-      mat = P.list ? P.list[it] : it;
+      if (it >= ((kList && P.nlist) ? *P.nlist : P.batch)) break;
+      mat = (kList && P.list) ? P.list[it] : it;
     }
     int* const lhdr = kMode == 4 ? reinterpret_cast<int*>(P.logbase + (size_t)region * P.region_bytes) : nullptr;
     if (kMode == 4) {
@@ -968,7 +969,7 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
           P.sched[P.ready_off + ticket] = region;
         } else {  // too many rotations for the log region: the matrix is redone by the fallback launch (workspace mode)
           P.sched[P.fb_off + atomicAdd(P.sched + 5, 1)] = mat;
-          if (region & 1) busy1 = false; else busy0 = false;
+          s_state[region & 1] = 0;
         }
         __threadfence();
         atomicAdd(P.sched + 4, 1);
