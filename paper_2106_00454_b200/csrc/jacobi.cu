@@ -455,6 +455,7 @@ struct JacobiParams {
   size_t region_bytes;
   int log_cap, log_steps;  // capacity of a region in entries (rotating slots) and in tournament steps
   int rbp, npanels;        // row blocks of C per replay unit, replay units per matrix
+  int nsolvers;            // CTAs that own log regions and an A workspace (the others only replay)
   int ready_off, fb_off;   // offsets (ints) of the ready list and of the fallback list inside the scheduler block
 };
 
@@ -735,7 +736,7 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
           int* done = P.sched + kSchedDone + 2 * blockIdx.x;
           if (s_state[0] && sc[kSchedDone + 2 * blockIdx.x] >= P.npanels) { done[0] = 0; s_state[0] = 0; }
           if (s_state[1] && sc[kSchedDone + 2 * blockIdx.x + 1] >= P.npanels) { done[1] = 0; s_state[1] = 0; }
-          if (!(s_state[0] && s_state[1]) && sc[0] < P.batch) {
+          if ((int)blockIdx.x < P.nsolvers && !(s_state[0] && s_state[1]) && sc[0] < P.batch) {
             const int mnew = atomicAdd(P.sched, 1);
             if (mnew < P.batch) {
               kind = kJobSolve; a = mnew; b = s_state[0] ? 1 : 0;
@@ -1040,7 +1041,7 @@ int launch_mode(WpcdHandle* h, const JacobiParams& P, int grid, size_t smem, cud
 constexpr int kLogSweeps = 7;
 struct LogGeometry {
   bool use;
-  int grid, cap, steps, rbp, npanels, ready_off, fb_off;
+  int grid, nsolvers, cap, steps, rbp, npanels, ready_off, fb_off;
   size_t region_bytes, smem, sched_bytes, a_bytes, off_sched, off_a, off_log, off_fb, total;
 };
 
@@ -1056,7 +1057,8 @@ LogGeometry log_geometry(const WpcdHandle* h, const Geometry& g, int batch) {
   if (rbp > 2) rbp &= ~1;
   L.use = g.mode == 2 && sweeps > 0 && rbp >= 1;
   if (!L.use) return L;
-  L.grid = batch < h->num_sms ? batch : h->num_sms;
+  L.grid = h->num_sms;  // small batches: the CTAs beyond the batch take replay units only
+  L.nsolvers = batch < h->num_sms ? batch : h->num_sms;
   L.cap = sweeps * (g.m - 1) * g.nslots;
   L.steps = 16 * (g.m - 1);
   L.rbp = rbp;
@@ -1064,15 +1066,15 @@ LogGeometry log_geometry(const WpcdHandle* h, const Geometry& g, int batch) {
   L.region_bytes = (log_q_off(g.np, L.steps, L.cap) + (size_t)L.cap * kQSlot * 8 + 255) & ~(size_t)255;
   const size_t smem_b = (size_t)rbp * per_rb + 4 * (size_t)(g.np + 8);
   L.smem = g.smem > smem_b ? g.smem : smem_b;
-  L.ready_off = kSchedDone + 2 * L.grid;
+  L.ready_off = kSchedDone + 2 * L.nsolvers;
   L.fb_off = L.ready_off + batch;
   L.sched_bytes = (((size_t)(L.fb_off + batch) * 4) + 255) & ~(size_t)255;
   L.a_bytes = (size_t)(g.nb * (g.nb + 1) / 2) * 512;
   L.off_sched = g.tab_bytes;
   L.off_a = L.off_sched + L.sched_bytes;
-  L.off_log = L.off_a + (size_t)L.grid * L.a_bytes;
-  L.off_fb = L.off_log + (size_t)2 * L.grid * L.region_bytes;
-  L.total = L.off_fb + 256 + (size_t)L.grid * g.gstride * 8;  // fallback: its own counter and mode-2 workspaces
+  L.off_log = L.off_a + (size_t)L.nsolvers * L.a_bytes;
+  L.off_fb = L.off_log + (size_t)2 * L.nsolvers * L.region_bytes;
+  L.total = L.off_fb + 256 + (size_t)L.nsolvers * g.gstride * 8;  // fallback: its own counter and mode-2 workspaces
   return L;
 }
 
@@ -1109,7 +1111,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   P.list = nullptr; P.nlist = nullptr; P.sched = nullptr; P.logbase = nullptr;
-  P.region_bytes = 0; P.log_cap = P.log_steps = P.rbp = P.npanels = P.ready_off = P.fb_off = 0;
+  P.region_bytes = 0; P.log_cap = P.log_steps = P.rbp = P.npanels = P.nsolvers = P.ready_off = P.fb_off = 0;
   const LogGeometry L = log_geometry(h, g, batch);
   if (L.use) {
     // Log mode: one persistent launch solves the matrices without their eigenvectors (A through L2, as in mode 2),
@@ -1125,7 +1127,7 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
     P4.gstride = L.a_bytes / 8;
     P4.logbase = w + L.off_log;
     P4.region_bytes = L.region_bytes;
-    P4.log_cap = L.cap; P4.log_steps = L.steps; P4.rbp = L.rbp; P4.npanels = L.npanels;
+    P4.log_cap = L.cap; P4.log_steps = L.steps; P4.rbp = L.rbp; P4.npanels = L.npanels; P4.nsolvers = L.nsolvers;
     P4.ready_off = L.ready_off; P4.fb_off = L.fb_off;
     P4.stream_v = 0;
     k_sched_init<<<64, 256, 0, st>>>(P4.sched, L.ready_off, 2 * batch);
@@ -1136,9 +1138,9 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
     P2.nlist = P4.sched + 5;
     P2.next = reinterpret_cast<int*>(w + L.off_fb);
     P2.gwork = reinterpret_cast<double*>(w + L.off_fb + 256);
-    P2.stream_v = (size_t)L.grid * L.a_bytes <= ((size_t)96 << 20);
-    k_set_counter<<<1, 1, 0, st>>>(P2.next, L.grid);
-    rc = launch_mode<2, 640>(h, P2, L.grid, g.smem, st);
+    P2.stream_v = (size_t)L.nsolvers * L.a_bytes <= ((size_t)96 << 20);
+    k_set_counter<<<1, 1, 0, st>>>(P2.next, L.nsolvers);
+    rc = launch_mode<2, 640>(h, P2, L.nsolvers, g.smem, st);
     if (rc) return rc;
     k_log_watchdog<<<8, 256, 0, st>>>(P4.sched, d_info, batch);
     return wpcd_check_cuda(h, cudaGetLastError(), "diag_batched launch (log mode)");
