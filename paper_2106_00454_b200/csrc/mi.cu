@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
   int* prow = reinterpret_cast<int*>(D + M);              // [n] pivot row of column c
   int* lst = prow + n;                                    // [2][n] rows not yet used as a pivot (double buffered)
   __shared__ double sV0[WPCD_MAX_TERMS], sVT;
-  __shared__ double cval[2 * kMiWarps];                   // pivot candidate of every warp (double buffered over the columns)
+  __shared__ unsigned ckey[2 * kMiWarps];                 // pivot candidate of every warp (double buffered over the columns): its key,
   __shared__ int cpos[2 * kMiWarps];
   __shared__ double pb[2 * kMiWarps * 8];                 // ... and the panel entries of that row
   __shared__ int pivpos[8];                               // list positions of the panel's pivot rows
@@ -225,26 +225,22 @@ __global__ void __launch_bounds__(kMiThreads) k_mi_solve(MiParams P) {
       for (int x = 0; x < 8; ++x) {
         if (x < w) {
           const int cb = x & 1;
-          double best = used ? -1.0 : fabs(a[x]);
-          int bj = tid;
-          for (int o = 16; o > 0; o >>= 1) {
-            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
-            const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
-            if (ob > best || (ob == best && oj < bj)) { best = ob; bj = oj; }
-          }
+          // arg-max of the warp by the high words of |a| (redux.sync; the order of positive doubles is that of their bit
+          // patterns): the row taken is within 2^-20 of the largest, which is all that partial pivoting needs
+          const double best = used ? -1.0 : fabs(a[x]);
+          const unsigned key = used ? 0u : (unsigned)__double2hiint(best) + 1u;
+          const unsigned kmax = __reduce_max_sync(0xffffffffu, key);
+          const int bj = (tid & ~31) + __ffs(__ballot_sync(0xffffffffu, key == kmax)) - 1;
           if (warp < nrw && bj == tid) {
-            cval[cb * kMiWarps + warp] = best;
+            ckey[cb * kMiWarps + warp] = kmax;
             cpos[cb * kMiWarps + warp] = tid;
 #pragma unroll
             for (int x2 = 0; x2 < 8; ++x2) pb[(cb * kMiWarps + warp) * 8 + x2] = a[x2];
           }
           __syncthreads();
-          double gbest = cval[cb * kMiWarps];
-          int gw = 0;
-          for (int ww = 1; ww < nrw; ++ww) {
-            const double ob = cval[cb * kMiWarps + ww];
-            if (ob > gbest) { gbest = ob; gw = ww; }
-          }
+          const unsigned wk = lane < nrw ? ckey[cb * kMiWarps + lane] : 0u;   // the winner among the warps, the same way
+          const unsigned wmax = __reduce_max_sync(0xffffffffu, wk);
+          const int gw = __ffs(__ballot_sync(0xffffffffu, wk == wmax)) - 1;
           const int gpos = cpos[cb * kMiWarps + gw];
           double pr[8];
 #pragma unroll
