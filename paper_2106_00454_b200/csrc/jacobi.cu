@@ -1109,6 +1109,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   // through L2 (n = 400: 13 beats 17)
   if (g.mode == 1) P.full_every = (g.m - 1 + 2) / 3 > 5 ? (g.m - 1 + 2) / 3 : 5;
   else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
+  if (g.m == 6) P.full_every = 3;  // n = 41 .. 48 (5 steps per sweep): two full pivot steps save a sweep (n = 48: 7.06 -> 6.02, 1.81 -> 1.72 ms)
+  if (g.m == 8) P.full_every = 4;  // n = 49 .. 64 (7 steps): n = 56 2.73 -> 2.65 ms, n = 64 unchanged
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   P.list = nullptr; P.nlist = nullptr; P.sched = nullptr; P.logbase = nullptr;
   P.region_bytes = 0; P.log_cap = P.log_steps = P.rbp = P.npanels = P.nsolvers = P.ready_off = P.fb_off = 0;
