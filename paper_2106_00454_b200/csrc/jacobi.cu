@@ -546,7 +546,9 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
     __syncwarp();
     // full sweep of the pivot every full_every-th step (every block then sits in a pivot at >= 1 full step per sweep,
     // so every pair is still met in every sweep); always for small matrices, where padding leaves few real pivots
-    const bool full = (tn % P.full_every) == 0 || P.nb < 6;  // nb >= 6: every block sits in >= 1 full real pivot per sweep
+    // nb >= 5 with two full steps per sweep (wpcd_jacobi_launch): a block is idle (paired with the one padding player of
+    // nb = 5, 7) at most once per sweep, so it sits in a full real pivot in at least one of them
+    const bool full = (tn % P.full_every) == 0 || P.nb < 5;
     rotated = inner_solve(A, Qn, I, J, P.tol, full, lane);
     if (kMode == 4 && rotated) {  // log mode: the eigenvectors are accumulated later, by a replay of these products
       int idx = 0;
@@ -1109,7 +1111,8 @@ int wpcd_jacobi_launch(WpcdHandle* h, int n, int batch, const double* d_A, doubl
   // through L2 (n = 400: 13 beats 17)
   if (g.mode == 1) P.full_every = (g.m - 1 + 2) / 3 > 5 ? (g.m - 1 + 2) / 3 : 5;
   else P.full_every = (g.m - 1 + 3) / 4 > 4 ? (g.m - 1 + 3) / 4 : 4;
-  if (g.m == 6) P.full_every = 3;  // n = 41 .. 48 (5 steps per sweep): two full pivot steps save a sweep (n = 48: 7.06 -> 6.02, 1.81 -> 1.72 ms)
+  if (g.m == 6) P.full_every = 3;  // n = 33 .. 48 (5 steps per sweep, steps 0 and 3 full): n = 48: 7.06 -> 6.02 sweeps, 1.81 -> 1.72 ms;
+                                   // n = 33 .. 40 had full pivots in every step: n = 40 1.65 -> 1.48 ms
   if (g.m == 8) P.full_every = 4;  // n = 49 .. 64 (7 steps): n = 56 2.73 -> 2.65 ms, n = 64 unchanged
   P.tol = tol > 0.0 ? tol : 2.220446049250313e-16;
   P.list = nullptr; P.nlist = nullptr; P.sched = nullptr; P.logbase = nullptr;

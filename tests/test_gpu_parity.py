@@ -230,7 +230,7 @@ def _diag_check(ctx, A, tol_rel=1e-11):
     return W, C, info
 
 
-@pytest.mark.parametrize("n", [2, 3, 7, 8, 9, 16, 17, 31, 33, 63, 104, 105, 112, 113, 120, 129])
+@pytest.mark.parametrize("n", [2, 3, 7, 8, 9, 16, 17, 31, 33, 36, 40, 41, 48, 49, 56, 63, 104, 105, 112, 113, 120, 129])
 def test_diag_ragged_sizes_random(ctx, n):
     rng = np.random.default_rng(n)
     A = rng.standard_normal((5, n, n)); A = A + A.transpose(0, 2, 1)
