@@ -129,7 +129,11 @@ int wpcd_build_channels(void* handle, const wpcd_grid* grid, const wpcd_potentia
  *            internal ordering with a wanted row are not updated; every row outside the ranges is returned as ZEROS;
  *            the eigenvalues and the wanted rows are unaffected (bit-identical to the full run).  The on-shell T of
  *            the n <= 200 path only reads the rows of the on-shell bins.
- *   d_work : wpcd_diag_workspace_bytes(n, batch) bytes (never 0: the schedule tables live there) */
+ *   d_work : wpcd_diag_workspace_bytes(n, batch) bytes (never 0: the schedule tables live there; gigabytes for 200 < n <= 848)
+ * Test hook (csrc/jacobi.cu): the environment variable WPCD_JACOBI_LOG_SWEEPS, read at every call of this function and of
+ * wpcd_diag_workspace_bytes, sets the capacity of a log region in sweeps (default 7; 0 = the 200 < n <= 848 path accumulates the
+ * eigenvectors in the workspace as the larger sizes do, 1 = every matrix overflows its log and is redone by the fallback launch).
+ * The results do not depend on it (bit-identical, tests/test_gpu_parity.py). */
 int wpcd_diag_batched(void* handle, int n, int batch, const double* d_A, double* d_W, double* d_C, int* d_info,
                       double tol, int max_sweeps, const int* h_rows, int n_ranges, void* d_work, size_t work_bytes,
                       void* stream);
