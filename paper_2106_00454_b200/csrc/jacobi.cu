@@ -431,6 +431,49 @@ __device__ __forceinline__ void apply_V_item(double* __restrict__ V, int nb, con
   }
 }
 
+// The same product for the replay of the log mode, with the B fragments of Q already in registers (they are loaded, through
+// L2 only, before the warp waits for its item's turn).  Same arithmetic and order as apply_V_item<2>.
+__device__ __forceinline__ void load_bq_cg(const double* __restrict__ Q, int lane, double2 (&bq)[2][2]) {
+  const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+  for (int c = 0; c < 2; ++c)
+#pragma unroll
+    for (int r = 0; r < 2; ++r) bq[c][r] = __ldcg(reinterpret_cast<const double2*>(Q + qoff(8 * c + 4 * r + t, g)));
+}
+__device__ __forceinline__ void apply_V_bq(double* __restrict__ V, int nb, const double2 (&bq)[2][2], int I, int J,
+                                           const int* __restrict__ rb, int nrb, int lane) {
+  const int g = lane >> 2, t = lane & 3;
+  const int cb[2] = {I, J};
+#pragma unroll 1
+  for (int k = 0; k < nrb; k += 2) {
+    const bool two = k + 1 < nrb;
+    double* v0 = V + ((size_t)(rb[k] * nb) << 6) + 8 * g + 2 * t;
+    double* v1 = V + ((size_t)(rb[two ? k + 1 : k] * nb) << 6) + 8 * g + 2 * t;
+    double2 f0[2], f1[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      f0[c] = *reinterpret_cast<const double2*>(v0 + 64 * cb[c]);
+      f1[c] = *reinterpret_cast<const double2*>(v1 + 64 * cb[c]);
+    }
+    double o0[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, o1[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+      for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int ni = 0; ni < 2; ++ni) {
+          const double q = ni ? bq[c][r].y : bq[c][r].x;
+          dmma(o0[ni], r ? f0[c].y : f0[c].x, q);
+          dmma(o1[ni], r ? f1[c].y : f1[c].x, q);
+        }
+#pragma unroll
+    for (int ni = 0; ni < 2; ++ni) {
+      *reinterpret_cast<double2*>(v0 + 64 * cb[ni]) = make_double2(o0[ni][0], o0[ni][1]);
+      if (two) *reinterpret_cast<double2*>(v1 + 64 * cb[ni]) = make_double2(o1[ni][0], o1[ni][1]);
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------- the kernel
 struct JacobiParams {
   const double* H;
@@ -560,7 +603,13 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
         const double2* src = reinterpret_cast<const double2*>(Qn);
 #pragma unroll
         for (int u = 0; u < kQSlot / 64; ++u) __stcs(dst + lane + 32 * u, src[lane + 32 * u]);  // streaming: A stays in L2
-        if (lane == 0) sm.logtag[idx] = (I & 0xFFFF) | ((J & 0xFFFF) << 16);
+        if (lane == 0) {
+          sm.logtag[idx] = (I & 0xFFFF) | ((J & 0xFFFF) << 16);
+          // per-block sequence numbers for the replay's dataflow order (sm.act doubles as the counters in the log mode;
+          // a block sits in one slot per step and the steps are barrier-separated: no race)
+          sm.logtag[sm.logcap + idx] = (sm.act[I] & 0xFFFF) | ((sm.act[J] & 0xFFFF) << 16);
+          ++sm.act[I]; ++sm.act[J];
+        }
       } else if (lane == 0) {
         sm.ctr[5] = 1;
       }
@@ -574,13 +623,14 @@ __device__ __forceinline__ void prepare_slot(const Smem& sm, const JacobiParams&
 
 // ---------------------------------------------------------------------------------------------- log mode
 // Layout of a log region (ints, then the products): [0] entries, [1] steps, [2] overflow, [3] matrix, [8 ..) perm[np],
-// src[np], step_start[log_steps + 2], tags[log_cap]; the products [log_cap][256] doubles follow, 256-byte aligned.
+// src[np], step_start[log_steps + 2], tags[log_cap] (I | J << 16), seq[log_cap] (how many earlier entries touched block I |
+// the same for J << 16); the products [log_cap][256] doubles follow, 256-byte aligned.
 __host__ __device__ inline int log_perm_off() { return 8; }
 __host__ __device__ inline int log_src_off(int np) { return 8 + np; }
 __host__ __device__ inline int log_step_off(int np) { return 8 + 2 * np; }
 __host__ __device__ inline int log_tag_off(int np, int steps) { return 8 + 2 * np + steps + 2; }
 __host__ __device__ inline size_t log_q_off(int np, int steps, int cap) {
-  return (((size_t)(log_tag_off(np, steps) + cap) * 4) + 255) & ~(size_t)255;
+  return (((size_t)(log_tag_off(np, steps) + 2 * cap) * 4) + 255) & ~(size_t)255;   // tags[cap], then seq[cap]
 }
 constexpr int kJobWait = 0, kJobSolve = 1, kJobReplay = 2, kJobExit = 3;
 
@@ -613,27 +663,40 @@ __device__ __forceinline__ void replay_panel(const JacobiParams& P, int region, 
   for (int k = tid; k < n; k += kThreads) srcs[k] = __ldcg(src + k);
   if (tid < P.rbp) rbl[tid] = tid;
   __syncthreads();
+  // Items = (log entry, pair of row blocks of the panel), in log order, dealt round-robin to the warps.  No barrier per
+  // tournament step: an item may run as soon as the two column blocks of its entry have received all earlier products in
+  // its rows -- dn[pr][block] counts them, the entry carries the counts it must see (seq).  Log order is a topological
+  // order and every warp works through its items in that order, so the first unfinished item can always run.
   const int nper = (nrbp + 1) >> 1;  // items of two row blocks
-  for (int gs = 0; gs < nsteps; ++gs) {
-    const int e0 = __ldcg(step_start + gs), e1 = __ldcg(step_start + gs + 1);
-#ifndef WPCD_NO_REPLAY_PREFETCH
-    if (gs + 1 < nsteps) {  // the next step's products on their way from DRAM to L2 while this step computes
-      const int e2 = __ldcg(step_start + gs + 2);
-      const char* q = reinterpret_cast<const char*>(logq + (size_t)e1 * kQSlot);
-      for (int x = tid; x < (e2 - e1) * (kQSlot * 8 / 128); x += kThreads) asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)x * 128));
+  volatile int* dn = rbl + P.rbp;    // [nper][nb]
+  const int* seqs = tags + P.log_cap;
+  const int nent = __ldcg(hdr);
+  for (int x = tid; x < nper * nb; x += kThreads) dn[x] = 0;
+  __syncthreads();
+  constexpr int kWarps = kThreads / 32;
+  for (int itm = warp; itm < nent * nper; itm += kWarps) {
+    const int e = itm / nper, pr = itm - e * nper;
+    const int tag = __ldcg(tags + e), sq = __ldcg(seqs + e);
+    const int I = tag & 0xFFFF, J = tag >> 16;
+    {  // this warp's next product on its way from DRAM to L2 meanwhile
+      const int en = (itm + kWarps) / nper;
+      if (en < nent && lane < kQSlot * 8 / 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(logq + (size_t)en * kQSlot) + lane * 128));
     }
-#endif
-    if (e1 <= e0) continue;
-    for (int itm = warp; itm < (e1 - e0) * nper; itm += kThreads / 32) {
-      const int e = e0 + itm / nper, pr = itm - (itm / nper) * nper;
-      const int tag = __ldcg(tags + e);
-      const int I = tag & 0xFFFF, J = (tag >> 16) == 0xFFFF ? -1 : (tag >> 16);
-      const int nrb = nrbp - 2 * pr < 2 ? nrbp - 2 * pr : 2;
-      if (J >= 0) apply_V_item<2, true>(Vp, nb, logq + (size_t)e * kQSlot, I, J, rbl + 2 * pr, nrb, lane, false);
-      else apply_V_item<1, true>(Vp, nb, logq + (size_t)e * kQSlot, I, J, rbl + 2 * pr, nrb, lane, false);
+    double2 bq[2][2];
+    load_bq_cg(logq + (size_t)e * kQSlot, lane, bq);  // in flight while the warp waits for its turn
+    if (lane == 0) {
+      volatile int* d = dn + pr * nb;
+      int spins = 0;
+      while ((d[I] != (sq & 0xFFFF) || d[J] != (sq >> 16)) && ++spins < (1 << 26)) __nanosleep(32);
     }
-    __syncthreads();
+    __syncwarp();
+    const int nrb = nrbp - 2 * pr < 2 ? nrbp - 2 * pr : 2;
+    apply_V_bq(Vp, nb, bq, I, J, rbl + 2 * pr, nrb, lane);
+    __threadfence_block();
+    __syncwarp();
+    if (lane == 0) { dn[pr * nb + I] = (sq & 0xFFFF) + 1; dn[pr * nb + J] = (sq >> 16) + 1; }
   }
+  __syncthreads();
   double* Co = P.C + (size_t)mat * n * n;
   for (int lr = 0; lr < 8 * nrbp; ++lr) {
     const int i = 8 * rb0 + lr;
@@ -823,6 +886,8 @@ __global__ void __launch_bounds__(kThr, kThr == 128 ? 5 : 640 / kThr) k_jacobi(J
     const int nvgrp = (nact + kVRowBlocksPerItem - 1) / kVRowBlocksPerItem;
     const int nitems = kMode == 4 ? ntiles : ntiles + nslots * nvgrp;  // log mode: no eigenvector items
     const float rnvgrp = 1.0f / (float)(nvgrp > 0 ? nvgrp : 1);
+    if (kMode == 4)  // the list of active row blocks is not used in the log mode: its place holds the per-block entry counters
+      for (int rb = tid; rb < nb; rb += kThreads) sm.act[rb] = 0;
     __syncthreads();
     for (int e = tid; e < np * np; e += kThreads) {
       int r = e / np, c = e - r * np;
@@ -1053,7 +1118,7 @@ LogGeometry log_geometry(const WpcdHandle* h, const Geometry& g, int batch) {
   if (const char* e = getenv("WPCD_JACOBI_LOG_SWEEPS")) sweeps = atoi(e);
   const size_t cap_smem = (size_t)h->max_smem_optin;
   const size_t per_rb = (size_t)g.nb * 512;
-  size_t avail = cap_smem > 2048 + 4 * (size_t)g.np ? cap_smem - 2048 - 4 * (size_t)g.np : 0;
+  size_t avail = cap_smem > 2048 + 4 * (size_t)(g.np + 4 * g.nb) ? cap_smem - 2048 - 4 * (size_t)(g.np + 4 * g.nb) : 0;
   int rbp = (int)(avail / per_rb);
   if (rbp > 8) rbp = 8;
   if (rbp > 2) rbp &= ~1;
@@ -1066,7 +1131,7 @@ LogGeometry log_geometry(const WpcdHandle* h, const Geometry& g, int batch) {
   L.rbp = rbp;
   L.npanels = (g.nb + rbp - 1) / rbp;
   L.region_bytes = (log_q_off(g.np, L.steps, L.cap) + (size_t)L.cap * kQSlot * 8 + 255) & ~(size_t)255;
-  const size_t smem_b = (size_t)rbp * per_rb + 4 * (size_t)(g.np + 8);
+  const size_t smem_b = (size_t)rbp * per_rb + 4 * (size_t)(g.np + 8 + 4 * g.nb);
   L.smem = g.smem > smem_b ? g.smem : smem_b;
   L.ready_off = kSchedDone + 2 * L.nsolvers;
   L.fb_off = L.ready_off + batch;
