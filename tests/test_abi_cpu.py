@@ -43,6 +43,23 @@ def test_library_exports_every_declared_symbol():
         assert lib.wpcd_create(ctypes.byref(h), 0) == -4 and not h.value
 
 
+def test_static_workspace_constant_matches_the_header():
+    """wpcd_diag_batched_static: the binding's limit is the header's WPCD_STATIC_WORK_BYTES, the array is a file-scope
+    __device__ array in the .cu file that resolves its address with cudaGetSymbolAddress, and the entry point's translation
+    units call no allocator."""
+    from paper_2106_00454_b200 import wpcd
+    hdr = open(os.path.join(ROOT, "include", "wpcd.h")).read()
+    m = re.search(r"#define WPCD_STATIC_WORK_BYTES \((\d+)u << (\d+)\)", hdr)
+    assert m and (int(m.group(1)) << int(m.group(2))) == wpcd.Handle.STATIC_WORK_BYTES == 16 << 20
+    jac = open(os.path.join(ROOT, "paper_2106_00454_b200", "csrc", "jacobi.cu")).read()
+    assert "static __device__ __align__(256) unsigned char wpcd_static_work[WPCD_STATIC_WORK_BYTES];" in jac
+    assert "cudaGetSymbolAddress(&ptr, wpcd_static_work)" in jac
+    for f in ("jacobi.cu", "jacobi_small.cu", "api.cu"):
+        src = open(os.path.join(ROOT, "paper_2106_00454_b200", "csrc", f)).read()
+        src = re.sub(r"//.*", "", src)
+        assert not re.search(r"\bcuda(Malloc\w*|Free\w*|HostAlloc)\s*\(", src), f
+
+
 def test_input_recipe():
     p = inp.grid_edges(100)
     assert len(p) == 101 and p[0] == 0 and abs(p[100] - 127.96) < 0.01 and np.all(np.diff(p) > 0)
