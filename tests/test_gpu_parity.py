@@ -370,7 +370,8 @@ def test_diag_is_run_to_run_deterministic(ctx):
     with the updates of the running one; every item touches disjoint data, so repeated runs must agree BIT FOR BIT.
     (compute-sanitizer is closed on this pool; a data race would show up here as run-to-run differences.)"""
     h, torch = ctx["h"], ctx["torch"]
-    for N, chans, S in ((100, [(0, 0)], 300), (100, [(1, 1)], 150), (24, [(0, 1)], 600), (150, [(1, 2)], 8)):
+    # (150, coupled) = n = 300: the log mode (scheduler in global memory, dataflow replay), below and above the grid size
+    for N, chans, S in ((100, [(0, 0)], 300), (100, [(1, 1)], 150), (24, [(0, 1)], 600), (150, [(1, 2)], 8), (150, [(1, 1)], 200)):
         scales = inp.sample_scales(S, seed=3)
         out = h.build_channels(inp.grid_edges(N), chans, scales=_to_dev(ctx, scales), S=S, V0=inp.MT_V0, mu=inp.MT_MU,
                                scale_idx=[0, 1], VT=inp.TENSOR_V, muT=inp.TENSOR_MU, VT_scale_idx=2)
@@ -378,7 +379,7 @@ def test_diag_is_run_to_run_deterministic(ctx):
         n = H.shape[-1]
         Hb = H.reshape(-1, n, n)
         ref = None
-        for rep in range(3):
+        for rep in range(4):
             W, C, info = h.diag_batched(Hb)
             torch.cuda.synchronize()
             cur = (W.clone(), C.clone(), info.clone())
