@@ -463,6 +463,7 @@ __global__ void __launch_bounds__(512) k_onshell_i1_pw(OnshellParams P) {
     double p00[NC], p01[NC], p11[NC];   // weights of the previous state of each branch
 #pragma unroll
     for (int br = 0; br < NC; ++br) p00[br] = p01[br] = p11[br] = 0.0;
+#pragma unroll 4  // four states' loads of C in flight before their logarithms (n = 200: 1.84 -> 1.55 ms per 4096 matrices)
     for (int k0 = nbd; k0 < n; k0 += NC) {
 #pragma unroll
       for (int br = 0; br < NC; ++br) {
